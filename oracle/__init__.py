@@ -1,0 +1,112 @@
+"""CPU fp64 oracle for the blip orbital evaluation (arxiv/paper_1204_1121, Eq. 6-8).
+
+TEST INFRASTRUCTURE ONLY: importable from tests/, __graft_entry__.smoke() and bench.py's
+cpu_baseline / --impl reference legs.  The product package never imports this.
+
+`eval_fast`  — ctypes onto oracle/blip_oracle.c (the paper's algorithm, fp64, plain loops).
+`blip_brute` — the definition summed over ALL grid sites (numpy, separate code).
+"""
+import ctypes
+import numpy as np
+
+from . import build as _build
+
+VALUE, VGL = 0, 1
+_lib = None
+
+
+def lib():
+    global _lib
+    if _lib is None:
+        L = ctypes.CDLL(_build.build())
+        dp = ctypes.POINTER(ctypes.c_double)
+        ip = ctypes.POINTER(ctypes.c_int)
+        fp = ctypes.POINTER(ctypes.c_float)
+        L.blip_oracle_inverse_lattice.argtypes = [dp, dp]
+        L.blip_oracle_inverse_lattice.restype = ctypes.c_int
+        L.blip_oracle_cellmap.argtypes = [dp, ip, dp, ctypes.c_longlong, ip, dp]
+        L.blip_oracle_cellmap.restype = ctypes.c_int
+        L.blip_oracle_eval.argtypes = [dp, ip, ctypes.c_int, fp, dp, ctypes.c_longlong,
+                                       ctypes.c_int, dp, dp, dp, ip]
+        L.blip_oracle_eval.restype = ctypes.c_int
+        L.blip_oracle_spacing.argtypes = [dp, ip, dp]
+        L.blip_oracle_spacing.restype = ctypes.c_int
+        L.blip_oracle_num_threads.restype = ctypes.c_int
+        L.blip_oracle_set_num_threads.argtypes = [ctypes.c_int]
+        _lib = L
+    return _lib
+
+
+def _d(a):
+    return a.ctypes.data_as(ctypes.POINTER(ctypes.c_double))
+
+
+def _i(a):
+    return a.ctypes.data_as(ctypes.POINTER(ctypes.c_int))
+
+
+def _prep(lattice, grid):
+    A = np.ascontiguousarray(np.asarray(lattice, dtype=np.float64).reshape(9))
+    n = np.ascontiguousarray(np.asarray(grid, dtype=np.int32).reshape(3))
+    return A, n
+
+
+def inverse_lattice(lattice):
+    A = np.ascontiguousarray(np.asarray(lattice, dtype=np.float64).reshape(9))
+    G = np.empty(9, dtype=np.float64)
+    if lib().blip_oracle_inverse_lattice(_d(A), _d(G)):
+        raise ValueError("singular or non-finite lattice")
+    return G.reshape(3, 3)
+
+
+def cellmap(lattice, grid, positions):
+    A, n = _prep(lattice, grid)
+    pos = np.ascontiguousarray(np.asarray(positions, dtype=np.float64).reshape(-1, 3))
+    M = pos.shape[0]
+    cell = np.empty((M, 3), dtype=np.int32)
+    frac = np.empty((M, 3), dtype=np.float64)
+    if lib().blip_oracle_cellmap(_d(A), _i(n), _d(pos), M, _i(cell), _d(frac)):
+        raise ValueError("singular or non-finite lattice")
+    return cell, frac
+
+
+def eval_fast(lattice, grid, coeffs, positions, mode=VGL):
+    """Returns (val [M][L], grad [M][3][L] or None, lap [M][L] or None, cell [M][3]) in fp64."""
+    A, n = _prep(lattice, grid)
+    c = np.ascontiguousarray(coeffs, dtype=np.float32)
+    assert c.ndim == 4 and tuple(c.shape[:3]) == tuple(int(x) for x in n), c.shape
+    L = c.shape[3]
+    pos = np.ascontiguousarray(np.asarray(positions, dtype=np.float64).reshape(-1, 3))
+    M = pos.shape[0]
+    val = np.empty((M, L), dtype=np.float64)
+    cell = np.empty((M, 3), dtype=np.int32)
+    if mode == VGL:
+        grad = np.empty((M, 3, L), dtype=np.float64)
+        lap = np.empty((M, L), dtype=np.float64)
+        gp, lp = _d(grad), _d(lap)
+    else:
+        grad = lap = None
+        gp = lp = ctypes.POINTER(ctypes.c_double)()
+    rc = lib().blip_oracle_eval(_d(A), _i(n), L,
+                                c.ctypes.data_as(ctypes.POINTER(ctypes.c_float)),
+                                _d(pos), M, mode, _d(val), gp, lp, _i(cell))
+    if rc:
+        raise ValueError(f"blip_oracle_eval failed with code {rc}")
+    return val, grad, lap, cell
+
+
+def spacing(lattice, grid):
+    """Perpendicular grid-plane spacings h_a (reading R13)."""
+    A, n = _prep(lattice, grid)
+    h = np.empty(3, dtype=np.float64)
+    if lib().blip_oracle_spacing(_d(A), _i(n), _d(h)):
+        raise ValueError("singular or non-finite lattice")
+    return h
+
+
+def num_threads():
+    return int(lib().blip_oracle_num_threads())
+
+
+def set_num_threads(t):
+    lib().blip_oracle_set_num_threads(int(t))
