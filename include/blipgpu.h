@@ -1,0 +1,145 @@
+/*
+ * blipgpu.h — C ABI of the B200 (sm_100a) blip orbital evaluator.
+ *
+ * The one operation behind this boundary is the bottleneck of arxiv/paper_1204_1121
+ * (Uejima & Maezono, "GPGPU for orbital function evaluation with a new updating scheme"):
+ *
+ *     psi_l(r_j) = sum_{s=1..64} a_{l,s(r_j)} * Theta_s(r_j)                     (Eq. 6)
+ *     Theta_s(r) = phi((x-X_s)/b_x) phi((y-Y_s)/b_y) phi((z-Z_s)/b_z)            (Eq. 7)
+ *
+ * for every orbital l and every electron position r_j of a batch, the 64 sites s(r_j) being
+ * the 4x4x4 block of the periodic coefficient grid around r_j (Eq. 8), plus
+ * the Cartesian gradient and Laplacian of psi_l (needed by the local-energy call,
+ * PAPER.md:124; BASELINE.json north_star).  The coefficient table is loaded once and stays
+ * resident on the device; one call evaluates a batch of M positions,
+ * which stands in for the paper's quasi-simultaneous update of all N electrons
+ * (Eq. 11-12).
+ *
+ * Conventions: phi is the cardinal cubic B-spline (weights sum to 1);
+ * lattice A is 3x3 row-major with row a = lattice vector a (bohr); fractional u = r.A^-1;
+ * grid coordinate t_a = n_a u_a; the 4 sites along axis a are floor(t_a)-1 .. floor(t_a)+2,
+ * periodic; coefficient c[k1][k2][k3][l] sits at grid point (k1,k2,k3), orbital index l
+ * innermost ("l ... sequential memory access").
+ *
+ * Every pointer argument says HOST or DEVICE.  Nothing throws; every call returns a code.
+ * There is no CPU fallback: without a CUDA device of compute capability 10.x the library
+ * fails with BLIPGPU_EARCH / BLIPGPU_ECUDA.
+ */
+#ifndef BLIPGPU_H
+#define BLIPGPU_H
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct blipgpu_table blipgpu_table;       /* opaque handle: table + workspace */
+
+/* mode */
+#define BLIPGPU_VALUE 0                           /* psi only                              */
+#define BLIPGPU_VGL   1                           /* psi, Cartesian gradient, Laplacian    */
+
+/* return codes */
+#define BLIPGPU_OK       0
+#define BLIPGPU_EINVAL  (-1)                      /* bad argument (see each call)          */
+#define BLIPGPU_ENOMEM  (-2)                      /* host or device allocation failed      */
+#define BLIPGPU_ECUDA   (-3)                      /* CUDA runtime error: blipgpu_last_cuda_error */
+#define BLIPGPU_EARCH   (-4)                      /* current device is not sm_100 class    */
+
+/*
+ * blipgpu_create — load a coefficient table onto the current CUDA device.
+ * ("precomputed ... stored in memory at the beginning of the simulation".)
+ *
+ *   lattice   HOST  [9]   row-major, row a = lattice vector a (bohr); |det| must be finite, non-zero
+ *   grid      HOST  [3]   n1,n2,n3 grid points per axis, each >= 4 (fewer would alias the 4 sites)
+ *   norb            L >= 1 real orbitals; a complex orbital is two adjacent real channels
+ *   coeffs    HOST or DEVICE  [n1][n2][n3][L] fp32, C order, l innermost; n1*n2*n3 < 2^31
+ *   coeffs_on_device      0: `coeffs` is a host pointer; 1: a device pointer
+ *   stream    cudaStream_t (as void*), may be NULL; the copy is ordered on it and the call
+ *             returns only after the copy has completed (the caller's buffer is not retained)
+ *   out       HOST  receives the handle
+ *
+ * Ownership: the library keeps its own device copy (row pitch padded to a multiple of 4
+ * floats); the caller may free `coeffs` on return.  Errors: EINVAL (NULL pointer, n_a < 4,
+ * L < 1, singular / non-finite lattice, too many grid points), EARCH, ENOMEM, ECUDA.
+ */
+int blipgpu_create(const double* lattice, const int* grid, int norb, const float* coeffs,
+                   int coeffs_on_device, void* stream, blipgpu_table** out);
+
+/*
+ * blipgpu_eval — evaluate all L orbitals at M positions (steps a-1..a-5 of SURVEY.md §8a:
+ * cell map, per-axis weights, 64-row gather + FMA, grouping, output), asynchronously on
+ * `stream`.  No host synchronisation, no host<->device copy inside.
+ *
+ *   positions DEVICE [M][3] fp64 Cartesian (bohr); any finite value (wrapped into the cell)
+ *   M               >= 0; M == 0 returns OK without launching anything
+ *   mode            BLIPGPU_VALUE or BLIPGPU_VGL
+ *   val       DEVICE [M][ld]      fp32 out, required            val[j][l]     = psi_l(r_j)
+ *   grad      DEVICE [M][3][ld]   fp32 out, required iff VGL    grad[j][i][l] = d psi_l / d r_i
+ *   lap       DEVICE [M][ld]      fp32 out, required iff VGL    lap[j][l]     = nabla^2 psi_l
+ *   ld              row pitch in floats: ld >= L and ld % 4 == 0.  Columns L..ld-1 are
+ *                   padding; up to the next multiple of 4 they may be overwritten
+ *   cell      DEVICE [M][3] int32 out, optional (NULL ok): floor(t_a) in [0,n_a) of step a-1
+ *   stream    cudaStream_t (as void*), may be NULL
+ *
+ * Results are in the caller's position order whatever internal grouping is used.  A
+ * non-finite position gives NaN outputs and cell = -1 for that position (no error code:
+ * detecting it would need a synchronisation).  Output pointers must be 16-byte aligned.
+ * One handle serves one stream at a time (it owns the grouping workspace); if the
+ * workspace must grow the call synchronises `stream` once — blipgpu_reserve avoids that.
+ * Errors: EINVAL (NULL required pointer, M < 0, unknown mode, bad ld, misaligned output),
+ * ENOMEM, ECUDA.
+ */
+int blipgpu_eval(blipgpu_table* t, const double* positions, long long M, int mode,
+                 float* val, float* grad, float* lap, long long ld, int* cell, void* stream);
+
+/*
+ * blipgpu_eval_host — the same evaluation with HOST buffers: the paper's per-step data flow
+ * (trial positions host->device, orbital values device->host; Fig. 4,
+ * 336-343 Table XI).  Copies positions in, evaluates batch by batch and copies results out,
+ * overlapping the device->host copies of one batch with the evaluation of the next; returns
+ * after everything has landed (synchronises `stream`).  Pinned host buffers make the copies
+ * asynchronous; pageable ones work but serialise.
+ *
+ *   positions HOST [M][3] fp64;  val/grad/lap HOST, shapes and `ld` as in blipgpu_eval
+ *   (no alignment requirement);  cell HOST [M][3] int32, optional.
+ */
+int blipgpu_eval_host(blipgpu_table* t, const double* positions, long long M, int mode,
+                      float* val, float* grad, float* lap, long long ld, int* cell, void* stream);
+
+/* blipgpu_reserve — pre-size the grouping workspace for batches of up to M_max positions
+ * (and the staging buffers of blipgpu_eval_host).  Optional.  Errors: EINVAL, ENOMEM, ECUDA. */
+int blipgpu_reserve(blipgpu_table* t, long long M_max);
+
+/* blipgpu_destroy — free the table and workspace.  destroy(NULL) is a no-op returning OK. */
+int blipgpu_destroy(blipgpu_table* t);
+
+/* blipgpu_info — HOST out: grid[3], norb, internal row pitch (floats), table bytes on device.
+ * Any out pointer may be NULL. */
+int blipgpu_info(const blipgpu_table* t, int* grid, int* norb, long long* pitch,
+                 long long* table_bytes);
+
+/* blipgpu_launch_count — number of kernels this handle has launched since creation (the
+ * benchmark's "gpu_launches" evidence).  */
+long long blipgpu_launch_count(const blipgpu_table* t);
+
+/* blipgpu_set_profiling — on != 0: every following blipgpu_eval also records CUDA events on
+ * its stream at the start of the call, before and after the gather+FMA kernel (no
+ * synchronisation is added).  Off by default. */
+int blipgpu_set_profiling(blipgpu_table* t, int on);
+
+/* blipgpu_last_kernel_ms — waits for the last profiled blipgpu_eval and returns the device
+ * time (ms) of its grouping kernels (step a-4) and of its gather+FMA kernel (steps a-1..a-3,
+ * a-5).  HOST out pointers, either may be NULL.  EINVAL if profiling is off or nothing ran. */
+int blipgpu_last_kernel_ms(blipgpu_table* t, float* group_ms, float* eval_ms);
+
+/* blipgpu_strerror — static string for a return code. */
+const char* blipgpu_strerror(int code);
+
+/* blipgpu_last_cuda_error — the cudaError_t (as int) behind the last BLIPGPU_ECUDA of this
+ * handle; with t == NULL, of the last failed blipgpu_create on this thread. */
+int blipgpu_last_cuda_error(const blipgpu_table* t);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* BLIPGPU_H */

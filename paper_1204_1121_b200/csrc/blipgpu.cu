@@ -1,0 +1,358 @@
+// blipgpu.cu — host side of the C ABI declared in include/blipgpu.h (product path).
+// Argument checking, the fp64 inverse lattice, device memory and kernel launches; every
+// step of the hot path itself runs in the kernels of blip_kernels.cuh.
+#include "blipgpu.h"
+#include "blip_kernels.cuh"
+
+#include <cmath>
+#include <cstdlib>
+#include <cstring>
+#include <new>
+
+struct blipgpu_table {
+    blip::Geom g;
+    int L = 0;
+    long long pitch = 0;             // floats per table row (multiple of 4)
+    long long nrows = 0;
+    float4* table = nullptr;         // device, [nrows][pitch/4]
+    int nbins = 0;
+    // grouping workspace (device)
+    long long cap = 0;               // electrons the workspace holds
+    int* bin = nullptr;              // [cap]
+    int* perm = nullptr;             // [cap]
+    unsigned* hist = nullptr;        // [nbins]
+    // staging for blipgpu_eval_host (device)
+    long long hcap = 0, hld = 0; int hmode = -1;
+    double* d_pos = nullptr; float* d_val = nullptr; float* d_grad = nullptr; float* d_lap = nullptr;
+    int* d_cell = nullptr;
+    cudaStream_t copy_stream = nullptr;
+    cudaEvent_t ev[2] = {nullptr, nullptr};
+    cudaEvent_t ev_in = nullptr;
+    // optional timing of the kernels of the last blipgpu_eval (blipgpu_set_profiling)
+    int profiling = 0;
+    cudaEvent_t pe[3] = {nullptr, nullptr, nullptr};   // call start, eval kernel start, end
+    int last_cuda = 0;
+    long long launches = 0;
+};
+
+static thread_local int g_create_cuda_error = 0;
+
+#define CK(t, call)                                                        \
+    do {                                                                   \
+        cudaError_t e_ = (call);                                           \
+        if (e_ != cudaSuccess) {                                           \
+            (t)->last_cuda = (int)e_;                                      \
+            (void)cudaGetLastError();                                      \
+            return e_ == cudaErrorMemoryAllocation ? BLIPGPU_ENOMEM : BLIPGPU_ECUDA; \
+        }                                                                  \
+    } while (0)
+
+// Inverse lattice by cofactors, G = adj(A)/det — the pinned fp64 sequence of DESIGN.md
+// "Index map" (each cofactor p*q - r*s, det = (A00 C00 + A01 C01) + A02 C02, true division).
+// Compiled with -ffp-contract=off on the host side.
+static bool inverse_lattice(const double* A, double* G)
+{
+    double C[3][3];
+    for (int i = 0; i < 3; ++i) {
+        const int i1 = (i + 1) % 3, i2 = (i + 2) % 3;
+        for (int j = 0; j < 3; ++j) {
+            const int j1 = (j + 1) % 3, j2 = (j + 2) % 3;
+            // cyclic form of the cofactor: sign is absorbed by the index rotation
+            C[i][j] = A[3 * i1 + j1] * A[3 * i2 + j2] - A[3 * i1 + j2] * A[3 * i2 + j1];
+        }
+    }
+    const double det = (A[0] * C[0][0] + A[1] * C[0][1]) + A[2] * C[0][2];
+    if (!(det != 0.0) || !std::isfinite(det)) return false;
+    for (int i = 0; i < 3; ++i)
+        for (int j = 0; j < 3; ++j) G[3 * i + j] = C[j][i] / det;
+    for (int k = 0; k < 9; ++k)
+        if (!std::isfinite(G[k])) return false;
+    return true;
+}
+
+static int ensure_workspace(blipgpu_table* t, long long M, cudaStream_t s)
+{
+    if (M <= t->cap) return BLIPGPU_OK;
+    CK(t, cudaStreamSynchronize(s));
+    if (t->bin) cudaFree(t->bin);
+    if (t->perm) cudaFree(t->perm);
+    t->bin = t->perm = nullptr; t->cap = 0;
+    CK(t, cudaMalloc(&t->bin, sizeof(int) * (size_t)M));
+    CK(t, cudaMalloc(&t->perm, sizeof(int) * (size_t)M));
+    t->cap = M;
+    return BLIPGPU_OK;
+}
+
+extern "C" int blipgpu_create(const double* lattice, const int* grid, int norb,
+                              const float* coeffs, int coeffs_on_device, void* stream,
+                              blipgpu_table** out)
+{
+    g_create_cuda_error = 0;
+    if (!lattice || !grid || !coeffs || !out) return BLIPGPU_EINVAL;
+    *out = nullptr;
+    if (norb < 1 || grid[0] < 4 || grid[1] < 4 || grid[2] < 4) return BLIPGPU_EINVAL;
+    for (int k = 0; k < 9; ++k)
+        if (!std::isfinite(lattice[k])) return BLIPGPU_EINVAL;
+    const long long nrows = (long long)grid[0] * grid[1] * grid[2];
+    if (nrows >= (1LL << 31)) return BLIPGPU_EINVAL;
+
+    int dev = 0;
+    cudaError_t ce = cudaGetDevice(&dev);
+    cudaDeviceProp prop;
+    if (ce == cudaSuccess) ce = cudaGetDeviceProperties(&prop, dev);
+    if (ce != cudaSuccess) { g_create_cuda_error = (int)ce; (void)cudaGetLastError(); return BLIPGPU_ECUDA; }
+    if (prop.major != 10) return BLIPGPU_EARCH;      // sm_100a code only; no fallback
+
+    blipgpu_table* t = new (std::nothrow) blipgpu_table();
+    if (!t) return BLIPGPU_ENOMEM;
+    if (!inverse_lattice(lattice, t->g.G)) { delete t; return BLIPGPU_EINVAL; }
+    double Jd[3][3];
+    for (int a = 0; a < 3; ++a) {
+        t->g.n[a] = grid[a];
+        t->g.nb[a] = (grid[a] + blip::kBrick - 1) / blip::kBrick;
+        for (int i = 0; i < 3; ++i) {
+            Jd[a][i] = (double)grid[a] * t->g.G[3 * i + a];
+            t->g.J[3 * a + i] = (float)Jd[a][i];
+        }
+    }
+    const int qa[6] = {0, 1, 2, 0, 0, 1}, qb[6] = {0, 1, 2, 1, 2, 2};
+    for (int k = 0; k < 6; ++k)
+        t->g.Q[k] = (float)(Jd[qa[k]][0] * Jd[qb[k]][0] + Jd[qa[k]][1] * Jd[qb[k]][1]
+                            + Jd[qa[k]][2] * Jd[qb[k]][2]);
+    t->L = norb;
+    t->pitch = ((long long)norb + 3) / 4 * 4;
+    t->nrows = nrows;
+    t->g.L = norb;
+    t->g.pitch4 = (int)(t->pitch / 4);
+    t->nbins = t->g.nb[0] * t->g.nb[1] * t->g.nb[2];
+
+    cudaStream_t s = (cudaStream_t)stream;
+    int rc = BLIPGPU_OK;
+    auto fail = [&](cudaError_t e) {
+        g_create_cuda_error = (int)e; (void)cudaGetLastError();
+        rc = (e == cudaErrorMemoryAllocation) ? BLIPGPU_ENOMEM : BLIPGPU_ECUDA;
+    };
+    cudaError_t e;
+    const size_t bytes = (size_t)nrows * (size_t)t->pitch * sizeof(float);
+    if ((e = cudaMalloc(&t->table, bytes)) != cudaSuccess) fail(e);
+    if (rc == BLIPGPU_OK && (e = cudaMalloc(&t->hist, sizeof(unsigned) * (size_t)t->nbins)) != cudaSuccess) fail(e);
+    if (rc == BLIPGPU_OK) {
+        const cudaMemcpyKind kind = coeffs_on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice;
+        if (t->pitch == norb) {
+            e = cudaMemcpyAsync(t->table, coeffs, bytes, kind, s);
+        } else {
+            e = cudaMemsetAsync(t->table, 0, bytes, s);          // zero the pad columns
+            if (e == cudaSuccess)
+                e = cudaMemcpy2DAsync(t->table, (size_t)t->pitch * sizeof(float), coeffs,
+                                      (size_t)norb * sizeof(float), (size_t)norb * sizeof(float),
+                                      (size_t)nrows, kind, s);
+        }
+        if (e == cudaSuccess) e = cudaStreamSynchronize(s);
+        if (e != cudaSuccess) fail(e);
+    }
+    if (rc == BLIPGPU_OK && (e = cudaStreamCreateWithFlags(&t->copy_stream, cudaStreamNonBlocking)) != cudaSuccess) fail(e);
+    for (int k = 0; k < 2 && rc == BLIPGPU_OK; ++k)
+        if ((e = cudaEventCreateWithFlags(&t->ev[k], cudaEventDisableTiming)) != cudaSuccess) fail(e);
+    if (rc == BLIPGPU_OK && (e = cudaEventCreateWithFlags(&t->ev_in, cudaEventDisableTiming)) != cudaSuccess) fail(e);
+    if (rc != BLIPGPU_OK) { blipgpu_destroy(t); return rc; }
+    *out = t;
+    return BLIPGPU_OK;
+}
+
+extern "C" int blipgpu_destroy(blipgpu_table* t)
+{
+    if (!t) return BLIPGPU_OK;
+    cudaFree(t->table); cudaFree(t->bin); cudaFree(t->perm); cudaFree(t->hist);
+    cudaFree(t->d_pos); cudaFree(t->d_val); cudaFree(t->d_grad); cudaFree(t->d_lap); cudaFree(t->d_cell);
+    if (t->copy_stream) cudaStreamDestroy(t->copy_stream);
+    for (int k = 0; k < 2; ++k) if (t->ev[k]) cudaEventDestroy(t->ev[k]);
+    for (int k = 0; k < 3; ++k) if (t->pe[k]) cudaEventDestroy(t->pe[k]);
+    if (t->ev_in) cudaEventDestroy(t->ev_in);
+    (void)cudaGetLastError();
+    delete t;
+    return BLIPGPU_OK;
+}
+
+static int check_eval_args(const blipgpu_table* t, const double* positions, long long M, int mode,
+                           const float* val, const float* grad, const float* lap, long long ld)
+{
+    if (!t || M < 0) return BLIPGPU_EINVAL;
+    if (mode != BLIPGPU_VALUE && mode != BLIPGPU_VGL) return BLIPGPU_EINVAL;
+    if (ld < t->L || (ld % 4) != 0) return BLIPGPU_EINVAL;
+    if (M == 0) return BLIPGPU_OK;
+    if (!positions || !val) return BLIPGPU_EINVAL;
+    if (mode == BLIPGPU_VGL && (!grad || !lap)) return BLIPGPU_EINVAL;
+    return BLIPGPU_OK;
+}
+
+// Batches of at most this many electrons are evaluated in caller order: every electron of
+// the batch is in flight at once, so grouping cannot improve locality and costs 3 launches.
+static const long long kGroupThreshold = 2048;
+
+static int launch_eval(blipgpu_table* t, const double* positions, long long M, int mode,
+                       float* val, float* grad, float* lap, long long ld, int* cell,
+                       cudaStream_t s)
+{
+    const int* perm = nullptr;
+    if (t->profiling) CK(t, cudaEventRecord(t->pe[0], s));
+    if (M > kGroupThreshold) {
+        int rc = ensure_workspace(t, M, s);
+        if (rc != BLIPGPU_OK) return rc;
+        CK(t, cudaMemsetAsync(t->hist, 0, sizeof(unsigned) * (size_t)t->nbins, s));
+        const unsigned nb = (unsigned)((M + 255) / 256);
+        blip::bin_kernel<<<nb, 256, 0, s>>>(t->g, positions, M, t->bin, t->hist, cell);
+        blip::scan_kernel<<<1, blip::kScanThreads, 0, s>>>(t->hist, t->nbins);
+        blip::scatter_kernel<<<nb, 256, 0, s>>>(t->bin, t->hist, M, t->perm);
+        t->launches += 3;
+        perm = t->perm;
+        cell = nullptr;                                  // already written by bin_kernel
+    }
+    const dim3 grid((unsigned)((M + blip::kWarpsPerBlock - 1) / blip::kWarpsPerBlock),
+                    (unsigned)((t->g.pitch4 + 31) / 32));
+    const dim3 block(blip::kWarpsPerBlock * 32);
+    if (t->profiling) CK(t, cudaEventRecord(t->pe[1], s));
+    if (mode == BLIPGPU_VALUE)
+        blip::eval_kernel<0><<<grid, block, 0, s>>>(t->g, t->table, positions, perm, M,
+                                                    val, grad, lap, ld, cell);
+    else
+        blip::eval_kernel<1><<<grid, block, 0, s>>>(t->g, t->table, positions, perm, M,
+                                                    val, grad, lap, ld, cell);
+    t->launches += 1;
+    CK(t, cudaGetLastError());
+    if (t->profiling) CK(t, cudaEventRecord(t->pe[2], s));
+    return BLIPGPU_OK;
+}
+
+extern "C" int blipgpu_eval(blipgpu_table* t, const double* positions, long long M, int mode,
+                            float* val, float* grad, float* lap, long long ld, int* cell,
+                            void* stream)
+{
+    int rc = check_eval_args(t, positions, M, mode, val, grad, lap, ld);
+    if (rc != BLIPGPU_OK || M == 0) return rc;
+    if (((uintptr_t)val & 15) || (mode == BLIPGPU_VGL && (((uintptr_t)grad & 15) || ((uintptr_t)lap & 15))))
+        return BLIPGPU_EINVAL;
+    if (M >= (1LL << 31)) return BLIPGPU_EINVAL;
+    return launch_eval(t, positions, M, mode, val, grad, lap, ld, cell, (cudaStream_t)stream);
+}
+
+extern "C" int blipgpu_reserve(blipgpu_table* t, long long M_max)
+{
+    if (!t || M_max < 0 || M_max >= (1LL << 31)) return BLIPGPU_EINVAL;
+    if (M_max == 0) return BLIPGPU_OK;
+    return ensure_workspace(t, M_max, nullptr);
+}
+
+// Staging buffers of blipgpu_eval_host: full-batch device copies of positions and outputs.
+static int ensure_host_staging(blipgpu_table* t, long long M, int mode, long long ld, bool want_cell,
+                               cudaStream_t s)
+{
+    const bool fits = M <= t->hcap && ld == t->hld && (mode <= t->hmode) && (!want_cell || t->d_cell);
+    if (fits) return BLIPGPU_OK;
+    CK(t, cudaStreamSynchronize(s));
+    CK(t, cudaStreamSynchronize(t->copy_stream));
+    cudaFree(t->d_pos); cudaFree(t->d_val); cudaFree(t->d_grad); cudaFree(t->d_lap); cudaFree(t->d_cell);
+    t->d_pos = nullptr; t->d_val = t->d_grad = t->d_lap = nullptr; t->d_cell = nullptr;
+    t->hcap = 0; t->hmode = -1;
+    const long long cap = M > t->hcap ? M : t->hcap;
+    CK(t, cudaMalloc(&t->d_pos, sizeof(double) * 3 * (size_t)cap));
+    CK(t, cudaMalloc(&t->d_val, sizeof(float) * (size_t)cap * (size_t)ld));
+    if (mode == BLIPGPU_VGL) {
+        CK(t, cudaMalloc(&t->d_grad, sizeof(float) * 3 * (size_t)cap * (size_t)ld));
+        CK(t, cudaMalloc(&t->d_lap, sizeof(float) * (size_t)cap * (size_t)ld));
+    }
+    CK(t, cudaMalloc(&t->d_cell, sizeof(int) * 3 * (size_t)cap));
+    t->hcap = cap; t->hld = ld; t->hmode = mode;
+    return BLIPGPU_OK;
+}
+
+extern "C" int blipgpu_eval_host(blipgpu_table* t, const double* positions, long long M, int mode,
+                                 float* val, float* grad, float* lap, long long ld, int* cell,
+                                 void* stream)
+{
+    int rc = check_eval_args(t, positions, M, mode, val, grad, lap, ld);
+    if (rc != BLIPGPU_OK || M == 0) return rc;
+    if (M >= (1LL << 31)) return BLIPGPU_EINVAL;
+    cudaStream_t s = (cudaStream_t)stream;
+    rc = ensure_host_staging(t, M, mode, ld, cell != nullptr, s);
+    if (rc != BLIPGPU_OK) return rc;
+    CK(t, cudaMemcpyAsync(t->d_pos, positions, sizeof(double) * 3 * (size_t)M, cudaMemcpyHostToDevice, s));
+    // Batches: evaluate batch b on `s`, then copy its results out on the copy stream while
+    // batch b+1 is evaluated (the device->host copy of psi is the largest transfer in the
+    // paper's Table XI).
+    const long long B = 8192;
+    long long b0 = 0; int k = 0;
+    while (b0 < M) {
+        const long long nb = (M - b0 < B) ? (M - b0) : B;
+        rc = launch_eval(t, t->d_pos + 3 * b0, nb, mode, t->d_val + b0 * ld,
+                         mode == BLIPGPU_VGL ? t->d_grad + 3 * b0 * ld : nullptr,
+                         mode == BLIPGPU_VGL ? t->d_lap + b0 * ld : nullptr, ld,
+                         cell ? t->d_cell + 3 * b0 : nullptr, s);
+        if (rc != BLIPGPU_OK) return rc;
+        CK(t, cudaEventRecord(t->ev[k], s));
+        CK(t, cudaStreamWaitEvent(t->copy_stream, t->ev[k], 0));
+        const size_t rowb = sizeof(float) * (size_t)ld;
+        CK(t, cudaMemcpyAsync(val + b0 * ld, t->d_val + b0 * ld, rowb * (size_t)nb, cudaMemcpyDeviceToHost, t->copy_stream));
+        if (mode == BLIPGPU_VGL) {
+            CK(t, cudaMemcpyAsync(grad + 3 * b0 * ld, t->d_grad + 3 * b0 * ld, 3 * rowb * (size_t)nb, cudaMemcpyDeviceToHost, t->copy_stream));
+            CK(t, cudaMemcpyAsync(lap + b0 * ld, t->d_lap + b0 * ld, rowb * (size_t)nb, cudaMemcpyDeviceToHost, t->copy_stream));
+        }
+        if (cell)
+            CK(t, cudaMemcpyAsync(cell + 3 * b0, t->d_cell + 3 * b0, sizeof(int) * 3 * (size_t)nb, cudaMemcpyDeviceToHost, t->copy_stream));
+        b0 += nb; k ^= 1;
+    }
+    CK(t, cudaStreamSynchronize(t->copy_stream));
+    CK(t, cudaStreamSynchronize(s));
+    return BLIPGPU_OK;
+}
+
+extern "C" int blipgpu_info(const blipgpu_table* t, int* grid, int* norb, long long* pitch,
+                            long long* table_bytes)
+{
+    if (!t) return BLIPGPU_EINVAL;
+    if (grid) { grid[0] = t->g.n[0]; grid[1] = t->g.n[1]; grid[2] = t->g.n[2]; }
+    if (norb) *norb = t->L;
+    if (pitch) *pitch = t->pitch;
+    if (table_bytes) *table_bytes = t->nrows * t->pitch * (long long)sizeof(float);
+    return BLIPGPU_OK;
+}
+
+extern "C" int blipgpu_set_profiling(blipgpu_table* t, int on)
+{
+    if (!t) return BLIPGPU_EINVAL;
+    if (on)
+        for (int k = 0; k < 3; ++k)
+            if (!t->pe[k]) CK(t, cudaEventCreate(&t->pe[k]));
+    t->profiling = on ? 1 : 0;
+    return BLIPGPU_OK;
+}
+
+extern "C" int blipgpu_last_kernel_ms(blipgpu_table* t, float* group_ms, float* eval_ms)
+{
+    if (!t || !t->profiling || !t->pe[2]) return BLIPGPU_EINVAL;
+    CK(t, cudaEventSynchronize(t->pe[2]));
+    float a = 0.f, b = 0.f;
+    CK(t, cudaEventElapsedTime(&a, t->pe[0], t->pe[1]));
+    CK(t, cudaEventElapsedTime(&b, t->pe[1], t->pe[2]));
+    if (group_ms) *group_ms = a;
+    if (eval_ms) *eval_ms = b;
+    return BLIPGPU_OK;
+}
+
+extern "C" long long blipgpu_launch_count(const blipgpu_table* t) { return t ? t->launches : 0; }
+
+extern "C" const char* blipgpu_strerror(int code)
+{
+    switch (code) {
+        case BLIPGPU_OK: return "ok";
+        case BLIPGPU_EINVAL: return "invalid argument";
+        case BLIPGPU_ENOMEM: return "out of memory";
+        case BLIPGPU_ECUDA: return "CUDA runtime error (see blipgpu_last_cuda_error)";
+        case BLIPGPU_EARCH: return "device is not compute capability 10.x (sm_100a code only, no fallback)";
+        default: return "unknown blipgpu error code";
+    }
+}
+
+extern "C" int blipgpu_last_cuda_error(const blipgpu_table* t)
+{
+    return t ? t->last_cuda : g_create_cuda_error;
+}

@@ -1,0 +1,158 @@
+"""Edge cases of the CUDA path against the oracle: ragged orbital counts, padded pitch, empty
+batch, wrap-everywhere grids, grids that are not a multiple of the grouping brick, far-away
+and non-finite positions, adversarial cell-index inputs, the host-buffer entry point, and
+argument errors."""
+import ctypes
+
+import numpy as np
+import pytest
+
+import oracle
+import workloads
+from test_gpu_parity import compare, run_gpu, tolerances, torch_cuda, blip  # noqa: F401 (fixtures)
+
+pytestmark = pytest.mark.gpu
+
+TRICLINIC = ((20.0, 0.0, 0.0), (3.0, 19.0, 0.0), (2.0, 2.0, 24.0))
+SKEW = ((5.0, 0.3, -0.2), (1.1, 4.0, 0.7), (-0.6, 0.9, 6.0))
+
+
+@pytest.mark.parametrize("L", [1, 3, 5, 33, 130, 257])
+def test_ragged_orbital_counts(torch_cuda, blip, L):
+    A, c, pos = workloads.small_case((6, 5, 7), L, 300, SKEW, seed=L, spread=4.0)
+    for mode in (0, 1):
+        compare(A, (6, 5, 7), c, pos, run_gpu(torch_cuda, blip, A, (6, 5, 7), c, pos, mode=mode), mode=mode)
+
+
+def test_wider_output_pitch(torch_cuda, blip):
+    A, c, pos = workloads.small_case((8, 8, 8), 10, 100, TRICLINIC, seed=2)
+    compare(A, (8, 8, 8), c, pos, run_gpu(torch_cuda, blip, A, (8, 8, 8), c, pos, ld=24))
+
+
+def test_empty_batch(torch_cuda, blip):
+    A, c, pos = workloads.small_case((4, 4, 4), 4, 1, SKEW, seed=2)
+    t = blip.BlipTable(A, (4, 4, 4), 4, c)
+    n0 = t.launch_count()
+    val, grad, lap, cell = t.eval(torch_cuda.empty((0, 3), dtype=torch_cuda.float64, device="cuda"))
+    assert val.shape == (0, 4) and t.launch_count() == n0
+    t.close()
+
+
+@pytest.mark.parametrize("grid", [(4, 4, 4), (5, 7, 9), (4, 13, 6)])
+@pytest.mark.parametrize("M", [700, 5000])
+def test_wrap_everywhere_and_non_brick_grids(torch_cuda, blip, grid, M):
+    """4x4x4: every block of 64 sites wraps.  M = 5000 goes through the grouping path with
+    grids that are not a multiple of the 4-cell brick."""
+    A, c, pos = workloads.small_case(grid, 12, M, TRICLINIC, seed=M, spread=6.0)
+    compare(A, grid, c, pos, run_gpu(torch_cuda, blip, A, grid, c, pos))
+
+
+def test_grouped_equals_ungrouped(torch_cuda, blip):
+    """The same positions evaluated in one grouped call (M > threshold) and in small
+    ungrouped calls give bit-identical results: caller order is preserved."""
+    A, c, pos = workloads.small_case((12, 9, 10), 40, 6000, SKEW, seed=8, spread=2.0)
+    t = blip.BlipTable(A, (12, 9, 10), 40, c)
+    full = run_gpu(torch_cuda, blip, A, (12, 9, 10), c, pos, table=t)
+    for lo in range(0, 6000, 1500):
+        part = run_gpu(torch_cuda, blip, A, (12, 9, 10), c, pos[lo:lo + 1500], table=t)
+        for a, b in zip(full, part):
+            assert np.array_equal(a[lo:lo + 1500], b)
+    t.close()
+
+
+def test_non_finite_positions(torch_cuda, blip):
+    A, c, pos = workloads.small_case((6, 6, 6), 8, 3000, SKEW, seed=4)
+    bad = [0, 17, 1500, 2999]
+    pos[bad[0], 0] = np.nan
+    pos[bad[1], 1] = np.inf
+    pos[bad[2], 2] = -np.inf
+    pos[bad[3]] = np.nan
+    for M in (64, 3000):                      # ungrouped and grouped paths
+        val, grad, lap, cell = run_gpu(torch_cuda, blip, A, (6, 6, 6), c, pos[:M])
+        oval, ograd, olap, ocell = oracle.eval_fast(A, (6, 6, 6), c, pos[:M])
+        assert np.array_equal(cell, ocell)
+        nanrows = np.isnan(oval).all(axis=1)
+        assert np.array_equal(np.isnan(val).all(axis=1), nanrows)
+        assert np.isnan(grad[nanrows]).all() and np.isnan(lap[nanrows]).all()
+        good = ~nanrows
+        compare(A, (6, 6, 6), c, pos[:M][good], (val[good], grad[good], lap[good], cell[good]))
+
+
+def test_adversarial_cell_indices(torch_cuda, blip):
+    """exact grid planes, denormal and tiny negative coordinates, +-1e3 cells, 1 ulp either
+    side of a plane: GPU cell == oracle cell bit for bit."""
+    lat = ((10.0, 0, 0), (0, 10.0, 0), (0, 0, 10.0))
+    grid = (16, 16, 16)
+    ks = np.arange(-40, 41, dtype=np.float64)
+    planes = np.stack([ks * 0.625, ks * 0.625 + 0.3125, -ks * 0.625], axis=1)
+    x = 0.625 * 5
+    special = np.array([[-1e-300, 1e-300, -5e-324], [np.nextafter(x, 0), x, np.nextafter(x, 10)],
+                        [1e4 + 0.1, -1e4 - 0.1, 6250.0], [-0.0, 0.0, 10.0],
+                        [np.nextafter(10.0, 0), np.nextafter(10.0, 20), -10.0]])
+    rng = np.random.default_rng(5)
+    near = np.round(rng.random((2000, 3)) * 16) * 0.625 + rng.choice([-1, 0, 1], size=(2000, 3)) * 1e-15
+    pos = np.concatenate([planes, special, near])
+    c = workloads.coefficients(grid, 4)
+    gpu = run_gpu(torch_cuda, blip, lat, grid, c, pos)
+    compare(np.array(lat), grid, c, pos, gpu)
+    # triclinic large grid, positions within a few ulp of cell faces in fractional space
+    A = np.array(TRICLINIC)
+    g2 = (96, 96, 112)
+    u = rng.integers(0, 96, size=(3000, 3)) / np.array(g2) + rng.choice([-1, 0, 1], size=(3000, 3)) * 2e-16
+    c2 = np.zeros((*g2, 1), dtype=np.float32)
+    val, grad, lap, cell = run_gpu(torch_cuda, blip, A, g2, c2, u @ A)
+    ocell, _ = oracle.cellmap(A, g2, u @ A)
+    assert np.array_equal(cell, ocell)
+
+
+def test_eval_host_matches_eval(torch_cuda, blip):
+    torch = torch_cuda
+    A, c, pos = workloads.small_case((10, 11, 9), 37, 20000, SKEW, seed=3)
+    L, ld = 37, 40
+    t = blip.BlipTable(A, (10, 11, 9), L, c)
+    dev = run_gpu(torch, blip, A, (10, 11, 9), c, pos, table=t)
+    M = pos.shape[0]
+    hpos = torch.from_numpy(pos).pin_memory()
+    hval = torch.empty((M, ld), dtype=torch.float32).pin_memory()
+    hgrad = torch.empty((M, 3, ld), dtype=torch.float32).pin_memory()
+    hlap = torch.empty((M, ld), dtype=torch.float32).pin_memory()
+    hcell = torch.empty((M, 3), dtype=torch.int32).pin_memory()
+    blip.blipgpu_eval_host(t.handle, hpos, M, blip.VGL, hval, hgrad, hlap, ld, hcell)
+    assert np.array_equal(hval.numpy()[:, :L], dev[0])
+    assert np.array_equal(hgrad.numpy()[:, :, :L], dev[1])
+    assert np.array_equal(hlap.numpy()[:, :L], dev[2])
+    assert np.array_equal(hcell.numpy(), dev[3])
+    # pageable numpy buffers, value-only
+    nval = np.empty((M, ld), dtype=np.float32)
+    blip.blipgpu_eval_host(t.handle, pos, M, blip.VALUE, nval, None, None, ld, None)
+    assert np.array_equal(nval[:, :L], dev[0])
+    t.close()
+
+
+def test_argument_errors(torch_cuda, blip):
+    torch = torch_cuda
+    A, c, pos = workloads.small_case((4, 4, 4), 6, 8, SKEW, seed=2)
+    t = blip.BlipTable(A, (4, 4, 4), 6, c)
+    L = blip.lib()
+    dpos = torch.from_numpy(pos).cuda()
+    out = torch.empty((8, 8), dtype=torch.float32, device="cuda")
+    g = torch.empty((8, 3, 8), dtype=torch.float32, device="cuda")
+
+    def ev(M=8, mode=1, val=out, grad=g, lap=out, ld=8, p=dpos):
+        q = lambda x: ctypes.c_void_p(0 if x is None else x.data_ptr())
+        return L.blipgpu_eval(t.handle, q(p), M, mode, q(val), q(grad), q(lap), ld, None, None)
+
+    assert ev() == blip.OK
+    assert ev(M=-1) == blip.EINVAL
+    assert ev(mode=2) == blip.EINVAL
+    assert ev(ld=4) == blip.EINVAL            # ld < L
+    assert ev(ld=10) == blip.EINVAL           # ld % 4 != 0
+    assert ev(val=None) == blip.EINVAL
+    assert ev(grad=None) == blip.EINVAL
+    assert ev(p=None) == blip.EINVAL
+    assert ev(mode=0, grad=None, lap=None) == blip.OK
+    mis = out.view(-1)[1:]
+    assert L.blipgpu_eval(t.handle, ctypes.c_void_p(dpos.data_ptr()), 1, 0, ctypes.c_void_p(mis.data_ptr()),
+                          None, None, 8, None, None) == blip.EINVAL
+    torch.cuda.synchronize()
+    t.close()
