@@ -139,17 +139,30 @@ __device__ __forceinline__ int wrap_site(int k, int n)
     return k < 0 ? k + n : (k >= n ? k - n : k);
 }
 
-// Per-warp shared scratch: per-axis factors, then the 64 folded weight sets + row indices.
+// Per-warp shared scratch: per-axis factors, then the weights of the 16 (m1, m2) columns.
 struct WarpScratch {
     float ax[3][3][4];          // [axis][w, w', w''][m]
     int   k[3][4];              // wrapped site index per axis
-    float4 wg[64];              // {W, Gx, Gy, Gz} per site
-    float2 lr[64];              // {Lam, row index (int bits)} per site
+    float4 cw[16];              // column (m1,m2): {P00, P10, P01, La}  (see warp_prepare)
+    float  lb[16];              // column (m1,m2): Lb
+    int    rb[16];              // column (m1,m2): first table row of the column, (k1*n2 + k2)*n3
 };
 
-// Computes the cell, the per-axis factors and the 64 folded weights of electron `e` into
+// Computes the cell and the per-axis factors of electron `e`, then the column weights, into
 // this warp's scratch.  All 32 lanes call it.  Returns false for a non-finite position.
-template <int MODE>
+//
+// With S the spline in grid coordinates t, T_a = dS/dt_a and H_ab = d2S/dt_a dt_b, the z axis
+// (k3, contiguous table rows) is contracted first: for column (m1, m2)
+//     a = sum_m3 w3[m3] c,   b = sum_m3 w3'[m3] c,   d = sum_m3 (Q22 w3''[m3]) c
+// and the column is folded into 5 accumulators with 5 per-column weights
+//     val += P00 a                     P00 = w1 w2
+//     T1  += P10 a                     P10 = w1' w2
+//     T2  += P01 a                     P01 = w1 w2'
+//     T3  += P00 b
+//     lap += La a + Lb b + P00 d       La = Q00 w1'' w2 + Q11 w1 w2'' + 2 Q01 w1' w2'
+//                                      Lb = 2 (Q02 w1' w2 + Q12 w1 w2')
+// (lap = sum_ab Q_ab H_ab, Q = J J^T).  19 FMAs per column and orbital for any lattice; the
+// Cartesian gradient grad_i = sum_a J[a][i] T_a is formed once per orbital in the epilogue.
 __device__ __forceinline__ bool warp_prepare(const Geom& g, const double* __restrict__ pos,
                                              long long e, WarpScratch& ws, int lane,
                                              int* __restrict__ cell_out)
@@ -168,29 +181,14 @@ __device__ __forceinline__ bool warp_prepare(const Geom& g, const double* __rest
     ok = __all_sync(0xffffffffu, ok);
     __syncwarp();
     if (!ok) return false;
-#pragma unroll
-    for (int h = 0; h < 2; ++h) {
-        const int s = lane + 32 * h;
-        const int m0 = s >> 4, m1 = (s >> 2) & 3, m2 = s & 3;
-        const float a0 = ws.ax[0][0][m0], a1 = ws.ax[1][0][m1], a2 = ws.ax[2][0][m2];
-        const int row = (ws.k[0][m0] * g.n[1] + ws.k[1][m1]) * g.n[2] + ws.k[2][m2];
-        const float W = a0 * a1 * a2;
-        if (MODE == 0) {
-            ws.lr[s] = make_float2(W, __int_as_float(row));
-        } else {
-            const float b0 = ws.ax[0][1][m0], b1 = ws.ax[1][1][m1], b2 = ws.ax[2][1][m2];
-            const float c0 = ws.ax[0][2][m0], c1 = ws.ax[1][2][m1], c2 = ws.ax[2][2][m2];
-            const float a12 = a1 * a2, a02 = a0 * a2, a01 = a0 * a1;
-            const float T0 = b0 * a12, T1 = b1 * a02, T2 = b2 * a01;         // dS/dt_a weights
-            const float gx = g.J[0] * T0 + g.J[3] * T1 + g.J[6] * T2;
-            const float gy = g.J[1] * T0 + g.J[4] * T1 + g.J[7] * T2;
-            const float gz = g.J[2] * T0 + g.J[5] * T1 + g.J[8] * T2;
-            const float lam = g.Q[0] * (c0 * a12) + g.Q[1] * (c1 * a02) + g.Q[2] * (c2 * a01)
-                            + 2.0f * (g.Q[3] * (b0 * b1 * a2) + g.Q[4] * (b0 * b2 * a1)
-                                      + g.Q[5] * (b1 * b2 * a0));
-            ws.wg[s] = make_float4(W, gx, gy, gz);
-            ws.lr[s] = make_float2(lam, __int_as_float(row));
-        }
+    if (lane < 16) {
+        const int m1 = lane >> 2, m2 = lane & 3;
+        const float a0 = ws.ax[0][0][m1], b0 = ws.ax[0][1][m1], c0 = ws.ax[0][2][m1];
+        const float a1 = ws.ax[1][0][m2], b1 = ws.ax[1][1][m2], c1 = ws.ax[1][2][m2];
+        const float la = g.Q[0] * (c0 * a1) + g.Q[1] * (a0 * c1) + 2.0f * g.Q[3] * (b0 * b1);
+        ws.cw[lane] = make_float4(a0 * a1, b0 * a1, a0 * b1, la);
+        ws.lb[lane] = 2.0f * (g.Q[4] * (b0 * a1) + g.Q[5] * (a0 * b1));
+        ws.rb[lane] = (ws.k[0][m1] * g.n[1] + ws.k[1][m2]) * g.n[2];
     }
     __syncwarp();
     return true;
@@ -202,16 +200,88 @@ __device__ __forceinline__ void st_stream(float4* p, const float4& v)
                  :: "l"(p), "f"(v.x), "f"(v.y), "f"(v.z), "f"(v.w) : "memory");
 }
 
+// Packed fp32 pairs (sm_100 FFMA2 / FMUL2: two FMAs per issue slot at the same FP32-pipe
+// rate).  A pair is two consecutive orbitals; a weight is broadcast to both halves (ptxas
+// folds the {w, w} move into the instruction's scalar-operand form).
+typedef unsigned long long u64;
+__device__ __forceinline__ u64 dup2(float w)
+{
+    u64 r; asm("mov.b64 %0, {%1, %1};" : "=l"(r) : "f"(w)); return r;
+}
+__device__ __forceinline__ u64 fma2(u64 a, u64 b, u64 c)
+{
+    u64 d; asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(d) : "l"(a), "l"(b), "l"(c)); return d;
+}
+__device__ __forceinline__ u64 mul2(u64 a, u64 b)
+{
+    u64 d; asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b)); return d;
+}
+__device__ __forceinline__ float2 unpack2(u64 v)
+{
+    float2 r; asm("mov.b64 {%0, %1}, %2;" : "=f"(r.x), "=f"(r.y) : "l"(v)); return r;
+}
+
 // ---------------------------------------------------------------------------------------
-// a-3 + a-5, v0: warp = (electron, chunk of 128 orbitals), lane = 4 consecutive orbitals.
-// grid.x = groups of kWarpsPerBlock electrons in grouped order, grid.y = orbital chunk, so
-// that the CTAs in flight share one 512-byte column of the table rows (L1/L2 locality).
-// 64 x LDG.128 per lane, coalesced across the warp (l is the sequential
-// index), 5 FMAs per coefficient, streaming 128-bit stores.
+// a-3 + a-5: warp = (electron, chunk of NQ*128 orbitals); lane owns NQ quads of 4 consecutive
+// orbitals, quad q = (chunk*NQ + j)*32 + lane.  grid.x = groups of kWarpsPerBlock electrons in
+// grouped order, grid.y = orbital chunk (chunk-major launch order: the CTAs in flight share
+// one column slab of the table, which streams through L2 once).  Per column (m1, m2): 4*NQ
+// LDG.128, coalesced across the warp (l is the sequential index), prefetched
+// one column ahead of the FMAs that consume them; streaming 128-bit stores.
 // ---------------------------------------------------------------------------------------
-template <int MODE>
+template <int MODE, int NQ>
+struct EvalAcc {
+    u64 val[2 * NQ], t1[2 * NQ], t2[2 * NQ], t3[2 * NQ], lp[2 * NQ];
+};
+
+template <int NQ>
+__device__ __forceinline__ void load_column(const ulonglong2* __restrict__ table, const int (&quad)[NQ],
+                                            const Geom& g, const WarpScratch& ws, int c,
+                                            const int (&zoff)[4], ulonglong2 (&buf)[4 * NQ])
+{
+    const ulonglong2* base = table + (size_t)ws.rb[c] * (size_t)g.pitch4;
+#pragma unroll
+    for (int m = 0; m < 4; ++m)
+#pragma unroll
+        for (int j = 0; j < NQ; ++j) buf[m * NQ + j] = __ldg(base + zoff[m] + quad[j]);
+}
+
+template <int MODE, int NQ>
+__device__ __forceinline__ void fold_column(const WarpScratch& ws, int c, const float (&wz)[3][4],
+                                            const ulonglong2 (&buf)[4 * NQ], EvalAcc<MODE, NQ>& acc)
+{
+    const float4 w = ws.cw[c];
+    const float lb = ws.lb[c];
+#pragma unroll
+    for (int j = 0; j < NQ; ++j)
+#pragma unroll
+        for (int h = 0; h < 2; ++h) {
+            const u64 c0 = h ? buf[0 * NQ + j].y : buf[0 * NQ + j].x;
+            const u64 c1 = h ? buf[1 * NQ + j].y : buf[1 * NQ + j].x;
+            const u64 c2 = h ? buf[2 * NQ + j].y : buf[2 * NQ + j].x;
+            const u64 c3 = h ? buf[3 * NQ + j].y : buf[3 * NQ + j].x;
+            const int p = 2 * j + h;
+            u64 a = mul2(c0, dup2(wz[0][0]));
+            a = fma2(c1, dup2(wz[0][1]), a); a = fma2(c2, dup2(wz[0][2]), a); a = fma2(c3, dup2(wz[0][3]), a);
+            acc.val[p] = fma2(a, dup2(w.x), acc.val[p]);
+            if (MODE != 0) {
+                u64 b = mul2(c0, dup2(wz[1][0]));
+                b = fma2(c1, dup2(wz[1][1]), b); b = fma2(c2, dup2(wz[1][2]), b); b = fma2(c3, dup2(wz[1][3]), b);
+                u64 d = mul2(c0, dup2(wz[2][0]));
+                d = fma2(c1, dup2(wz[2][1]), d); d = fma2(c2, dup2(wz[2][2]), d); d = fma2(c3, dup2(wz[2][3]), d);
+                acc.t1[p] = fma2(a, dup2(w.y), acc.t1[p]);
+                acc.t2[p] = fma2(a, dup2(w.z), acc.t2[p]);
+                acc.t3[p] = fma2(b, dup2(w.x), acc.t3[p]);
+                u64 l = fma2(a, dup2(w.w), acc.lp[p]);
+                l = fma2(b, dup2(lb), l);
+                acc.lp[p] = fma2(d, dup2(w.x), l);
+            }
+        }
+}
+
+template <int MODE, int NQ>
 __global__ void __launch_bounds__(kWarpsPerBlock * 32)
-eval_kernel(Geom g, const float4* __restrict__ table, const double* __restrict__ pos,
+eval_kernel(Geom g, const float4* __restrict__ table4, const double* __restrict__ pos,
             const int* __restrict__ perm, long long M,
             float* __restrict__ val, float* __restrict__ grad, float* __restrict__ lap,
             long long ld, int* __restrict__ cell_out)
@@ -222,58 +292,72 @@ eval_kernel(Geom g, const float4* __restrict__ table, const double* __restrict__
     if (sidx >= M) return;                                   // warp-uniform; no block barrier below
     const long long e = perm ? (long long)perm[sidx] : sidx;
     WarpScratch& ws = scratch[warp];
-    const int quad = blockIdx.y * 32 + lane;
-    const bool active = quad < g.pitch4;
-    const bool ok = warp_prepare<MODE>(g, pos, e, ws, lane, blockIdx.y == 0 ? cell_out : nullptr);
+    const ulonglong2* __restrict__ table = reinterpret_cast<const ulonglong2*>(table4);
+    int quad[NQ], lquad[NQ];
+#pragma unroll
+    for (int j = 0; j < NQ; ++j) {
+        quad[j] = (blockIdx.y * NQ + j) * 32 + lane;
+        lquad[j] = min(quad[j], g.pitch4 - 1);               // lanes past the row end re-read its last quad
+    }
+    const bool ok = warp_prepare(g, pos, e, ws, lane, blockIdx.y == 0 ? cell_out : nullptr);
 
-    float4 v = make_float4(0.f, 0.f, 0.f, 0.f), gx = v, gy = v, gz = v, lp = v;
-    if (ok && active) {
-        const float4* __restrict__ col = table + quad;
-        constexpr int U = 8;
+    EvalAcc<MODE, NQ> acc;
+#pragma unroll
+    for (int p = 0; p < 2 * NQ; ++p) acc.val[p] = acc.t1[p] = acc.t2[p] = acc.t3[p] = acc.lp[p] = 0ull;
+    if (ok) {
+        float wz[3][4]; int zoff[4];
+#pragma unroll
+        for (int m = 0; m < 4; ++m) {
+            wz[0][m] = ws.ax[2][0][m]; wz[1][m] = ws.ax[2][1][m]; wz[2][m] = g.Q[2] * ws.ax[2][2][m];
+            zoff[m] = ws.k[2][m] * g.pitch4;
+        }
+        ulonglong2 buf0[4 * NQ], buf1[4 * NQ];
+        load_column<NQ>(table, lquad, g, ws, 0, zoff, buf0);
 #pragma unroll 1
-        for (int s0 = 0; s0 < 64; s0 += U) {
-            float4 c[U];
-#pragma unroll
-            for (int u = 0; u < U; ++u) {
-                const int row = __float_as_int(ws.lr[s0 + u].y);
-                c[u] = __ldg(col + (size_t)row * (size_t)g.pitch4);
-            }
-#pragma unroll
-            for (int u = 0; u < U; ++u) {
-                if (MODE == 0) {
-                    const float W = ws.lr[s0 + u].x;
-                    v.x = fmaf(W, c[u].x, v.x); v.y = fmaf(W, c[u].y, v.y);
-                    v.z = fmaf(W, c[u].z, v.z); v.w = fmaf(W, c[u].w, v.w);
-                } else {
-                    const float4 w = ws.wg[s0 + u];
-                    const float lam = ws.lr[s0 + u].x;
-                    v.x = fmaf(w.x, c[u].x, v.x); v.y = fmaf(w.x, c[u].y, v.y);
-                    v.z = fmaf(w.x, c[u].z, v.z); v.w = fmaf(w.x, c[u].w, v.w);
-                    gx.x = fmaf(w.y, c[u].x, gx.x); gx.y = fmaf(w.y, c[u].y, gx.y);
-                    gx.z = fmaf(w.y, c[u].z, gx.z); gx.w = fmaf(w.y, c[u].w, gx.w);
-                    gy.x = fmaf(w.z, c[u].x, gy.x); gy.y = fmaf(w.z, c[u].y, gy.y);
-                    gy.z = fmaf(w.z, c[u].z, gy.z); gy.w = fmaf(w.z, c[u].w, gy.w);
-                    gz.x = fmaf(w.w, c[u].x, gz.x); gz.y = fmaf(w.w, c[u].y, gz.y);
-                    gz.z = fmaf(w.w, c[u].z, gz.z); gz.w = fmaf(w.w, c[u].w, gz.w);
-                    lp.x = fmaf(lam, c[u].x, lp.x); lp.y = fmaf(lam, c[u].y, lp.y);
-                    lp.z = fmaf(lam, c[u].z, lp.z); lp.w = fmaf(lam, c[u].w, lp.w);
-                }
-            }
+        for (int c = 0; c < 16; c += 2) {
+            load_column<NQ>(table, lquad, g, ws, c + 1, zoff, buf1);
+            fold_column<MODE, NQ>(ws, c, wz, buf0, acc);
+            if (c + 2 < 16) load_column<NQ>(table, lquad, g, ws, c + 2, zoff, buf0);
+            fold_column<MODE, NQ>(ws, c + 1, wz, buf1, acc);
         }
     }
-    if (!active) return;
-    if (!ok) {
-        const float nan = __int_as_float(0x7fc00000);
-        v = make_float4(nan, nan, nan, nan); gx = gy = gz = lp = v;
-    }
-    const size_t o = (size_t)e * (size_t)ld + 4 * (size_t)quad;
-    st_stream(reinterpret_cast<float4*>(val + o), v);
-    if (MODE != 0) {
-        const size_t og = (size_t)e * 3 * (size_t)ld + 4 * (size_t)quad;
-        st_stream(reinterpret_cast<float4*>(grad + og), gx);
-        st_stream(reinterpret_cast<float4*>(grad + og + ld), gy);
-        st_stream(reinterpret_cast<float4*>(grad + og + 2 * ld), gz);
-        st_stream(reinterpret_cast<float4*>(lap + o), lp);
+    const float nan = __int_as_float(0x7fc00000);
+#pragma unroll
+    for (int j = 0; j < NQ; ++j) {
+        if (quad[j] >= g.pitch4) continue;
+        float4 v, gx, gy, gz, lp;
+        if (ok) {
+            const float2 v0 = unpack2(acc.val[2 * j]), v1 = unpack2(acc.val[2 * j + 1]);
+            v = make_float4(v0.x, v0.y, v1.x, v1.y);
+            if (MODE != 0) {
+                const float2 a0 = unpack2(acc.t1[2 * j]), a1 = unpack2(acc.t1[2 * j + 1]);
+                const float2 b0 = unpack2(acc.t2[2 * j]), b1 = unpack2(acc.t2[2 * j + 1]);
+                const float2 c0 = unpack2(acc.t3[2 * j]), c1 = unpack2(acc.t3[2 * j + 1]);
+                const float2 l0 = unpack2(acc.lp[2 * j]), l1 = unpack2(acc.lp[2 * j + 1]);
+                const float4 T1 = make_float4(a0.x, a0.y, a1.x, a1.y);
+                const float4 T2 = make_float4(b0.x, b0.y, b1.x, b1.y);
+                const float4 T3 = make_float4(c0.x, c0.y, c1.x, c1.y);
+#define BLIP_GRAD(i, out)                                                                       \
+                out.x = fmaf(g.J[i], T1.x, fmaf(g.J[3 + i], T2.x, g.J[6 + i] * T3.x));         \
+                out.y = fmaf(g.J[i], T1.y, fmaf(g.J[3 + i], T2.y, g.J[6 + i] * T3.y));         \
+                out.z = fmaf(g.J[i], T1.z, fmaf(g.J[3 + i], T2.z, g.J[6 + i] * T3.z));         \
+                out.w = fmaf(g.J[i], T1.w, fmaf(g.J[3 + i], T2.w, g.J[6 + i] * T3.w));
+                BLIP_GRAD(0, gx) BLIP_GRAD(1, gy) BLIP_GRAD(2, gz)
+#undef BLIP_GRAD
+                lp = make_float4(l0.x, l0.y, l1.x, l1.y);
+            }
+        } else {
+            v = make_float4(nan, nan, nan, nan); gx = gy = gz = lp = v;
+        }
+        const size_t o = (size_t)e * (size_t)ld + 4 * (size_t)quad[j];
+        st_stream(reinterpret_cast<float4*>(val + o), v);
+        if (MODE != 0) {
+            const size_t og = (size_t)e * 3 * (size_t)ld + 4 * (size_t)quad[j];
+            st_stream(reinterpret_cast<float4*>(grad + og), gx);
+            st_stream(reinterpret_cast<float4*>(grad + og + ld), gy);
+            st_stream(reinterpret_cast<float4*>(grad + og + 2 * ld), gz);
+            st_stream(reinterpret_cast<float4*>(lap + o), lp);
+        }
     }
 }
 

@@ -16,6 +16,7 @@ struct blipgpu_table {
     long long nrows = 0;
     float4* table = nullptr;         // device, [nrows][pitch/4]
     int nbins = 0;
+    int nq = 1;                      // quads of 4 orbitals per lane in the eval kernel (1..3)
     // grouping workspace (device)
     long long cap = 0;               // electrons the workspace holds
     int* bin = nullptr;              // [cap]
@@ -68,6 +69,17 @@ static bool inverse_lattice(const double* A, double* G)
     for (int k = 0; k < 9; ++k)
         if (!std::isfinite(G[k])) return false;
     return true;
+}
+
+// Quads per lane: a warp covers nq*128 orbitals of one electron.  Larger nq amortises the
+// per-column weight reads and address arithmetic over more FMAs at the cost of registers.
+static int default_nq(int pitch4)
+{
+    if (const char* env = std::getenv("BLIPGPU_NQ")) {
+        const int v = std::atoi(env);
+        if (v >= 1 && v <= 3) return v;
+    }
+    return pitch4 <= 32 ? 1 : 2;
 }
 
 static int ensure_workspace(blipgpu_table* t, long long M, cudaStream_t s)
@@ -125,6 +137,7 @@ extern "C" int blipgpu_create(const double* lattice, const int* grid, int norb,
     t->g.L = norb;
     t->g.pitch4 = (int)(t->pitch / 4);
     t->nbins = t->g.nb[0] * t->g.nb[1] * t->g.nb[2];
+    t->nq = default_nq(t->g.pitch4);
 
     cudaStream_t s = (cudaStream_t)stream;
     int rc = BLIPGPU_OK;
@@ -207,16 +220,20 @@ static int launch_eval(blipgpu_table* t, const double* positions, long long M, i
         perm = t->perm;
         cell = nullptr;                                  // already written by bin_kernel
     }
+    const int nq = t->nq;
     const dim3 grid((unsigned)((M + blip::kWarpsPerBlock - 1) / blip::kWarpsPerBlock),
-                    (unsigned)((t->g.pitch4 + 31) / 32));
+                    (unsigned)((t->g.pitch4 + 32 * nq - 1) / (32 * nq)));
     const dim3 block(blip::kWarpsPerBlock * 32);
     if (t->profiling) CK(t, cudaEventRecord(t->pe[1], s));
-    if (mode == BLIPGPU_VALUE)
-        blip::eval_kernel<0><<<grid, block, 0, s>>>(t->g, t->table, positions, perm, M,
-                                                    val, grad, lap, ld, cell);
-    else
-        blip::eval_kernel<1><<<grid, block, 0, s>>>(t->g, t->table, positions, perm, M,
-                                                    val, grad, lap, ld, cell);
+#define BLIP_LAUNCH(MODE, NQ)                                                                  \
+    blip::eval_kernel<MODE, NQ><<<grid, block, 0, s>>>(t->g, t->table, positions, perm, M,     \
+                                                       val, grad, lap, ld, cell)
+    if (mode == BLIPGPU_VALUE) {
+        if (nq == 1) BLIP_LAUNCH(0, 1); else if (nq == 2) BLIP_LAUNCH(0, 2); else BLIP_LAUNCH(0, 3);
+    } else {
+        if (nq == 1) BLIP_LAUNCH(1, 1); else if (nq == 2) BLIP_LAUNCH(1, 2); else BLIP_LAUNCH(1, 3);
+    }
+#undef BLIP_LAUNCH
     t->launches += 1;
     CK(t, cudaGetLastError());
     if (t->profiling) CK(t, cudaEventRecord(t->pe[2], s));
