@@ -58,9 +58,12 @@ typedef struct blipgpu_table blipgpu_table;       /* opaque handle: table + work
  *             returns only after the copy has completed (the caller's buffer is not retained)
  *   out       HOST  receives the handle
  *
- * Ownership: the library keeps its own device copy (row pitch padded to a multiple of 4
- * floats); the caller may free `coeffs` on return.  Errors: EINVAL (NULL pointer, n_a < 4,
- * L < 1, singular / non-finite lattice, too many grid points), EARCH, ENOMEM, ECUDA.
+ * Ownership: the library keeps its own device copy, re-laid-out: row pitch padded to a
+ * multiple of 4 floats and 3 periodic ghost planes per axis ((n1+3)(n2+3)(n3+3) rows), so the
+ * 4x4x4 block of any cell is a box without wrap-around; the caller may free `coeffs` on
+ * return.  A host table is staged through a temporary device buffer of its own size.
+ * Errors: EINVAL (NULL pointer, n_a < 4, L < 1, singular / non-finite lattice, too many grid
+ * points, padded table of 64 GiB or more), EARCH, ENOMEM, ECUDA.
  */
 int blipgpu_create(const double* lattice, const int* grid, int norb, const float* coeffs,
                    int coeffs_on_device, void* stream, blipgpu_table** out);
@@ -117,6 +120,14 @@ int blipgpu_destroy(blipgpu_table* t);
  * Any out pointer may be NULL. */
 int blipgpu_info(const blipgpu_table* t, int* grid, int* norb, long long* pitch,
                  long long* table_bytes);
+
+/* blipgpu_set_tuning — expert knob; the defaults are chosen from the table and batch shape.
+ *   path  0: automatic; 1: always the direct-gather kernel; 2: always the shared-memory
+ *            staged kernel (EINVAL if this table cannot use it: fewer than 128 orbitals, a grid
+ *            smaller than one staging box, or no TMA descriptor)
+ *   nq    direct kernel: quads of 4 orbitals per lane, 1..3; 0 restores the default.
+ * Both kernels compute the same arithmetic sequence; results do not depend on the choice. */
+int blipgpu_set_tuning(blipgpu_table* t, int path, int nq);
 
 /* blipgpu_launch_count — number of kernels this handle has launched since creation (the
  * benchmark's "gpu_launches" evidence).  */

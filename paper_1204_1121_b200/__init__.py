@@ -34,6 +34,7 @@ SIGNATURES = {
     "blipgpu_reserve": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_longlong]),
     "blipgpu_destroy": (ctypes.c_int, [ctypes.c_void_p]),
     "blipgpu_info": (ctypes.c_int, [ctypes.c_void_p, _c_ip, _c_ip, _c_llp, _c_llp]),
+    "blipgpu_set_tuning": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_int, ctypes.c_int]),
     "blipgpu_launch_count": (ctypes.c_longlong, [ctypes.c_void_p]),
     "blipgpu_set_profiling": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_int]),
     "blipgpu_last_kernel_ms": (ctypes.c_int, [ctypes.c_void_p, _c_fp, _c_fp]),
@@ -124,6 +125,11 @@ def blipgpu_reserve(handle, M_max):
 
 def blipgpu_destroy(handle):
     _check(lib().blipgpu_destroy(handle), "blipgpu_destroy")
+
+
+def blipgpu_set_tuning(handle, path=0, nq=0):
+    """path: 0 auto, 1 direct-gather kernel, 2 staged kernel; nq: direct kernel quads per lane (0 = default)."""
+    _check(lib().blipgpu_set_tuning(handle, int(path), int(nq)), "blipgpu_set_tuning", handle)
 
 
 def blipgpu_launch_count(handle):

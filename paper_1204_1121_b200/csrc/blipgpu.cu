@@ -9,18 +9,34 @@
 #include <cstring>
 #include <new>
 
+// Staged kernel configuration (template constants of blip::eval_staged_kernel).
+namespace {
+constexpr int kSVec = 4;             // floats per lane -> 128 orbitals per tile row
+constexpr int kSBY = 4, kSBZ = 8;    // pencil cross-section in cells
+constexpr int kSRing = 5;            // table planes resident in shared memory
+constexpr int kSWarps = 8;           // consumer warps (+1 producer warp)
+constexpr int kSSeg = 16;            // cell planes per pencil segment
+using SCfg = blip::StagedCfg<kSVec, kSBY, kSBZ, kSRing, kSWarps>;
+}
+
 struct blipgpu_table {
     blip::Geom g;
+    blip::StagedGeom sg;
     int L = 0;
     long long pitch = 0;             // floats per table row (multiple of 4)
-    long long nrows = 0;
-    float4* table = nullptr;         // device, [nrows][pitch/4]
-    int nbins = 0;
-    int nq = 1;                      // quads of 4 orbitals per lane in the eval kernel (1..3)
+    long long nrows = 0;             // rows of the padded table, (n1+3)(n2+3)(n3+3)
+    float4* table = nullptr;         // device, ghost-padded [n1+3][n2+3][n3+3][pitch/4]
+    int nbins = 0;                   // max(bricks, staged bins)
+    int nbins_direct = 0, nbins_staged = 0;
+    int nq = 1;                      // direct kernel: quads of 4 orbitals per lane (1..3)
+    int path = 0;                    // 0 auto, 1 direct, 2 staged
+    int staged_ok = 0;               // TMA descriptor built and the grid is large enough
+    CUtensorMap tmap;
     // grouping workspace (device)
     long long cap = 0;               // electrons the workspace holds
     int* bin = nullptr;              // [cap]
     int* perm = nullptr;             // [cap]
+    float4* recs = nullptr;          // [cap][24] per-electron records (staged path)
     unsigned* hist = nullptr;        // [nbins]
     // staging for blipgpu_eval_host (device)
     long long hcap = 0, hld = 0; int hmode = -1;
@@ -88,11 +104,41 @@ static int ensure_workspace(blipgpu_table* t, long long M, cudaStream_t s)
     CK(t, cudaStreamSynchronize(s));
     if (t->bin) cudaFree(t->bin);
     if (t->perm) cudaFree(t->perm);
-    t->bin = t->perm = nullptr; t->cap = 0;
+    if (t->recs) cudaFree(t->recs);
+    t->bin = t->perm = nullptr; t->recs = nullptr; t->cap = 0;
     CK(t, cudaMalloc(&t->bin, sizeof(int) * (size_t)M));
     CK(t, cudaMalloc(&t->perm, sizeof(int) * (size_t)M));
+    if (t->staged_ok) CK(t, cudaMalloc(&t->recs, sizeof(float) * blip::kRecFloats * (size_t)M));
     t->cap = M;
     return BLIPGPU_OK;
+}
+
+// TMA descriptor of the padded table for the staged kernel: 4-D tensor {pitch, n3+3, n2+3,
+// n1+3} of fp32, box {C, BZ+3, BY+3, 1} (one plane of a pencil's cross-section), no swizzle,
+// out-of-range elements read as zero.  cuTensorMapEncodeTiled is fetched through the runtime
+// so that the library does not link against libcuda.
+static bool build_tensor_map(blipgpu_table* t)
+{
+    typedef CUresult (*encode_fn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
+                                  const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
+                                  CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+    void* fn = nullptr;
+    cudaDriverEntryPointQueryResult qres;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres) != cudaSuccess ||
+        qres != cudaDriverEntryPointSuccess || !fn) {
+        (void)cudaGetLastError();
+        return false;
+    }
+    const cuuint64_t pitchB = (cuuint64_t)t->pitch * sizeof(float);
+    const cuuint64_t dims[4] = {(cuuint64_t)t->pitch, (cuuint64_t)t->g.np[2], (cuuint64_t)t->g.np[1],
+                                (cuuint64_t)t->g.np[0]};
+    const cuuint64_t strides[3] = {pitchB, pitchB * t->g.np[2], pitchB * t->g.np[2] * t->g.np[1]};
+    const cuuint32_t box[4] = {(cuuint32_t)SCfg::C, (cuuint32_t)SCfg::PZ, (cuuint32_t)SCfg::PY, 1u};
+    const cuuint32_t estr[4] = {1u, 1u, 1u, 1u};
+    const CUresult r = ((encode_fn)fn)(&t->tmap, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 4, t->table, dims, strides, box,
+                                       estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
+                                       CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    return r == CUDA_SUCCESS;
 }
 
 extern "C" int blipgpu_create(const double* lattice, const int* grid, int norb,
@@ -105,8 +151,12 @@ extern "C" int blipgpu_create(const double* lattice, const int* grid, int norb,
     if (norb < 1 || grid[0] < 4 || grid[1] < 4 || grid[2] < 4) return BLIPGPU_EINVAL;
     for (int k = 0; k < 9; ++k)
         if (!std::isfinite(lattice[k])) return BLIPGPU_EINVAL;
-    const long long nrows = (long long)grid[0] * grid[1] * grid[2];
-    if (nrows >= (1LL << 31)) return BLIPGPU_EINVAL;
+    const long long nsites = (long long)grid[0] * grid[1] * grid[2];
+    if (nsites >= (1LL << 31)) return BLIPGPU_EINVAL;
+    const long long pitch = ((long long)norb + 3) / 4 * 4;
+    const long long nrows = ((long long)grid[0] + 3) * ((long long)grid[1] + 3) * ((long long)grid[2] + 3);
+    // the kernels address the padded table with 32-bit float4 indices (tables up to 64 GiB)
+    if (nrows >= (1LL << 31) || nrows * (pitch / 4) >= (1LL << 32)) return BLIPGPU_EINVAL;
 
     int dev = 0;
     cudaError_t ce = cudaGetDevice(&dev);
@@ -121,6 +171,7 @@ extern "C" int blipgpu_create(const double* lattice, const int* grid, int norb,
     double Jd[3][3];
     for (int a = 0; a < 3; ++a) {
         t->g.n[a] = grid[a];
+        t->g.np[a] = grid[a] + 3;
         t->g.nb[a] = (grid[a] + blip::kBrick - 1) / blip::kBrick;
         for (int i = 0; i < 3; ++i) {
             Jd[a][i] = (double)grid[a] * t->g.G[3 * i + a];
@@ -132,11 +183,19 @@ extern "C" int blipgpu_create(const double* lattice, const int* grid, int norb,
         t->g.Q[k] = (float)(Jd[qa[k]][0] * Jd[qb[k]][0] + Jd[qa[k]][1] * Jd[qb[k]][1]
                             + Jd[qa[k]][2] * Jd[qb[k]][2]);
     t->L = norb;
-    t->pitch = ((long long)norb + 3) / 4 * 4;
+    t->pitch = pitch;
     t->nrows = nrows;
     t->g.L = norb;
-    t->g.pitch4 = (int)(t->pitch / 4);
-    t->nbins = t->g.nb[0] * t->g.nb[1] * t->g.nb[2];
+    t->g.pitch4 = (int)(pitch / 4);
+    t->sg.by = kSBY; t->sg.bz = kSBZ;
+    t->sg.nby = (grid[1] + kSBY - 1) / kSBY;
+    t->sg.nbz = (grid[2] + kSBZ - 1) / kSBZ;
+    t->sg.seg = kSSeg;
+    t->sg.nseg = (grid[0] + kSSeg - 1) / kSSeg;
+    t->nbins_direct = t->g.nb[0] * t->g.nb[1] * t->g.nb[2];
+    const long long sbins = (long long)t->sg.nby * t->sg.nbz * grid[0];
+    t->nbins_staged = sbins < (1LL << 30) ? (int)sbins : 0;
+    t->nbins = t->nbins_direct > t->nbins_staged ? t->nbins_direct : t->nbins_staged;
     t->nq = default_nq(t->g.pitch4);
 
     cudaStream_t s = (cudaStream_t)stream;
@@ -146,27 +205,42 @@ extern "C" int blipgpu_create(const double* lattice, const int* grid, int norb,
         rc = (e == cudaErrorMemoryAllocation) ? BLIPGPU_ENOMEM : BLIPGPU_ECUDA;
     };
     cudaError_t e;
-    const size_t bytes = (size_t)nrows * (size_t)t->pitch * sizeof(float);
+    const size_t bytes = (size_t)nrows * (size_t)pitch * sizeof(float);
+    const size_t src_bytes = (size_t)nsites * (size_t)norb * sizeof(float);
+    float* staging = nullptr;                         // device copy of a host table, until padded
     if ((e = cudaMalloc(&t->table, bytes)) != cudaSuccess) fail(e);
     if (rc == BLIPGPU_OK && (e = cudaMalloc(&t->hist, sizeof(unsigned) * (size_t)t->nbins)) != cudaSuccess) fail(e);
+    if (rc == BLIPGPU_OK && !coeffs_on_device) {
+        if ((e = cudaMalloc(&staging, src_bytes)) != cudaSuccess) fail(e);
+        else if ((e = cudaMemcpyAsync(staging, coeffs, src_bytes, cudaMemcpyHostToDevice, s)) != cudaSuccess) fail(e);
+    }
     if (rc == BLIPGPU_OK) {
-        const cudaMemcpyKind kind = coeffs_on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice;
-        if (t->pitch == norb) {
-            e = cudaMemcpyAsync(t->table, coeffs, bytes, kind, s);
-        } else {
-            e = cudaMemsetAsync(t->table, 0, bytes, s);          // zero the pad columns
-            if (e == cudaSuccess)
-                e = cudaMemcpy2DAsync(t->table, (size_t)t->pitch * sizeof(float), coeffs,
-                                      (size_t)norb * sizeof(float), (size_t)norb * sizeof(float),
-                                      (size_t)nrows, kind, s);
-        }
-        if (e == cudaSuccess) e = cudaStreamSynchronize(s);
+        const long long total4 = nrows * (pitch / 4);
+        const unsigned nblk = (unsigned)((total4 + 255) / 256);
+        blip::pad_kernel<<<nblk, 256, 0, s>>>(t->g, coeffs_on_device ? coeffs : staging, t->table, total4);
+        if ((e = cudaGetLastError()) == cudaSuccess) e = cudaStreamSynchronize(s);
         if (e != cudaSuccess) fail(e);
     }
+    if (staging) cudaFree(staging);
     if (rc == BLIPGPU_OK && (e = cudaStreamCreateWithFlags(&t->copy_stream, cudaStreamNonBlocking)) != cudaSuccess) fail(e);
     for (int k = 0; k < 2 && rc == BLIPGPU_OK; ++k)
         if ((e = cudaEventCreateWithFlags(&t->ev[k], cudaEventDisableTiming)) != cudaSuccess) fail(e);
     if (rc == BLIPGPU_OK && (e = cudaEventCreateWithFlags(&t->ev_in, cudaEventDisableTiming)) != cudaSuccess) fail(e);
+    if (rc == BLIPGPU_OK) {
+        // staged path: needs a full tile row (pitch >= C), a grid at least as large as one box,
+        // the opt-in shared memory size, and the TMA descriptor
+        const bool fits = t->pitch >= SCfg::C && t->g.np[1] >= SCfg::PY && t->g.np[2] >= SCfg::PZ &&
+                          t->nbins_staged > 0 && (size_t)prop.sharedMemPerBlockOptin >= sizeof(SCfg::Smem);
+        if (fits && build_tensor_map(t)) {
+            const int smem = (int)sizeof(SCfg::Smem);
+            e = cudaFuncSetAttribute(blip::eval_staged_kernel<0, kSVec, kSBY, kSBZ, kSRing, kSWarps>,
+                                     cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+            if (e == cudaSuccess)
+                e = cudaFuncSetAttribute(blip::eval_staged_kernel<1, kSVec, kSBY, kSBZ, kSRing, kSWarps>,
+                                         cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+            if (e == cudaSuccess) t->staged_ok = 1; else (void)cudaGetLastError();
+        }
+    }
     if (rc != BLIPGPU_OK) { blipgpu_destroy(t); return rc; }
     *out = t;
     return BLIPGPU_OK;
@@ -175,7 +249,7 @@ extern "C" int blipgpu_create(const double* lattice, const int* grid, int norb,
 extern "C" int blipgpu_destroy(blipgpu_table* t)
 {
     if (!t) return BLIPGPU_OK;
-    cudaFree(t->table); cudaFree(t->bin); cudaFree(t->perm); cudaFree(t->hist);
+    cudaFree(t->table); cudaFree(t->bin); cudaFree(t->perm); cudaFree(t->recs); cudaFree(t->hist);
     cudaFree(t->d_pos); cudaFree(t->d_val); cudaFree(t->d_grad); cudaFree(t->d_lap); cudaFree(t->d_cell);
     if (t->copy_stream) cudaStreamDestroy(t->copy_stream);
     for (int k = 0; k < 2; ++k) if (t->ev[k]) cudaEventDestroy(t->ev[k]);
@@ -201,39 +275,68 @@ static int check_eval_args(const blipgpu_table* t, const double* positions, long
 // Batches of at most this many electrons are evaluated in caller order: every electron of
 // the batch is in flight at once, so grouping cannot improve locality and costs 3 launches.
 static const long long kGroupThreshold = 2048;
+// The staged path pays (BY+3)(BZ+3)/(BY BZ) table rows per cell whatever the batch; it wins
+// once the rows are shared by enough electrons (average number of electrons touching a row).
+static const double kStagedMinReuse = 8.0;
+
+static bool use_staged(const blipgpu_table* t, long long M)
+{
+    if (!t->staged_ok || t->path == 1) return false;
+    if (t->path == 2) return true;
+    if (M <= kGroupThreshold) return false;
+    const double sites = (double)t->g.n[0] * t->g.n[1] * t->g.n[2];
+    return 64.0 * (double)M / sites >= kStagedMinReuse;
+}
 
 static int launch_eval(blipgpu_table* t, const double* positions, long long M, int mode,
                        float* val, float* grad, float* lap, long long ld, int* cell,
                        cudaStream_t s)
 {
     const int* perm = nullptr;
+    const bool staged = use_staged(t, M);
     if (t->profiling) CK(t, cudaEventRecord(t->pe[0], s));
-    if (M > kGroupThreshold) {
+    if (staged || M > kGroupThreshold) {
         int rc = ensure_workspace(t, M, s);
         if (rc != BLIPGPU_OK) return rc;
-        CK(t, cudaMemsetAsync(t->hist, 0, sizeof(unsigned) * (size_t)t->nbins, s));
+        const int nbins = staged ? t->nbins_staged : t->nbins_direct;
+        CK(t, cudaMemsetAsync(t->hist, 0, sizeof(unsigned) * (size_t)nbins, s));
         const unsigned nb = (unsigned)((M + 255) / 256);
-        blip::bin_kernel<<<nb, 256, 0, s>>>(t->g, positions, M, t->bin, t->hist, cell);
-        blip::scan_kernel<<<1, blip::kScanThreads, 0, s>>>(t->hist, t->nbins);
+        blip::bin_kernel<<<nb, 256, 0, s>>>(t->g, t->sg, staged ? 1 : 0, positions, M, t->bin, t->hist, cell);
+        blip::scan_kernel<<<1, blip::kScanThreads, 0, s>>>(t->hist, nbins);
         blip::scatter_kernel<<<nb, 256, 0, s>>>(t->bin, t->hist, M, t->perm);
         t->launches += 3;
         perm = t->perm;
         cell = nullptr;                                  // already written by bin_kernel
     }
-    const int nq = t->nq;
-    const dim3 grid((unsigned)((M + blip::kWarpsPerBlock - 1) / blip::kWarpsPerBlock),
-                    (unsigned)((t->g.pitch4 + 32 * nq - 1) / (32 * nq)));
-    const dim3 block(blip::kWarpsPerBlock * 32);
-    if (t->profiling) CK(t, cudaEventRecord(t->pe[1], s));
-#define BLIP_LAUNCH(MODE, NQ)                                                                  \
-    blip::eval_kernel<MODE, NQ><<<grid, block, 0, s>>>(t->g, t->table, positions, perm, M,     \
-                                                       val, grad, lap, ld, cell)
-    if (mode == BLIPGPU_VALUE) {
-        if (nq == 1) BLIP_LAUNCH(0, 1); else if (nq == 2) BLIP_LAUNCH(0, 2); else BLIP_LAUNCH(0, 3);
+    if (staged) {
+        blip::prep_kernel<<<(unsigned)((M + 127) / 128), 128, 0, s>>>(t->g, positions, t->perm, M, t->recs);
+        t->launches += 1;
+        if (t->profiling) CK(t, cudaEventRecord(t->pe[1], s));
+        const dim3 grid((unsigned)(t->sg.nby * t->sg.nbz * t->sg.nseg),
+                        (unsigned)((t->pitch + SCfg::C - 1) / SCfg::C));
+        const size_t smem = sizeof(SCfg::Smem);
+        if (mode == BLIPGPU_VALUE)
+            blip::eval_staged_kernel<0, kSVec, kSBY, kSBZ, kSRing, kSWarps><<<grid, SCfg::THREADS, smem, s>>>(
+                t->tmap, t->g, t->sg, t->recs, t->hist, val, grad, lap, ld);
+        else
+            blip::eval_staged_kernel<1, kSVec, kSBY, kSBZ, kSRing, kSWarps><<<grid, SCfg::THREADS, smem, s>>>(
+                t->tmap, t->g, t->sg, t->recs, t->hist, val, grad, lap, ld);
     } else {
-        if (nq == 1) BLIP_LAUNCH(1, 1); else if (nq == 2) BLIP_LAUNCH(1, 2); else BLIP_LAUNCH(1, 3);
-    }
+        const int nq = t->nq;
+        const dim3 grid((unsigned)((M + blip::kWarpsPerBlock - 1) / blip::kWarpsPerBlock),
+                        (unsigned)((t->g.pitch4 + 32 * nq - 1) / (32 * nq)));
+        const dim3 block(blip::kWarpsPerBlock * 32);
+        if (t->profiling) CK(t, cudaEventRecord(t->pe[1], s));
+#define BLIP_LAUNCH(MODE, NQ)                                                                         \
+        blip::eval_direct_kernel<MODE, NQ><<<grid, block, 0, s>>>(t->g, t->table, positions, perm, M, \
+                                                                  val, grad, lap, ld, cell)
+        if (mode == BLIPGPU_VALUE) {
+            if (nq == 1) BLIP_LAUNCH(0, 1); else if (nq == 2) BLIP_LAUNCH(0, 2); else BLIP_LAUNCH(0, 3);
+        } else {
+            if (nq == 1) BLIP_LAUNCH(1, 1); else if (nq == 2) BLIP_LAUNCH(1, 2); else BLIP_LAUNCH(1, 3);
+        }
 #undef BLIP_LAUNCH
+    }
     t->launches += 1;
     CK(t, cudaGetLastError());
     if (t->profiling) CK(t, cudaEventRecord(t->pe[2], s));
@@ -329,7 +432,7 @@ extern "C" int blipgpu_info(const blipgpu_table* t, int* grid, int* norb, long l
     if (grid) { grid[0] = t->g.n[0]; grid[1] = t->g.n[1]; grid[2] = t->g.n[2]; }
     if (norb) *norb = t->L;
     if (pitch) *pitch = t->pitch;
-    if (table_bytes) *table_bytes = t->nrows * t->pitch * (long long)sizeof(float);
+    if (table_bytes) *table_bytes = t->nrows * t->pitch * (long long)sizeof(float);   // ghost-padded
     return BLIPGPU_OK;
 }
 
@@ -352,6 +455,15 @@ extern "C" int blipgpu_last_kernel_ms(blipgpu_table* t, float* group_ms, float* 
     CK(t, cudaEventElapsedTime(&b, t->pe[1], t->pe[2]));
     if (group_ms) *group_ms = a;
     if (eval_ms) *eval_ms = b;
+    return BLIPGPU_OK;
+}
+
+extern "C" int blipgpu_set_tuning(blipgpu_table* t, int path, int nq)
+{
+    if (!t || path < 0 || path > 2 || nq < 0 || nq > 3) return BLIPGPU_EINVAL;
+    if (path == 2 && !t->staged_ok) return BLIPGPU_EINVAL;
+    t->path = path;
+    t->nq = nq ? nq : default_nq(t->g.pitch4);
     return BLIPGPU_OK;
 }
 

@@ -60,6 +60,62 @@ def test_grouped_equals_ungrouped(torch_cuda, blip):
     t.close()
 
 
+# ------------------------------------------------------------------ staged (TMA / shared memory) path
+STAGED_CASES = [((9, 10, 13), 130, 3000, TRICLINIC), ((20, 7, 8), 128, 1200, SKEW),
+                ((17, 12, 19), 257, 9000, TRICLINIC), ((4, 4, 8), 200, 700, SKEW)]
+
+
+@pytest.mark.parametrize("grid,L,M,lat", STAGED_CASES)
+def test_staged_path_matches_oracle_and_direct_path(torch_cuda, blip, grid, L, M, lat):
+    """The staged kernel forced on grids that are ragged against the 4x8 pencil cross-section and
+    the 16-plane segments, orbital counts that are not a multiple of the 128-orbital tile, and
+    pencils without electrons: parity with the oracle, and bit-identical to the direct kernel."""
+    A, c, pos = workloads.small_case(grid, L, M, lat, seed=L + M, spread=3.0)
+    t = blip.BlipTable(A, grid, L, c)
+    for mode in (1, 0):
+        blip.blipgpu_set_tuning(t.handle, path=2)
+        n0 = t.launch_count()
+        staged = run_gpu(torch_cuda, blip, A, grid, c, pos, mode=mode, table=t)
+        assert t.launch_count() - n0 == 5                # bin, scan, scatter, prep, staged eval
+        compare(A, grid, c, pos, staged, mode=mode)
+        blip.blipgpu_set_tuning(t.handle, path=1)
+        direct = run_gpu(torch_cuda, blip, A, grid, c, pos, mode=mode, table=t)
+        for a, b in zip(staged, direct):
+            assert (a is None and b is None) or np.array_equal(a, b)
+    t.close()
+
+
+def test_staged_path_clustered_and_non_finite(torch_cuda, blip):
+    """All electrons in a few cells (long unit lists per plane, most pencils empty), plus
+    non-finite positions, through the staged kernel."""
+    grid, L = (24, 9, 17), 132
+    A, c, pos = workloads.small_case(grid, L, 4000, TRICLINIC, seed=11, spread=0.02)
+    pos[::7] += np.array(TRICLINIC[0]) * 0.37
+    pos[5, 1] = np.nan
+    pos[3999] = np.inf
+    t = blip.BlipTable(A, grid, L, c)
+    blip.blipgpu_set_tuning(t.handle, path=2)
+    val, grad, lap, cell = run_gpu(torch_cuda, blip, A, grid, c, pos, table=t)
+    oval, ograd, olap, ocell = oracle.eval_fast(A, grid, c, pos)
+    assert np.array_equal(cell, ocell)
+    bad = np.isnan(oval).all(axis=1)
+    assert bad.sum() == 2 and np.array_equal(np.isnan(val).all(axis=1), bad)
+    assert np.isnan(grad[bad]).all() and np.isnan(lap[bad]).all()
+    good = ~bad
+    compare(A, grid, c, pos[good], (val[good], grad[good], lap[good], cell[good]))
+    t.close()
+
+
+def test_staged_path_unavailable_is_an_error(torch_cuda, blip):
+    A, c, pos = workloads.small_case((6, 6, 6), 8, 10, SKEW, seed=4)      # fewer than 128 orbitals
+    t = blip.BlipTable(A, (6, 6, 6), 8, c)
+    assert blip.lib().blipgpu_set_tuning(t.handle, 2, 0) == blip.EINVAL
+    assert blip.lib().blipgpu_set_tuning(t.handle, 3, 0) == blip.EINVAL
+    assert blip.lib().blipgpu_set_tuning(t.handle, 1, 4) == blip.EINVAL
+    assert blip.lib().blipgpu_set_tuning(t.handle, 1, 3) == blip.OK
+    t.close()
+
+
 def test_non_finite_positions(torch_cuda, blip):
     A, c, pos = workloads.small_case((6, 6, 6), 8, 3000, SKEW, seed=4)
     bad = [0, 17, 1500, 2999]
