@@ -51,7 +51,10 @@ struct StagedGeom {
     int nby, nbz;       // pencils per axis
     int seg;            // cell planes per segment
     int nseg;           // segments per pencil = ceil(n1 / seg)
+    int nps;            // pencil segments = nby * nbz * nseg (the work items, per orbital chunk)
+    int chunk_major;    // order of the work items (see eval_staged_kernel)
 };
+constexpr int kMaxSortedItems = 8192;      // pencil segments the scan kernel can order by load
 
 // ---------------------------------------------------------------------------------------
 // a-1: cell map.  The IEEE sequence is pinned so that the integer
@@ -107,17 +110,29 @@ bin_kernel(Geom g, StagedGeom sg, int staged, const double* __restrict__ pos, lo
     atomicAdd(&hist[b], 1u);
 }
 
-// a-4 (2/3): exclusive scan of the histogram, in place, one CTA.
+// a-4 (2/3): exclusive scan of the histogram, in place, one CTA.  For the staged path it also
+// orders the work items (pencil segments) by decreasing electron count — the persistent
+// staged kernel takes items from a shared counter, so heavy items first keeps the tail short
+// (longest-processing-time-first) — and resets that counter.
+//   order[0 .. nps)   {pencil segment id, first unit, units, 0}; units are indices into the
+//                     sorted records.  sg.chunk_major: x-slab by x-slab, heaviest first inside a
+//                     slab; else heaviest first overall; in id order if nps > kMaxSortedItems
+//   meta[0]           number of leading entries of `order` that hold electrons
+//   meta[1]           work counter of the staged kernel, reset to 0
 __global__ void __launch_bounds__(kScanThreads)
-scan_kernel(unsigned* __restrict__ hist, int nbins)
+scan_kernel(unsigned* __restrict__ hist, int nbins, long long M, int staged, Geom g, StagedGeom sg,
+            int4* __restrict__ order, int* __restrict__ meta)
 {
     __shared__ unsigned part[kScanThreads];
+    __shared__ unsigned keys[kMaxSortedItems];
+    __shared__ int nonempty;
     const int tid = threadIdx.x;
     const int per = (nbins + kScanThreads - 1) / kScanThreads;
     const int lo = min(tid * per, nbins), hi = min(lo + per, nbins);
     unsigned s = 0;
     for (int b = lo; b < hi; ++b) s += hist[b];
     part[tid] = s;
+    if (tid == 0) nonempty = 0;
     __syncthreads();
     for (int d = 1; d < kScanThreads; d <<= 1) {            // Hillis-Steele inclusive scan
         unsigned v = (tid >= d) ? part[tid - d] : 0u;
@@ -127,6 +142,69 @@ scan_kernel(unsigned* __restrict__ hist, int nbins)
     }
     unsigned run = part[tid] - s;                            // exclusive prefix of this segment
     for (int b = lo; b < hi; ++b) { unsigned c = hist[b]; hist[b] = run; run += c; }
+    if (!staged) return;
+    __syncthreads();                                         // hist[b] = start of bin b, block-visible
+    if (tid == 0) meta[1] = 0;
+    const int nps = sg.nps;
+    auto units_of = [&](int i, unsigned& u0, unsigned& u1) {
+        const int pencil = i / sg.nseg, segi = i - pencil * sg.nseg;
+        const int p0 = segi * sg.seg, p1 = min(p0 + sg.seg, g.n[0]);
+        const int bin0 = pencil * g.n[0] + p0, bin1 = pencil * g.n[0] + p1;         // [bin0, bin1)
+        u0 = hist[bin0];
+        u1 = (bin1 < nbins) ? hist[bin1] : (unsigned)M;
+    };
+    if (nps > kMaxSortedItems) {
+        for (int i = tid; i < nps; i += kScanThreads) {
+            unsigned u0, u1;
+            units_of(i, u0, u1);
+            order[i] = make_int4(i, (int)u0, (int)(u1 - u0), 0);
+        }
+        if (tid == 0) meta[0] = nps;
+        return;
+    }
+    int n2 = 1;
+    while (n2 < nps) n2 <<= 1;
+    int mine = 0;
+    for (int i = tid; i < n2; i += kScanThreads) {
+        unsigned key = 0;
+        if (i < nps) {
+            unsigned u0, u1;
+            units_of(i, u0, u1);
+            if (sg.chunk_major) {
+                // slab-major: all segments of x-slab 0 first (heaviest first inside the slab), then
+                // slab 1, ... — the CTAs in flight share one slab of one chunk of the table in L2
+                const unsigned segi = (unsigned)(i % sg.nseg);
+                key = ((127u - min(segi, 127u)) << 25) | (min(u1 - u0, 4095u) << 13) | (unsigned)i;
+                mine += 1;
+            } else {
+                const unsigned cnt = min(u1 - u0, (1u << 19) - 1u);
+                key = (cnt << 13) | (unsigned)i;
+                mine += (cnt != 0);
+            }
+        }
+        keys[i] = key;
+    }
+    if (mine) atomicAdd(&nonempty, mine);
+    __syncthreads();
+    for (int k = 2; k <= n2; k <<= 1)                         // bitonic sort, descending
+        for (int j = k >> 1; j > 0; j >>= 1) {
+            for (int i = tid; i < n2; i += kScanThreads) {
+                const int x = i ^ j;
+                if (x > i) {
+                    const unsigned a = keys[i], b = keys[x];
+                    const bool desc = (i & k) == 0;
+                    if ((a < b) == desc) { keys[i] = b; keys[x] = a; }
+                }
+            }
+            __syncthreads();
+        }
+    for (int i = tid; i < nps; i += kScanThreads) {
+        const int id = (int)(keys[i] & 8191u);
+        unsigned u0, u1;
+        units_of(id, u0, u1);
+        order[i] = make_int4(id, (int)u0, (int)(u1 - u0), 0);
+    }
+    if (tid == 0) meta[0] = nonempty;
 }
 
 // a-4 (3/3): scatter electron ids into bin order (order inside a bin is arbitrary; the
@@ -213,6 +291,17 @@ struct ElecRec {
 };
 static_assert(sizeof(ElecRec) == kRecFloats * 4, "ElecRec is 96 floats");
 
+// The same record as the staged kernel reads it: instead of the cell index it carries where
+// the electron's 4x4x4 block starts in the staged planes of its work item.
+struct StagedRec {
+    float4 cw[16];
+    float  lb[16];
+    float  wz[3][4];
+    int4   loc;         // {i1 - first plane of the pencil segment (-1: non-finite position),
+                        //  byte offset of row (i2, i3) in a staged plane, unused, electron id}
+};
+static_assert(sizeof(StagedRec) == sizeof(ElecRec), "one record layout");
+
 // Column weights of column `col` from the per-axis factors ax[axis][w, w', w''][m].
 template <typename AX>
 __device__ __forceinline__ void column_weights(const Geom& g, const AX& ax, int col, float4& cw, float& lb)
@@ -256,15 +345,18 @@ __device__ __forceinline__ void warp_prepare(const Geom& g, const double* __rest
     __syncwarp();
 }
 
-// a-1 + a-2 for the staged path: one thread per electron of the sorted order, records to
-// global memory (384 B each; read back through L2 by the staged kernel once per orbital chunk).
+// a-4 (3/3) + a-1 + a-2 for the staged path: one thread per electron takes its slot in bin
+// order and writes the electron's record there (384 B; read back through L2 by the staged
+// kernel once per orbital chunk).  On return offs[b] is the END of bin b.
 __global__ void __launch_bounds__(128)
-prep_kernel(Geom g, const double* __restrict__ pos, const int* __restrict__ perm, long long M,
-            float4* __restrict__ recs)
+scatter_prep_kernel(Geom g, StagedGeom sg, int tile_floats, const double* __restrict__ pos,
+                    const int* __restrict__ bin, unsigned* __restrict__ offs, long long M,
+                    float4* __restrict__ recs)
 {
-    const long long s = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-    if (s >= M) return;
-    const int e = perm[s];
+    const long long el = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (el >= M) return;
+    const int e = (int)el;
+    const unsigned s = atomicAdd(&offs[bin[e]], 1u);
     const double x = pos[3 * (size_t)e], y = pos[3 * (size_t)e + 1], z = pos[3 * (size_t)e + 2];
     float ax[3][3][4]; int ic[3];
 #pragma unroll
@@ -289,8 +381,14 @@ prep_kernel(Geom g, const double* __restrict__ pos, const int* __restrict__ perm
     out[21] = make_float4(ax[2][1][0], ax[2][1][1], ax[2][1][2], ax[2][1][3]);
     out[22] = make_float4(__fmul_rn(g.Q[2], ax[2][2][0]), __fmul_rn(g.Q[2], ax[2][2][1]),
                           __fmul_rn(g.Q[2], ax[2][2][2]), __fmul_rn(g.Q[2], ax[2][2][3]));
-    out[23] = make_float4(__int_as_float(ic[0]), __int_as_float(ic[1]), __int_as_float(ic[2]),
-                          __int_as_float(e));
+    // StagedRec::loc: plane within the pencil segment, byte offset of row (i2, i3) in a plane of
+    // (by+3) x (bz+3) rows of tile_floats floats
+    int pl = -1, off = 0;
+    if (ic[0] >= 0) {
+        pl = ic[0] % sg.seg;
+        off = ((ic[1] % sg.by) * (sg.bz + 3) + (ic[2] % sg.bz)) * tile_floats * 4;
+    }
+    out[23] = make_float4(__int_as_float(pl), __int_as_float(off), 0.f, __int_as_float(e));
 }
 
 // ---------------------------------------------------------------------------------------
@@ -318,6 +416,10 @@ __device__ __forceinline__ float2 unpack2(u64 v)
 
 // Accumulators of one pair of orbitals.
 struct PairAcc { u64 val, t1, t2, t3, lp; };
+__device__ __forceinline__ void set_nan(PairAcc& a)         // outputs of a non-finite position (R17)
+{
+    a.val = a.t1 = a.t2 = a.t3 = a.lp = 0x7fc000007fc00000ull;
+}
 
 // a-3 for one column (m1, m2) and one pair of orbitals: c0..c3 are the coefficient pairs of
 // the 4 z sites.  Both kernels call this with the same operands in the same order, so their
@@ -338,7 +440,7 @@ __device__ __forceinline__ void fold_pair(u64 c0, u64 c1, u64 c2, u64 c3, const 
         acc.t2 = fma2(a, dup2(w.z), acc.t2);
         acc.t3 = fma2(b, dup2(w.x), acc.t3);
         u64 l = fma2(a, dup2(w.w), acc.lp);
-        l = fma2(b, dup2(lb), l);
+        if (MODE == 1) l = fma2(b, dup2(lb), l);             // MODE 2: Q02 = Q12 = 0, so Lb = 0
         acc.lp = fma2(d, dup2(w.x), l);
     }
 }
@@ -356,29 +458,34 @@ __device__ __forceinline__ void st_stream2(float* p, float a, float b)
 // a-5 for NP consecutive pairs (NP = 1: 2 orbitals, NP = 2: 4 orbitals) starting at orbital
 // column `col0` of electron `e`: Cartesian gradient from the grid-space one, streaming stores
 // (evict-first: outputs are never re-read and must not push table rows out of L2).
+// MODE 2: J is diagonal (lattice vectors along the Cartesian axes).
 template <int MODE, int NP>
-__device__ __forceinline__ void store_pairs(const Geom& g, const PairAcc (&acc)[NP], bool ok, int e,
+__device__ __forceinline__ void store_pairs(const Geom& g, const PairAcc (&acc)[NP], int e,
                                             int col0, float* __restrict__ val, float* __restrict__ grad,
                                             float* __restrict__ lap, long long ld)
 {
-    const float nan = __int_as_float(0x7fc00000);
     float v[2 * NP], gx[2 * NP], gy[2 * NP], gz[2 * NP], lp[2 * NP];
 #pragma unroll
     for (int p = 0; p < NP; ++p) {
         const float2 s = unpack2(acc[p].val);
-        v[2 * p] = ok ? s.x : nan; v[2 * p + 1] = ok ? s.y : nan;
+        v[2 * p] = s.x; v[2 * p + 1] = s.y;
         if (MODE != 0) {
             const float2 a = unpack2(acc[p].t1), b = unpack2(acc[p].t2), c = unpack2(acc[p].t3);
             const float2 l = unpack2(acc[p].lp);
             const float ta[2] = {a.x, a.y}, tb[2] = {b.x, b.y}, tc[2] = {c.x, c.y};
 #pragma unroll
             for (int h = 0; h < 2; ++h) {
-                const float x = __fmaf_rn(g.J[0], ta[h], __fmaf_rn(g.J[3], tb[h], __fmul_rn(g.J[6], tc[h])));
-                const float y = __fmaf_rn(g.J[1], ta[h], __fmaf_rn(g.J[4], tb[h], __fmul_rn(g.J[7], tc[h])));
-                const float z = __fmaf_rn(g.J[2], ta[h], __fmaf_rn(g.J[5], tb[h], __fmul_rn(g.J[8], tc[h])));
-                gx[2 * p + h] = ok ? x : nan; gy[2 * p + h] = ok ? y : nan; gz[2 * p + h] = ok ? z : nan;
+                if (MODE == 2) {
+                    gx[2 * p + h] = __fmul_rn(g.J[0], ta[h]);
+                    gy[2 * p + h] = __fmul_rn(g.J[4], tb[h]);
+                    gz[2 * p + h] = __fmul_rn(g.J[8], tc[h]);
+                } else {
+                    gx[2 * p + h] = __fmaf_rn(g.J[0], ta[h], __fmaf_rn(g.J[3], tb[h], __fmul_rn(g.J[6], tc[h])));
+                    gy[2 * p + h] = __fmaf_rn(g.J[1], ta[h], __fmaf_rn(g.J[4], tb[h], __fmul_rn(g.J[7], tc[h])));
+                    gz[2 * p + h] = __fmaf_rn(g.J[2], ta[h], __fmaf_rn(g.J[5], tb[h], __fmul_rn(g.J[8], tc[h])));
+                }
             }
-            lp[2 * p] = ok ? l.x : nan; lp[2 * p + 1] = ok ? l.y : nan;
+            lp[2 * p] = l.x; lp[2 * p + 1] = l.y;
         }
     }
     const size_t o = (size_t)e * (size_t)ld + (size_t)col0;
@@ -469,7 +576,10 @@ eval_direct_kernel(Geom g, const float4* __restrict__ table4, const double* __re
     for (int j = 0; j < NQ; ++j)
 #pragma unroll
         for (int h = 0; h < 2; ++h) acc[j][h].val = acc[j][h].t1 = acc[j][h].t2 = acc[j][h].t3 = acc[j][h].lp = 0ull;
-    if (ok) {
+    if (!ok) {
+#pragma unroll
+        for (int j = 0; j < NQ; ++j) { set_nan(acc[j][0]); set_nan(acc[j][1]); }
+    } else {
         float wz[3][4];
 #pragma unroll
         for (int k = 0; k < 3; ++k)
@@ -494,18 +604,35 @@ eval_direct_kernel(Geom g, const float4* __restrict__ table4, const double* __re
     }
 #pragma unroll
     for (int j = 0; j < NQ; ++j)
-        if (quad[j] < g.pitch4) store_pairs<MODE, 2>(g, acc[j], ok, e, 4 * quad[j], val, grad, lap, ld);
+        if (quad[j] < g.pitch4) store_pairs<MODE, 2>(g, acc[j], e, 4 * quad[j], val, grad, lap, ld);
 }
 
 // ---------------------------------------------------------------------------------------
-// Staged kernel.  Work item (blockIdx.x = pencil segment, blockIdx.y = orbital chunk of C =
-// 32*VEC orbitals): the electrons of the segment, sorted by cell plane i1, are the units; the
-// table planes p1 = lo .. hi+3 of the pencil's (BY+3) x (BZ+3) cross-section slide through a
-// ring of R shared-memory slots.  One producer warp issues one TMA box per plane; NW consumer
-// warps take units from a shared counter.  A consumer at plane i1 waits for planes i1..i1+3
-// (full barriers) and, when it moves past plane s, releases it (empty barriers, NW arrivals),
-// which lets the producer overwrite the slot of plane s with plane s+R.
+// Staged kernel (persistent: one CTA per SM).  A work item is (pencil segment, orbital chunk
+// of C = 32*VEC orbitals): the electrons of the segment, sorted by cell plane i1, are its
+// units; the table planes p1 = lo .. hi+3 of the pencil's (BY+3) x (BZ+3) cross-section slide
+// through a ring of R shared-memory slots, one TMA box per plane.
+//
+//   producer warp   takes items from the global counter meta[1] (chunk-major, heaviest segment
+//                   first: `order`), publishes them through a 2-entry item queue and issues the
+//                   planes of item after item into the ring — the planes of the next item
+//                   arrive while the consumers finish the current one;
+//   NW consumers    take units of the current item from a shared counter.  Planes carry a
+//                   CTA-wide sequence number; every consumer waits for and releases every
+//                   plane in sequence order (full / empty barriers, NW arrivals per plane), so
+//                   barrier phases follow from the sequence number alone.
 // ---------------------------------------------------------------------------------------
+#ifndef BLIP_SUSPEND_NS
+#define BLIP_SUSPEND_NS 20000u      // try_wait suspend-time hint: a waiting warp sleeps instead of polling
+#endif
+__device__ __forceinline__ ulonglong2 lds128(unsigned addr)
+{
+    ulonglong2 v; asm volatile("ld.shared.v2.b64 {%0, %1}, [%2];" : "=l"(v.x), "=l"(v.y) : "r"(addr)); return v;
+}
+__device__ __forceinline__ u64 lds64(unsigned addr)
+{
+    u64 v; asm volatile("ld.shared.b64 %0, [%1];" : "=l"(v) : "r"(addr)); return v;
+}
 __device__ __forceinline__ unsigned smem_u32(const void* p) { return (unsigned)__cvta_generic_to_shared(p); }
 __device__ __forceinline__ void mbar_init(unsigned bar, unsigned count)
 {
@@ -524,11 +651,29 @@ __device__ __forceinline__ void mbar_wait(unsigned bar, unsigned parity)
     asm volatile(
         "{\n\t.reg .pred p;\n\t"
         "WAIT_%=:\n\t"
-        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n\t"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1, %2;\n\t"
         "@p bra DONE_%=;\n\t"
         "bra WAIT_%=;\n\t"
         "DONE_%=:\n\t}"
-        :: "r"(bar), "r"(parity) : "memory");
+        :: "r"(bar), "r"(parity), "r"(BLIP_SUSPEND_NS) : "memory");
+}
+#ifndef BLIP_BACKOFF_NS
+#define BLIP_BACKOFF_NS 32
+#endif
+// Producer-side wait: the producer has nothing else to do, so it backs off between polls and
+// leaves the issue slots of its scheduler to the consumer warps that share it.
+__device__ __forceinline__ void mbar_wait_backoff(unsigned bar, unsigned parity)
+{
+    unsigned done = 0;
+    while (true) {
+        asm volatile(
+            "{\n\t.reg .pred p;\n\t"
+            "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
+            "selp.u32 %0, 1, 0, p;\n\t}"
+            : "=r"(done) : "r"(bar), "r"(parity) : "memory");
+        if (done) break;
+        if (BLIP_BACKOFF_NS > 0) __nanosleep(BLIP_BACKOFF_NS);
+    }
 }
 __device__ __forceinline__ void tma_load_4d(unsigned dst, const CUtensorMap* tmap, int c0, int c1, int c2, int c3,
                                             unsigned bar)
@@ -540,6 +685,36 @@ __device__ __forceinline__ void tma_load_4d(unsigned dst, const CUtensorMap* tma
         : "memory");
 }
 
+#ifdef BLIP_STATS
+// Development instrumentation (not compiled into the product): per CTA {start, end} in ns and,
+// per consumer warp, {units, cycles waiting for planes, cycles waiting for items, cycles total}.
+__device__ unsigned long long g_stats[160][2 + 16 * 4 + 8];
+__device__ __forceinline__ unsigned long long gtime()
+{
+    unsigned long long t; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t)); return t;
+}
+#endif
+constexpr int kItemQueue = 3;              // item descriptors in flight per CTA: finishing, current, next
+
+__device__ __forceinline__ void tma_prefetch_4d(const CUtensorMap* tmap, int c0, int c1, int c2, int c3)
+{
+#ifdef BLIP_NO_L2PF
+    return;
+#endif
+    asm volatile("cp.async.bulk.prefetch.tensor.4d.L2.global.tile [%0, {%1, %2, %3, %4}];"
+                 :: "l"(reinterpret_cast<uint64_t>(tmap)), "r"(c0), "r"(c1), "r"(c2), "r"(c3) : "memory");
+}
+
+struct WorkItem {
+    int nplanes;        // planes of this item (0: no electrons, -1: no more work)
+    int chunk;          // orbital chunk
+    int by, bz;         // pencil coordinates
+    int lo;             // first cell plane
+    unsigned seq0;      // CTA-wide sequence number of plane lo
+    unsigned u0;        // first unit (index into the sorted records)
+    unsigned nunits;
+};
+
 template <int VEC, int BY, int BZ, int R, int NW>
 struct StagedCfg {
     static constexpr int C = 32 * VEC;                       // orbitals per tile row
@@ -550,143 +725,260 @@ struct StagedCfg {
     struct Smem {
         alignas(128) float plane[R][PLANE_FLOATS];
         alignas(16) ElecRec rec[NW][2];
+        alignas(16) WorkItem item[kItemQueue];
         alignas(8) u64 full[R];
         alignas(8) u64 empty[R];
-        int counter;
+        alignas(8) u64 ifull[kItemQueue];
+        alignas(8) u64 iempty[kItemQueue];
     };
 };
 
+// Deadlock freedom of the two queues.  The producer publishes item k+1 before it issues any
+// plane of item k, and needs for that only the descriptor slot of item k-2, which every
+// consumer gives back when it leaves item k-2.  A consumer looks at the descriptor of item
+// k+1 (to prefetch its first record) only while it works on a unit of item k, i.e. after it
+// has left item k-1 and released all planes of it; so whatever a consumer waits for never
+// depends on something that consumer still holds.
 template <int MODE, int VEC, int BY, int BZ, int R, int NW>
 __global__ void __launch_bounds__((NW + 1) * 32, 1)
 eval_staged_kernel(const __grid_constant__ CUtensorMap tmap, Geom g, StagedGeom sg,
-                   const float4* __restrict__ recs, const unsigned* __restrict__ bin_end,
-                   float* __restrict__ val, float* __restrict__ grad, float* __restrict__ lap, long long ld)
+                   const float4* __restrict__ recs, const int4* __restrict__ order, int* __restrict__ meta,
+                   int nchunk, float* __restrict__ val, float* __restrict__ grad, float* __restrict__ lap,
+                   long long ld)
 {
     using Cfg = StagedCfg<VEC, BY, BZ, R, NW>;
     extern __shared__ __align__(128) unsigned char smem_raw[];
     typename Cfg::Smem& sm = *reinterpret_cast<typename Cfg::Smem*>(smem_raw);
     constexpr int NP = VEC / 2;
+    constexpr unsigned IQ = kItemQueue;
+    constexpr unsigned RU = R;
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    const int pencil = blockIdx.x / sg.nseg, segi = blockIdx.x - pencil * sg.nseg;
-    const int lo = segi * sg.seg, hi = min(lo + sg.seg, g.n[0]) - 1;         // cell planes of this segment
-    const int bin0 = pencil * g.n[0] + lo, bin1 = pencil * g.n[0] + hi;
-    const unsigned u0 = bin0 ? bin_end[bin0 - 1] : 0u, u1 = bin_end[bin1];
-    if (u0 == u1) return;                                                    // no electrons here
-    const int chunk = blockIdx.y;
-    const int by = pencil / sg.nbz, bz = pencil - by * sg.nbz;
-
     if (threadIdx.x == 0) {
         for (int s = 0; s < R; ++s) { mbar_init(smem_u32(&sm.full[s]), 1); mbar_init(smem_u32(&sm.empty[s]), NW); }
-        sm.counter = 0;
+        for (int s = 0; s < (int)IQ; ++s) { mbar_init(smem_u32(&sm.ifull[s]), 1); mbar_init(smem_u32(&sm.iempty[s]), NW); }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
         asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
     }
     __syncthreads();
 
     if (warp == NW) {
-        // ---- producer: one TMA box {C, PZ, PY, 1} per table plane, in plane order; before
-        // leaving, wait until the last planes have landed (no copy may outlive the CTA)
+        // ---- producer.  It may leave as soon as everything is issued: every consumer waits
+        // for every plane before it leaves, so no copy outlives the CTA.
         if (lane == 0) {
-            const int nplanes = hi + 4 - lo;
-            for (int k = 0; k < nplanes; ++k) {
-                const int slot = k % R, round = k / R;
-                if (round > 0) mbar_wait(smem_u32(&sm.empty[slot]), (unsigned)((round & 1) ^ 1));
-                const unsigned bar = smem_u32(&sm.full[slot]);
-                mbar_expect_tx(bar, Cfg::PLANE_BYTES);
-                tma_load_4d(smem_u32(&sm.plane[slot][0]), &tmap, chunk * Cfg::C, bz * BZ, by * BY, lo + k, bar);
+            const int nps = meta[0];
+            const int nitems = nps * nchunk;
+            unsigned seq_pub = 0;                            // sequence number of the next item's first plane
+            struct Desc { int nplanes, chunk, by, bz, lo; };
+            auto fetch = [&](unsigned k) -> Desc {           // take item k from the global queue and publish it
+                const unsigned q = k % IQ;
+                if (k >= IQ) mbar_wait_backoff(smem_u32(&sm.iempty[q]), ((k / IQ) & 1u) ^ 1u);
+                const int w = atomicAdd(&meta[1], 1);
+                WorkItem& it = sm.item[q];
+                Desc d = {-1, 0, 0, 0, 0};
+                if (w < nitems) {
+                    // heaviest segment first, its chunks side by side (sg.chunk_major: all segments
+                    // of chunk 0, then chunk 1, ... — better L2 locality, longer tail)
+                    d.chunk = sg.chunk_major ? w / nps : w % nchunk;
+                    const int4 o = __ldg(order + (sg.chunk_major ? w - d.chunk * nps : w / nchunk));
+                    const int pencil = o.x / sg.nseg, segi = o.x - pencil * sg.nseg;
+                    d.lo = segi * sg.seg;
+                    const int hi = min(d.lo + sg.seg, g.n[0]) - 1;
+                    d.by = pencil / sg.nbz; d.bz = pencil - d.by * sg.nbz;
+                    d.nplanes = o.z > 0 ? hi + 4 - d.lo : 0;
+                    it.chunk = d.chunk; it.by = d.by; it.bz = d.bz; it.lo = d.lo; it.seq0 = seq_pub;
+                    it.u0 = (unsigned)o.y; it.nunits = (unsigned)o.z;
+                    seq_pub += (unsigned)d.nplanes;
+                    for (int k2 = 0; k2 < min(d.nplanes, R); ++k2)       // warm L2 with the item's first planes
+                        tma_prefetch_4d(&tmap, d.chunk * Cfg::C, d.bz * BZ, d.by * BY, d.lo + k2);
+                }
+                it.nplanes = d.nplanes;
+                mbar_arrive(smem_u32(&sm.ifull[q]));
+                return d;
+            };
+            unsigned seq = 0;
+            Desc cur = fetch(0);
+            for (unsigned k = 0; cur.nplanes >= 0; ++k) {
+                const Desc nxt = fetch(k + 1);
+                for (int j = 0; j < cur.nplanes; ++j, ++seq) {
+                    const unsigned slot = seq % RU, round = seq / RU;
+                    if (j + R < cur.nplanes)
+                        tma_prefetch_4d(&tmap, cur.chunk * Cfg::C, cur.bz * BZ, cur.by * BY, cur.lo + j + R);
+                    if (round > 0) mbar_wait_backoff(smem_u32(&sm.empty[slot]), (round & 1u) ^ 1u);
+                    const unsigned bar = smem_u32(&sm.full[slot]);
+                    mbar_expect_tx(bar, Cfg::PLANE_BYTES);
+                    tma_load_4d(smem_u32(&sm.plane[slot][0]), &tmap, cur.chunk * Cfg::C, cur.bz * BZ, cur.by * BY,
+                                cur.lo + j, bar);
+                }
+                cur = nxt;
             }
-            for (int k = max(0, nplanes - R); k < nplanes; ++k)
-                mbar_wait(smem_u32(&sm.full[k % R]), (unsigned)((k / R) & 1));
         }
         return;
     }
 
-    // ---- consumers
-    const unsigned nunits = u1 - u0;
-    const float4* __restrict__ rsrc = recs + (size_t)u0 * (kRecFloats / 4);
-    // Every warp walks through the planes in order: it waits for plane q only after releasing
-    // plane q-R (whose slot plane q reuses), and releases a plane only after having waited for
-    // it, so that its NW arrivals on an empty barrier always belong to the barrier's current phase.
-    int released = lo;                 // planes < released have been released by this warp
-    int waited = lo - 1;               // planes <= waited have been waited for by this warp
-    auto advance = [&](int need_upto, int release_below) {
-        for (int q = waited + 1; q <= need_upto; ++q) {
-            for (; released <= q - R; ++released)
-                if (lane == 0) mbar_arrive(smem_u32(&sm.empty[(released - lo) % R]));
-            mbar_wait(smem_u32(&sm.full[(q - lo) % R]), (unsigned)(((q - lo) / R) & 1));
+    // ---- consumers.  Warp w takes units w, w + NW, ... of every item.  Planes are counted by
+    // their CTA-wide sequence number; a warp waits for plane q only after releasing plane q-R
+    // (whose slot plane q reuses) and releases a plane only after having waited for it, so
+    // its arrival on an empty barrier always belongs to the barrier's current phase.
+    //
+    // The loop below is bound by instruction issue (a packed FMA holds the issue port of its
+    // scheduler for two cycles, everything else for one), so the bookkeeping per unit is kept
+    // short: the record carries the unit's plane number and byte offset inside a plane.
+#ifdef BLIP_STATS
+    unsigned long long st_units = 0, st_pwait = 0;
+    long long st_pro = 0, st_main = 0, st_epi = 0;
+    const long long st_c0 = clock64();
+    if (threadIdx.x == 0) g_stats[blockIdx.x][0] = gtime();
+#endif
+    unsigned released = 0;             // planes < released have been released by this warp
+    unsigned waited = 0;               // planes < waited have been waited for by this warp
+    auto wait_upto = [&](unsigned need_end) {            // planes < need_end resident
+#pragma unroll 1
+        while (waited < need_end) {
+            if (released + RU <= waited) {
+                if (lane == 0) mbar_arrive(smem_u32(&sm.empty[released % RU]));
+                ++released;
+            }
+#ifdef BLIP_STATS
+            const long long c0 = clock64();
+#endif
+            mbar_wait(smem_u32(&sm.full[waited % RU]), (waited / RU) & 1u);
+#ifdef BLIP_STATS
+            st_pwait += clock64() - c0;
+#endif
+            ++waited;
         }
-        waited = max(waited, need_upto);
-        for (; released < release_below; ++released)
-            if (lane == 0) mbar_arrive(smem_u32(&sm.empty[(released - lo) % R]));
     };
-    auto grab = [&]() -> unsigned {
-        unsigned u = 0;
-        if (lane == 0) u = (unsigned)atomicAdd(&sm.counter, 1);
-        return __shfl_sync(0xffffffffu, u, 0);
+    auto release_upto = [&](unsigned release_end) {      // planes < release_end no longer needed by this warp
+#pragma unroll 1
+        while (released < release_end) {
+            if (lane == 0) mbar_arrive(smem_u32(&sm.empty[released % RU]));
+            ++released;
+        }
     };
-    unsigned u = grab();
-    int cur = 0;
-    if (u < nunits) {
-        if (lane < kRecFloats / 4)
-            reinterpret_cast<float4*>(&sm.rec[warp][0])[lane] = __ldg(rsrc + (size_t)u * (kRecFloats / 4) + lane);
-        __syncwarp();
-    }
-    while (u < nunits) {
-        const unsigned un = grab();
-        float4 pre = make_float4(0.f, 0.f, 0.f, 0.f);
-        if (un < nunits && lane < kRecFloats / 4) pre = __ldg(rsrc + (size_t)un * (kRecFloats / 4) + lane);
 
-        const ElecRec& rec = sm.rec[warp][cur];
-        const int i1 = rec.i[0], i2 = rec.i[1], i3 = rec.i[2], e = rec.e;
-        const bool ok = i1 >= 0;                             // non-finite positions (bin 0) touch no plane
-        const int pl = i1;
+    unsigned n = 0;                    // current item
+    unsigned u = (unsigned)warp;       // current unit of item n
+    bool have = false;                 // sm.rec[warp][cur] already holds the record of (n, u)
+    int cur = 0;
+    int it_nplanes, it_col0 = 0;
+    unsigned it_seq0 = 0, it_nunits = 0;
+    const float4* it_rsrc = recs;
+    auto load_item = [&](unsigned k) {
+        mbar_wait(smem_u32(&sm.ifull[k % IQ]), (k / IQ) & 1u);
+        const WorkItem& it = sm.item[k % IQ];
+        it_nplanes = it.nplanes;
+        if (it_nplanes >= 0) {
+            it_col0 = it.chunk * Cfg::C + lane * VEC;
+            it_seq0 = it.seq0;
+            it_nunits = it.nunits;
+            it_rsrc = recs + (size_t)it.u0 * (kRecFloats / 4);
+        }
+    };
+    load_item(0);
+    const unsigned lane_off = (unsigned)lane * (VEC * 4);
+    const unsigned plane0 = smem_u32(&sm.plane[0][0]);
+    while (true) {
+        while (it_nplanes >= 0 && u >= it_nunits) {          // leave item n: pass all its planes
+            if (it_nplanes > 0) { wait_upto(it_seq0 + it_nplanes); release_upto(it_seq0 + it_nplanes); }
+            __syncwarp();
+            if (lane == 0) mbar_arrive(smem_u32(&sm.iempty[n % IQ]));
+            ++n; u = (unsigned)warp;
+            load_item(n);
+        }
+        if (it_nplanes < 0) break;
+#ifdef BLIP_STATS
+        const long long cu0 = clock64();
+#endif
+        if (!have) {
+            if (lane < kRecFloats / 4)
+                reinterpret_cast<float4*>(&sm.rec[warp][cur])[lane] = __ldg(it_rsrc + (size_t)u * (kRecFloats / 4) + lane);
+            __syncwarp();
+        }
+        const StagedRec& rec = reinterpret_cast<const StagedRec&>(sm.rec[warp][cur]);
+        const int4 loc = rec.loc;                            // {plane in item or -1, byte offset in plane, -, electron}
+        const bool ok = loc.x >= 0;                          // non-finite positions (bin 0) touch no plane
+        const unsigned sq = it_seq0 + (unsigned)loc.x;
+        if (ok) { wait_upto(sq + 4); release_upto(sq); }     // planes i1..i1+3 resident, earlier ones released
+
+        // record of this warp's next unit, in flight during the FMAs
+        const float4* nsrc = nullptr;
+        if (u + NW < it_nunits) nsrc = it_rsrc + (size_t)(u + NW) * (kRecFloats / 4);
+        else {
+            mbar_wait(smem_u32(&sm.ifull[(n + 1) % IQ]), ((n + 1) / IQ) & 1u);     // published before item n's planes
+            const WorkItem& nx = sm.item[(n + 1) % IQ];
+            if (nx.nplanes >= 0 && (unsigned)warp < nx.nunits)
+                nsrc = recs + (size_t)(nx.u0 + (unsigned)warp) * (kRecFloats / 4);
+        }
+        float4 pre = make_float4(0.f, 0.f, 0.f, 0.f);
+        if (nsrc && lane < kRecFloats / 4) pre = __ldg(nsrc + lane);
+#ifdef BLIP_STATS
+        const long long cu1 = clock64();
+#endif
         PairAcc acc[NP];
+        if (!ok) {
 #pragma unroll
-        for (int p = 0; p < NP; ++p) acc[p].val = acc[p].t1 = acc[p].t2 = acc[p].t3 = acc[p].lp = 0ull;
-        if (ok) {
-            advance(pl + 3, pl);                             // planes pl..pl+3 resident, planes < pl released
+            for (int p = 0; p < NP; ++p) set_nan(acc[p]);
+        } else {
+#pragma unroll
+            for (int p = 0; p < NP; ++p) acc[p].val = acc[p].t1 = acc[p].t2 = acc[p].t3 = acc[p].lp = 0ull;
             float wz[3][4];
 #pragma unroll
             for (int k = 0; k < 3; ++k)
 #pragma unroll
                 for (int m = 0; m < 4; ++m) wz[k][m] = rec.wz[k][m];
-            const int r23 = ((i2 - by * BY) * Cfg::PZ + (i3 - bz * BZ)) * Cfg::C + lane * VEC;
+            const unsigned off = (unsigned)loc.y + lane_off;
 #pragma unroll
             for (int m1 = 0; m1 < 4; ++m1) {
-                const float* pp = &sm.plane[(pl + m1 - lo) % R][r23];
+                const unsigned pp = plane0 + ((sq + m1) % RU) * (unsigned)Cfg::PLANE_BYTES + off;
 #pragma unroll
                 for (int m2 = 0; m2 < 4; ++m2) {
-                    const float* cp = pp + m2 * Cfg::PZ * Cfg::C;
+                    const unsigned cp = pp + m2 * (Cfg::PZ * Cfg::C * 4);
                     const float4 w = rec.cw[4 * m1 + m2];
-                    const float lb = rec.lb[4 * m1 + m2];
+                    const float lb = (MODE == 1) ? rec.lb[4 * m1 + m2] : 0.f;
                     if (VEC == 4) {
-                        const ulonglong2 c0 = *reinterpret_cast<const ulonglong2*>(cp);
-                        const ulonglong2 c1 = *reinterpret_cast<const ulonglong2*>(cp + Cfg::C);
-                        const ulonglong2 c2 = *reinterpret_cast<const ulonglong2*>(cp + 2 * Cfg::C);
-                        const ulonglong2 c3 = *reinterpret_cast<const ulonglong2*>(cp + 3 * Cfg::C);
+                        const ulonglong2 c0 = lds128(cp), c1 = lds128(cp + Cfg::C * 4);
+                        const ulonglong2 c2 = lds128(cp + 2 * Cfg::C * 4), c3 = lds128(cp + 3 * Cfg::C * 4);
                         fold_pair<MODE>(c0.x, c1.x, c2.x, c3.x, wz, w, lb, acc[0]);
                         fold_pair<MODE>(c0.y, c1.y, c2.y, c3.y, wz, w, lb, acc[NP - 1]);
                     } else {
-                        const u64 c0 = *reinterpret_cast<const u64*>(cp);
-                        const u64 c1 = *reinterpret_cast<const u64*>(cp + Cfg::C);
-                        const u64 c2 = *reinterpret_cast<const u64*>(cp + 2 * Cfg::C);
-                        const u64 c3 = *reinterpret_cast<const u64*>(cp + 3 * Cfg::C);
+                        const u64 c0 = lds64(cp), c1 = lds64(cp + Cfg::C * 4);
+                        const u64 c2 = lds64(cp + 2 * Cfg::C * 4), c3 = lds64(cp + 3 * Cfg::C * 4);
                         fold_pair<MODE>(c0, c1, c2, c3, wz, w, lb, acc[0]);
                     }
                 }
             }
         }
-        const int col0 = chunk * Cfg::C + lane * VEC;
-        if (col0 < 4 * g.pitch4) store_pairs<MODE, NP>(g, acc, ok, e, col0, val, grad, lap, ld);
+#ifdef BLIP_STATS
+        const long long cu2 = clock64();
+#endif
+#ifdef BLIP_NO_STORE
+        if (it_col0 < 4 * g.pitch4 && loc.w == -12345) store_pairs<MODE, NP>(g, acc, loc.w, it_col0, val, grad, lap, ld);
+#else
+        if (it_col0 < 4 * g.pitch4) store_pairs<MODE, NP>(g, acc, loc.w, it_col0, val, grad, lap, ld);
+#endif
 
-        if (un < nunits && lane < kRecFloats / 4) reinterpret_cast<float4*>(&sm.rec[warp][cur ^ 1])[lane] = pre;
+        have = nsrc != nullptr;
+        if (have) {
+            if (lane < kRecFloats / 4) reinterpret_cast<float4*>(&sm.rec[warp][cur ^ 1])[lane] = pre;
+            cur ^= 1;
+        }
         __syncwarp();
-        cur ^= 1;
-        u = un;
+#ifdef BLIP_STATS
+        ++st_units;
+        st_pro += cu1 - cu0; st_main += cu2 - cu1; st_epi += clock64() - cu2;
+#endif
+        u += NW;
     }
-    __syncwarp();
-    advance(hi, hi + 1);
+#ifdef BLIP_STATS
+    if (lane == 0) {
+        unsigned long long* w = &g_stats[blockIdx.x][2 + 4 * warp];
+        w[0] = st_units; w[1] = st_pwait; w[2] = 0; w[3] = clock64() - st_c0;
+        if (warp == 0) { g_stats[blockIdx.x][1] = gtime();
+                         g_stats[blockIdx.x][5 + 4 * NW] = st_pro; g_stats[blockIdx.x][6 + 4 * NW] = st_main;
+                         g_stats[blockIdx.x][7 + 4 * NW] = st_epi; }
+    }
+#endif
 }
 
 }  // namespace blip

@@ -9,14 +9,70 @@
 #include <cstring>
 #include <new>
 
-// Staged kernel configuration (template constants of blip::eval_staged_kernel).
+// Staged kernel variants (template constants of blip::eval_staged_kernel): pencil cross-section
+// BY x BZ cells, ring of R table planes in shared memory, NW consumer warps.  All use 4 floats
+// per lane (128 orbitals per tile row).  The variant is fixed per table at creation.
 namespace {
-constexpr int kSVec = 4;             // floats per lane -> 128 orbitals per tile row
-constexpr int kSBY = 4, kSBZ = 8;    // pencil cross-section in cells
-constexpr int kSRing = 5;            // table planes resident in shared memory
-constexpr int kSWarps = 8;           // consumer warps (+1 producer warp)
-constexpr int kSSeg = 16;            // cell planes per pencil segment
-using SCfg = blip::StagedCfg<kSVec, kSBY, kSBZ, kSRing, kSWarps>;
+constexpr int kSVec = 4;
+constexpr int kSC = 32 * kSVec;
+
+struct StagedArgs {
+    const CUtensorMap* tmap; const blip::Geom* g; const blip::StagedGeom* sg; const float4* recs;
+    const int4* order; int* meta; int nchunk;
+    float* val; float* grad; float* lap; long long ld;
+};
+
+struct StagedVariant {
+    int by, bz, ring, warps;
+    size_t smem;
+    cudaError_t (*prepare)();
+    void (*launch)(int mode, unsigned nctas, cudaStream_t s, const StagedArgs& a);
+};
+
+template <int BY, int BZ, int R, int NW>
+struct SV {
+    using Cfg = blip::StagedCfg<kSVec, BY, BZ, R, NW>;
+    static cudaError_t prepare()
+    {
+        const int smem = (int)sizeof(typename Cfg::Smem);
+        cudaError_t e = cudaFuncSetAttribute(blip::eval_staged_kernel<0, kSVec, BY, BZ, R, NW>,
+                                             cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+        if (e == cudaSuccess)
+            e = cudaFuncSetAttribute(blip::eval_staged_kernel<1, kSVec, BY, BZ, R, NW>,
+                                     cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+        if (e == cudaSuccess)
+            e = cudaFuncSetAttribute(blip::eval_staged_kernel<2, kSVec, BY, BZ, R, NW>,
+                                     cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+        return e;
+    }
+    static void launch(int mode, unsigned nctas, cudaStream_t s, const StagedArgs& a)
+    {
+        const size_t smem = sizeof(typename Cfg::Smem);
+        if (mode == 0)
+            blip::eval_staged_kernel<0, kSVec, BY, BZ, R, NW><<<nctas, Cfg::THREADS, smem, s>>>(
+                *a.tmap, *a.g, *a.sg, a.recs, a.order, a.meta, a.nchunk, a.val, a.grad, a.lap, a.ld);
+        else if (mode == 2)
+            blip::eval_staged_kernel<2, kSVec, BY, BZ, R, NW><<<nctas, Cfg::THREADS, smem, s>>>(
+                *a.tmap, *a.g, *a.sg, a.recs, a.order, a.meta, a.nchunk, a.val, a.grad, a.lap, a.ld);
+        else
+            blip::eval_staged_kernel<1, kSVec, BY, BZ, R, NW><<<nctas, Cfg::THREADS, smem, s>>>(
+                *a.tmap, *a.g, *a.sg, a.recs, a.order, a.meta, a.nchunk, a.val, a.grad, a.lap, a.ld);
+    }
+    static constexpr StagedVariant variant() { return {BY, BZ, R, NW, sizeof(typename Cfg::Smem), &prepare, &launch}; }
+};
+
+const StagedVariant kVariants[] = {
+    SV<4, 8, 5, 8>::variant(),  SV<4, 8, 5, 12>::variant(),
+    SV<4, 4, 8, 8>::variant(),  SV<4, 4, 8, 12>::variant(), SV<4, 4, 8, 16>::variant(),
+};
+constexpr int kNumVariants = (int)(sizeof(kVariants) / sizeof(kVariants[0]));
+constexpr int kDefaultVariant = 2;
+
+int env_int(const char* name, int dflt)
+{
+    const char* v = std::getenv(name);
+    return v ? std::atoi(v) : dflt;
+}
 }
 
 struct blipgpu_table {
@@ -29,9 +85,15 @@ struct blipgpu_table {
     int nbins = 0;                   // max(bricks, staged bins)
     int nbins_direct = 0, nbins_staged = 0;
     int nq = 1;                      // direct kernel: quads of 4 orbitals per lane (1..3)
+    int diag = 0;                    // lattice vectors along the Cartesian axes: J diagonal (kernel MODE 2)
     int path = 0;                    // 0 auto, 1 direct, 2 staged
     int staged_ok = 0;               // TMA descriptor built and the grid is large enough
+    const StagedVariant* sv = nullptr;
+    int nchunk = 0;                  // staged path: orbital chunks of 128
+    int nsm = 0;                     // SMs of the device (CTAs of the persistent staged kernel)
     CUtensorMap tmap;
+    int4* order = nullptr;           // [sg.nps] work items {segment, first unit, units, 0}, heaviest first
+    int* meta = nullptr;             // [2] {non-empty pencil segments, work counter}
     // grouping workspace (device)
     long long cap = 0;               // electrons the workspace holds
     int* bin = nullptr;              // [cap]
@@ -102,9 +164,7 @@ static int ensure_workspace(blipgpu_table* t, long long M, cudaStream_t s)
 {
     if (M <= t->cap) return BLIPGPU_OK;
     CK(t, cudaStreamSynchronize(s));
-    if (t->bin) cudaFree(t->bin);
-    if (t->perm) cudaFree(t->perm);
-    if (t->recs) cudaFree(t->recs);
+    cudaFree(t->bin); cudaFree(t->perm); cudaFree(t->recs);
     t->bin = t->perm = nullptr; t->recs = nullptr; t->cap = 0;
     CK(t, cudaMalloc(&t->bin, sizeof(int) * (size_t)M));
     CK(t, cudaMalloc(&t->perm, sizeof(int) * (size_t)M));
@@ -133,7 +193,7 @@ static bool build_tensor_map(blipgpu_table* t)
     const cuuint64_t dims[4] = {(cuuint64_t)t->pitch, (cuuint64_t)t->g.np[2], (cuuint64_t)t->g.np[1],
                                 (cuuint64_t)t->g.np[0]};
     const cuuint64_t strides[3] = {pitchB, pitchB * t->g.np[2], pitchB * t->g.np[2] * t->g.np[1]};
-    const cuuint32_t box[4] = {(cuuint32_t)SCfg::C, (cuuint32_t)SCfg::PZ, (cuuint32_t)SCfg::PY, 1u};
+    const cuuint32_t box[4] = {(cuuint32_t)kSC, (cuuint32_t)(t->sv->bz + 3), (cuuint32_t)(t->sv->by + 3), 1u};
     const cuuint32_t estr[4] = {1u, 1u, 1u, 1u};
     const CUresult r = ((encode_fn)fn)(&t->tmap, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 4, t->table, dims, strides, box,
                                        estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
@@ -178,6 +238,10 @@ extern "C" int blipgpu_create(const double* lattice, const int* grid, int norb,
             t->g.J[3 * a + i] = (float)Jd[a][i];
         }
     }
+    t->diag = 1;
+    for (int a = 0; a < 3; ++a)
+        for (int i = 0; i < 3; ++i)
+            if (a != i && Jd[a][i] != 0.0) t->diag = 0;
     const int qa[6] = {0, 1, 2, 0, 0, 1}, qb[6] = {0, 1, 2, 1, 2, 2};
     for (int k = 0; k < 6; ++k)
         t->g.Q[k] = (float)(Jd[qa[k]][0] * Jd[qb[k]][0] + Jd[qa[k]][1] * Jd[qb[k]][1]
@@ -187,14 +251,34 @@ extern "C" int blipgpu_create(const double* lattice, const int* grid, int norb,
     t->nrows = nrows;
     t->g.L = norb;
     t->g.pitch4 = (int)(pitch / 4);
-    t->sg.by = kSBY; t->sg.bz = kSBZ;
-    t->sg.nby = (grid[1] + kSBY - 1) / kSBY;
-    t->sg.nbz = (grid[2] + kSBZ - 1) / kSBZ;
-    t->sg.seg = kSSeg;
-    t->sg.nseg = (grid[0] + kSSeg - 1) / kSSeg;
+    int vi = env_int("BLIPGPU_SCFG", kDefaultVariant);
+    if (vi < 0 || vi >= kNumVariants) vi = kDefaultVariant;
+    t->sv = &kVariants[vi];
+    t->nsm = prop.multiProcessorCount;
+    t->nchunk = (int)((pitch + kSC - 1) / kSC);
+    t->sg.by = t->sv->by; t->sg.bz = t->sv->bz;
+    t->sg.nby = (grid[1] + t->sg.by - 1) / t->sg.by;
+    t->sg.nbz = (grid[2] + t->sg.bz - 1) / t->sg.bz;
+    // pencil segments: whole pencils unless that leaves fewer than ~4 work items per SM
+    {
+        int seg = env_int("BLIPGPU_SEG", 0);
+        if (seg <= 0) {
+            seg = grid[0];
+            const long long pencils = (long long)t->sg.nby * t->sg.nbz * t->nchunk;
+            while (seg > 16 && pencils * ((grid[0] + seg - 1) / seg) < 4LL * t->nsm) seg = (seg + 1) / 2;
+        }
+        if (seg > grid[0]) seg = grid[0];
+        t->sg.seg = seg;
+    }
+    t->sg.nseg = (grid[0] + t->sg.seg - 1) / t->sg.seg;
+    t->sg.chunk_major = env_int("BLIPGPU_CHUNK_MAJOR", 1);
+    {
+        const long long nps = (long long)t->sg.nby * t->sg.nbz * t->sg.nseg;
+        t->sg.nps = nps < (1LL << 24) ? (int)nps : 0;
+    }
     t->nbins_direct = t->g.nb[0] * t->g.nb[1] * t->g.nb[2];
     const long long sbins = (long long)t->sg.nby * t->sg.nbz * grid[0];
-    t->nbins_staged = sbins < (1LL << 30) ? (int)sbins : 0;
+    t->nbins_staged = (sbins < (1LL << 30) && t->sg.nps > 0) ? (int)sbins : 0;
     t->nbins = t->nbins_direct > t->nbins_staged ? t->nbins_direct : t->nbins_staged;
     t->nq = default_nq(t->g.pitch4);
 
@@ -210,6 +294,8 @@ extern "C" int blipgpu_create(const double* lattice, const int* grid, int norb,
     float* staging = nullptr;                         // device copy of a host table, until padded
     if ((e = cudaMalloc(&t->table, bytes)) != cudaSuccess) fail(e);
     if (rc == BLIPGPU_OK && (e = cudaMalloc(&t->hist, sizeof(unsigned) * (size_t)t->nbins)) != cudaSuccess) fail(e);
+    if (rc == BLIPGPU_OK && (e = cudaMalloc(&t->order, sizeof(int4) * (size_t)(t->sg.nps + 1))) != cudaSuccess) fail(e);
+    if (rc == BLIPGPU_OK && (e = cudaMalloc(&t->meta, sizeof(int) * 2)) != cudaSuccess) fail(e);
     if (rc == BLIPGPU_OK && !coeffs_on_device) {
         if ((e = cudaMalloc(&staging, src_bytes)) != cudaSuccess) fail(e);
         else if ((e = cudaMemcpyAsync(staging, coeffs, src_bytes, cudaMemcpyHostToDevice, s)) != cudaSuccess) fail(e);
@@ -229,15 +315,10 @@ extern "C" int blipgpu_create(const double* lattice, const int* grid, int norb,
     if (rc == BLIPGPU_OK) {
         // staged path: needs a full tile row (pitch >= C), a grid at least as large as one box,
         // the opt-in shared memory size, and the TMA descriptor
-        const bool fits = t->pitch >= SCfg::C && t->g.np[1] >= SCfg::PY && t->g.np[2] >= SCfg::PZ &&
-                          t->nbins_staged > 0 && (size_t)prop.sharedMemPerBlockOptin >= sizeof(SCfg::Smem);
+        const bool fits = t->pitch >= kSC && t->g.np[1] >= t->sv->by + 3 && t->g.np[2] >= t->sv->bz + 3 &&
+                          t->nbins_staged > 0 && (size_t)prop.sharedMemPerBlockOptin >= t->sv->smem;
         if (fits && build_tensor_map(t)) {
-            const int smem = (int)sizeof(SCfg::Smem);
-            e = cudaFuncSetAttribute(blip::eval_staged_kernel<0, kSVec, kSBY, kSBZ, kSRing, kSWarps>,
-                                     cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
-            if (e == cudaSuccess)
-                e = cudaFuncSetAttribute(blip::eval_staged_kernel<1, kSVec, kSBY, kSBZ, kSRing, kSWarps>,
-                                         cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+            e = t->sv->prepare();
             if (e == cudaSuccess) t->staged_ok = 1; else (void)cudaGetLastError();
         }
     }
@@ -250,6 +331,7 @@ extern "C" int blipgpu_destroy(blipgpu_table* t)
 {
     if (!t) return BLIPGPU_OK;
     cudaFree(t->table); cudaFree(t->bin); cudaFree(t->perm); cudaFree(t->recs); cudaFree(t->hist);
+    cudaFree(t->order); cudaFree(t->meta);
     cudaFree(t->d_pos); cudaFree(t->d_val); cudaFree(t->d_grad); cudaFree(t->d_lap); cudaFree(t->d_cell);
     if (t->copy_stream) cudaStreamDestroy(t->copy_stream);
     for (int k = 0; k < 2; ++k) if (t->ev[k]) cudaEventDestroy(t->ev[k]);
@@ -294,6 +376,7 @@ static int launch_eval(blipgpu_table* t, const double* positions, long long M, i
 {
     const int* perm = nullptr;
     const bool staged = use_staged(t, M);
+    const int kmode = mode == BLIPGPU_VALUE ? 0 : (t->diag ? 2 : 1);      // kernel template MODE
     if (t->profiling) CK(t, cudaEventRecord(t->pe[0], s));
     if (staged || M > kGroupThreshold) {
         int rc = ensure_workspace(t, M, s);
@@ -302,25 +385,22 @@ static int launch_eval(blipgpu_table* t, const double* positions, long long M, i
         CK(t, cudaMemsetAsync(t->hist, 0, sizeof(unsigned) * (size_t)nbins, s));
         const unsigned nb = (unsigned)((M + 255) / 256);
         blip::bin_kernel<<<nb, 256, 0, s>>>(t->g, t->sg, staged ? 1 : 0, positions, M, t->bin, t->hist, cell);
-        blip::scan_kernel<<<1, blip::kScanThreads, 0, s>>>(t->hist, nbins);
-        blip::scatter_kernel<<<nb, 256, 0, s>>>(t->bin, t->hist, M, t->perm);
+        blip::scan_kernel<<<1, blip::kScanThreads, 0, s>>>(t->hist, nbins, M, staged ? 1 : 0, t->g, t->sg,
+                                                          t->order, t->meta);
+        if (staged)
+            blip::scatter_prep_kernel<<<(unsigned)((M + 127) / 128), 128, 0, s>>>(t->g, t->sg, kSC, positions, t->bin,
+                                                                                 t->hist, M, t->recs);
+        else
+            blip::scatter_kernel<<<nb, 256, 0, s>>>(t->bin, t->hist, M, t->perm);
         t->launches += 3;
         perm = t->perm;
         cell = nullptr;                                  // already written by bin_kernel
     }
     if (staged) {
-        blip::prep_kernel<<<(unsigned)((M + 127) / 128), 128, 0, s>>>(t->g, positions, t->perm, M, t->recs);
-        t->launches += 1;
         if (t->profiling) CK(t, cudaEventRecord(t->pe[1], s));
-        const dim3 grid((unsigned)(t->sg.nby * t->sg.nbz * t->sg.nseg),
-                        (unsigned)((t->pitch + SCfg::C - 1) / SCfg::C));
-        const size_t smem = sizeof(SCfg::Smem);
-        if (mode == BLIPGPU_VALUE)
-            blip::eval_staged_kernel<0, kSVec, kSBY, kSBZ, kSRing, kSWarps><<<grid, SCfg::THREADS, smem, s>>>(
-                t->tmap, t->g, t->sg, t->recs, t->hist, val, grad, lap, ld);
-        else
-            blip::eval_staged_kernel<1, kSVec, kSBY, kSBZ, kSRing, kSWarps><<<grid, SCfg::THREADS, smem, s>>>(
-                t->tmap, t->g, t->sg, t->recs, t->hist, val, grad, lap, ld);
+        const StagedArgs a = {&t->tmap, &t->g, &t->sg, t->recs, t->order, t->meta, t->nchunk,
+                              val, grad, lap, ld};
+        t->sv->launch(kmode, (unsigned)t->nsm, s, a);
     } else {
         const int nq = t->nq;
         const dim3 grid((unsigned)((M + blip::kWarpsPerBlock - 1) / blip::kWarpsPerBlock),
@@ -330,8 +410,10 @@ static int launch_eval(blipgpu_table* t, const double* positions, long long M, i
 #define BLIP_LAUNCH(MODE, NQ)                                                                         \
         blip::eval_direct_kernel<MODE, NQ><<<grid, block, 0, s>>>(t->g, t->table, positions, perm, M, \
                                                                   val, grad, lap, ld, cell)
-        if (mode == BLIPGPU_VALUE) {
+        if (kmode == 0) {
             if (nq == 1) BLIP_LAUNCH(0, 1); else if (nq == 2) BLIP_LAUNCH(0, 2); else BLIP_LAUNCH(0, 3);
+        } else if (kmode == 2) {
+            if (nq == 1) BLIP_LAUNCH(2, 1); else if (nq == 2) BLIP_LAUNCH(2, 2); else BLIP_LAUNCH(2, 3);
         } else {
             if (nq == 1) BLIP_LAUNCH(1, 1); else if (nq == 2) BLIP_LAUNCH(1, 2); else BLIP_LAUNCH(1, 3);
         }
@@ -466,6 +548,13 @@ extern "C" int blipgpu_set_tuning(blipgpu_table* t, int path, int nq)
     t->nq = nq ? nq : default_nq(t->g.pitch4);
     return BLIPGPU_OK;
 }
+
+#ifdef BLIP_STATS
+extern "C" int blipgpu_debug_stats(unsigned long long* out)          /* HOST [160][74] */
+{
+    return (int)cudaMemcpyFromSymbol(out, blip::g_stats, sizeof(unsigned long long) * 160 * 74);
+}
+#endif
 
 extern "C" long long blipgpu_launch_count(const blipgpu_table* t) { return t ? t->launches : 0; }
 

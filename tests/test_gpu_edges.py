@@ -76,7 +76,7 @@ def test_staged_path_matches_oracle_and_direct_path(torch_cuda, blip, grid, L, M
         blip.blipgpu_set_tuning(t.handle, path=2)
         n0 = t.launch_count()
         staged = run_gpu(torch_cuda, blip, A, grid, c, pos, mode=mode, table=t)
-        assert t.launch_count() - n0 == 5                # bin, scan, scatter, prep, staged eval
+        assert t.launch_count() - n0 == 4                # bin, scan, scatter+prep, staged eval
         compare(A, grid, c, pos, staged, mode=mode)
         blip.blipgpu_set_tuning(t.handle, path=1)
         direct = run_gpu(torch_cuda, blip, A, grid, c, pos, mode=mode, table=t)
