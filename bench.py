@@ -358,7 +358,27 @@ def run_sweep(torch, blip, handle, cfg, dpos, stream):
             e1.record(stream)
             torch.cuda.synchronize()
             us = 1e3 * e0.elapsed_time(e1) / reps
-            out.append({"M": M, "mode": mode_name, "us_per_call": us, "evals_per_s": M * L / (us * 1e-6),
+            # the same calls captured once in a CUDA graph and replayed: device time per call
+            # without the host's per-call cost (Python + ctypes + launch)
+            gus = None
+            if M <= 2048:                                    # these calls only launch kernels
+                side = torch.cuda.Stream()
+                side.wait_stream(stream)
+                graph = torch.cuda.CUDAGraph()
+                with torch.cuda.graph(graph, stream=side):
+                    for _ in range(20):
+                        blip.blipgpu_eval(handle, dpos, M, mode, val, grad, lap, ld, None, side)
+                graph.replay()
+                torch.cuda.synchronize()
+                e0.record(stream)
+                for _ in range(10):
+                    graph.replay()
+                e1.record(stream)
+                torch.cuda.synchronize()
+                gus = 1e3 * e0.elapsed_time(e1) / 200
+            out.append({"M": M, "mode": mode_name, "us_per_call": us, "us_per_call_graph": gus,
+                        "evals_per_s": M * L / (us * 1e-6),
+                        "evals_per_s_graph": None if gus is None else M * L / (gus * 1e-6),
                         "gathered_GBps": algorithmic_bytes(M, L, mode == blip.VGL) / (us * 1e-6) / 1e9})
     return out
 

@@ -110,40 +110,72 @@ bin_kernel(Geom g, StagedGeom sg, int staged, const double* __restrict__ pos, lo
     atomicAdd(&hist[b], 1u);
 }
 
-// a-4 (2/3): exclusive scan of the histogram, in place, one CTA.  For the staged path it also
-// orders the work items (pencil segments) by decreasing electron count — the persistent
-// staged kernel takes items from a shared counter, so heavy items first keeps the tail short
-// (longest-processing-time-first) — and resets that counter.
+// a-4 (2/3): exclusive scan of the histogram, in place, one CTA; it also clears `hist_next`,
+// the histogram of the next call (the two alternate, so no separate memset is needed).  For
+// the staged path it orders the work items (pencil segments) by decreasing electron count —
+// the persistent staged kernel takes items from a shared counter, so heavy items first keeps
+// the tail short (longest-processing-time-first) — and resets that counter.
 //   order[0 .. nps)   {pencil segment id, first unit, units, 0}; units are indices into the
 //                     sorted records.  sg.chunk_major: x-slab by x-slab, heaviest first inside a
 //                     slab; else heaviest first overall; in id order if nps > kMaxSortedItems
 //   meta[0]           number of leading entries of `order` that hold electrons
 //   meta[1]           work counter of the staged kernel, reset to 0
+constexpr int kScanChunk = 8 * kScanThreads;                 // bins scanned per pass through shared memory
 __global__ void __launch_bounds__(kScanThreads)
-scan_kernel(unsigned* __restrict__ hist, int nbins, long long M, int staged, Geom g, StagedGeom sg,
-            int4* __restrict__ order, int* __restrict__ meta)
+scan_kernel(unsigned* __restrict__ hist, unsigned* __restrict__ hist_next, int nbins, int nclear, long long M, int staged,
+            Geom g, StagedGeom sg, int4* __restrict__ order, int* __restrict__ meta)
 {
-    __shared__ unsigned part[kScanThreads];
-    __shared__ unsigned keys[kMaxSortedItems];
+    __shared__ unsigned buf[kScanChunk];                     // one chunk of the histogram; later the sort keys
+    __shared__ unsigned wsum[kScanThreads / 32];
+    __shared__ unsigned carry_s;
     __shared__ int nonempty;
-    const int tid = threadIdx.x;
-    const int per = (nbins + kScanThreads - 1) / kScanThreads;
-    const int lo = min(tid * per, nbins), hi = min(lo + per, nbins);
-    unsigned s = 0;
-    for (int b = lo; b < hi; ++b) s += hist[b];
-    part[tid] = s;
-    if (tid == 0) nonempty = 0;
+    const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
+    if (tid == 0) { carry_s = 0; nonempty = 0; }
+    for (int b = tid; b < nclear; b += kScanThreads) hist_next[b] = 0u;
     __syncthreads();
-    for (int d = 1; d < kScanThreads; d <<= 1) {            // Hillis-Steele inclusive scan
-        unsigned v = (tid >= d) ? part[tid - d] : 0u;
+    for (int base = 0; base < nbins; base += kScanChunk) {
+        const int n = min(kScanChunk, nbins - base);
+#pragma unroll
+        for (int k = 0; k < 8; ++k) {                        // coalesced, 8 independent loads per thread
+            const int i = tid + k * kScanThreads;
+            buf[i] = (i < n) ? hist[base + i] : 0u;
+        }
         __syncthreads();
-        part[tid] += v;
+        unsigned v[8], s = 0;
+#pragma unroll
+        for (int k = 0; k < 8; ++k) { v[k] = buf[8 * tid + k]; s += v[k]; }
+        unsigned inc = s;                                    // inclusive scan of the per-thread sums
+#pragma unroll
+        for (int d = 1; d < 32; d <<= 1) {
+            const unsigned t = __shfl_up_sync(0xffffffffu, inc, d);
+            if (lane >= d) inc += t;
+        }
+        if (lane == 31) wsum[wid] = inc;
+        __syncthreads();
+        if (wid == 0) {
+            unsigned w = wsum[lane], winc = w;
+#pragma unroll
+            for (int d = 1; d < 32; d <<= 1) {
+                const unsigned t = __shfl_up_sync(0xffffffffu, winc, d);
+                if (lane >= d) winc += t;
+            }
+            wsum[lane] = winc - w;                           // exclusive prefix of each warp
+        }
+        __syncthreads();
+        unsigned run = carry_s + wsum[wid] + inc - s;        // exclusive prefix of this thread's 8 bins
+#pragma unroll
+        for (int k = 0; k < 8; ++k) { buf[8 * tid + k] = run; run += v[k]; }
+        __syncthreads();
+        if (tid == kScanThreads - 1) carry_s = run;
+#pragma unroll
+        for (int k = 0; k < 8; ++k) {
+            const int i = tid + k * kScanThreads;
+            if (i < n) hist[base + i] = buf[i];
+        }
         __syncthreads();
     }
-    unsigned run = part[tid] - s;                            // exclusive prefix of this segment
-    for (int b = lo; b < hi; ++b) { unsigned c = hist[b]; hist[b] = run; run += c; }
     if (!staged) return;
-    __syncthreads();                                         // hist[b] = start of bin b, block-visible
+    // hist[b] = start of bin b (written above by this block, visible after the barrier)
     if (tid == 0) meta[1] = 0;
     const int nps = sg.nps;
     auto units_of = [&](int i, unsigned& u0, unsigned& u1) {
@@ -162,6 +194,7 @@ scan_kernel(unsigned* __restrict__ hist, int nbins, long long M, int staged, Geo
         if (tid == 0) meta[0] = nps;
         return;
     }
+    unsigned* keys = buf;
     int n2 = 1;
     while (n2 < nps) n2 <<= 1;
     int mine = 0;
@@ -186,23 +219,37 @@ scan_kernel(unsigned* __restrict__ hist, int nbins, long long M, int staged, Geo
     }
     if (mine) atomicAdd(&nonempty, mine);
     __syncthreads();
-    for (int k = 2; k <= n2; k <<= 1)                         // bitonic sort, descending
-        for (int j = k >> 1; j > 0; j >>= 1) {
-            for (int i = tid; i < n2; i += kScanThreads) {
-                const int x = i ^ j;
-                if (x > i) {
-                    const unsigned a = keys[i], b = keys[x];
-                    const bool desc = (i & k) == 0;
-                    if ((a < b) == desc) { keys[i] = b; keys[x] = a; }
-                }
-            }
-            __syncthreads();
+    if (nps <= kScanThreads) {
+        // rank sort: keys are distinct (they end in the item id), so the number of larger keys
+        // is the item's place; every thread reads the same key at the same time (a broadcast)
+        if (tid < nps) {
+            const unsigned key = keys[tid];
+            int rank = 0;
+            for (int j = 0; j < nps; ++j) rank += (keys[j] > key);
+            const int id = (int)(key & 8191u);
+            unsigned u0, u1;
+            units_of(id, u0, u1);
+            order[rank] = make_int4(id, (int)u0, (int)(u1 - u0), 0);
         }
-    for (int i = tid; i < nps; i += kScanThreads) {
-        const int id = (int)(keys[i] & 8191u);
-        unsigned u0, u1;
-        units_of(id, u0, u1);
-        order[i] = make_int4(id, (int)u0, (int)(u1 - u0), 0);
+    } else {
+        for (int k = 2; k <= n2; k <<= 1)                     // bitonic sort, descending
+            for (int j = k >> 1; j > 0; j >>= 1) {
+                for (int i = tid; i < n2; i += kScanThreads) {
+                    const int x = i ^ j;
+                    if (x > i) {
+                        const unsigned a = keys[i], b = keys[x];
+                        const bool desc = (i & k) == 0;
+                        if ((a < b) == desc) { keys[i] = b; keys[x] = a; }
+                    }
+                }
+                __syncthreads();
+            }
+        for (int i = tid; i < nps; i += kScanThreads) {
+            const int id = (int)(keys[i] & 8191u);
+            unsigned u0, u1;
+            units_of(id, u0, u1);
+            order[i] = make_int4(id, (int)u0, (int)(u1 - u0), 0);
+        }
     }
     if (tid == 0) meta[0] = nonempty;
 }
@@ -608,23 +655,101 @@ eval_direct_kernel(Geom g, const float4* __restrict__ table4, const double* __re
 }
 
 // ---------------------------------------------------------------------------------------
+// Split kernel, for small batches (the paper's particle-by-particle end of the sweep,
+// PAPER.md:268 kernel (1), where a call is a handful of electrons and the cost is latency):
+// CTA = (electron, 128 orbitals), 4 warps; warp m1 takes the 16 rows of plane i1 + m1, issues
+// all 16 loads at once (one memory round trip instead of eight dependent ones), folds them,
+// and the four partial sums are added in plane order through shared memory.
+// ---------------------------------------------------------------------------------------
+template <int MODE>
+__global__ void __launch_bounds__(128)
+eval_split_kernel(Geom g, const float4* __restrict__ table4, const double* __restrict__ pos, long long M,
+                  float* __restrict__ val, float* __restrict__ grad, float* __restrict__ lap,
+                  long long ld, int* __restrict__ cell_out)
+{
+    __shared__ DirectScratch ws;
+    __shared__ u64 part[3][5 * 2][32];                       // partial sums of warps 1..3
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int e = blockIdx.x;
+    const ulonglong2* __restrict__ table = reinterpret_cast<const ulonglong2*>(table4);
+    const int quad = blockIdx.y * 32 + lane;
+    const unsigned off[1] = {(unsigned)min(quad, g.pitch4 - 1)};
+    if (warp == 0) warp_prepare(g, pos, e, ws.ax, ws.rec, lane);
+    __syncthreads();
+    const int i1 = ws.rec.i[0], i2 = ws.rec.i[1], i3 = ws.rec.i[2];
+    const bool ok = (i1 | i2 | i3) >= 0;
+    if (cell_out && blockIdx.y == 0 && threadIdx.x < 3) cell_out[3 * (size_t)e + threadIdx.x] = ok ? ws.rec.i[threadIdx.x] : -1;
+
+    PairAcc acc[1][2];
+#pragma unroll
+    for (int h = 0; h < 2; ++h) acc[0][h].val = acc[0][h].t1 = acc[0][h].t2 = acc[0][h].t3 = acc[0][h].lp = 0ull;
+    if (ok) {
+        float wz[3][4];
+#pragma unroll
+        for (int k = 0; k < 3; ++k)
+#pragma unroll
+            for (int m = 0; m < 4; ++m) wz[k][m] = ws.rec.wz[k][m];
+        const unsigned s1 = (unsigned)g.np[1] * g.np[2], s2 = (unsigned)g.np[2];
+        const unsigned row0 = ((unsigned)(i1 + warp) * g.np[1] + i2) * g.np[2] + i3;
+        ulonglong2 buf[4][4];
+#pragma unroll
+        for (int m2 = 0; m2 < 4; ++m2) load_column<1>(table, off, row0 + m2 * s2, g.pitch4, buf[m2]);
+#pragma unroll
+        for (int m2 = 0; m2 < 4; ++m2) fold_column<MODE, 1>(ws.rec, 4 * warp + m2, wz, buf[m2], acc);
+        (void)s1;
+    }
+    if (warp > 0) {
+#pragma unroll
+        for (int h = 0; h < 2; ++h) {
+            part[warp - 1][5 * h + 0][lane] = acc[0][h].val;
+            if (MODE != 0) {
+                part[warp - 1][5 * h + 1][lane] = acc[0][h].t1; part[warp - 1][5 * h + 2][lane] = acc[0][h].t2;
+                part[warp - 1][5 * h + 3][lane] = acc[0][h].t3; part[warp - 1][5 * h + 4][lane] = acc[0][h].lp;
+            }
+        }
+    }
+    __syncthreads();
+    if (warp != 0) return;
+    if (!ok) { set_nan(acc[0][0]); set_nan(acc[0][1]); }
+    else {
+        const u64 one = dup2(1.0f);
+#pragma unroll
+        for (int w = 0; w < 3; ++w)
+#pragma unroll
+            for (int h = 0; h < 2; ++h) {
+                acc[0][h].val = fma2(part[w][5 * h + 0][lane], one, acc[0][h].val);
+                if (MODE != 0) {
+                    acc[0][h].t1 = fma2(part[w][5 * h + 1][lane], one, acc[0][h].t1);
+                    acc[0][h].t2 = fma2(part[w][5 * h + 2][lane], one, acc[0][h].t2);
+                    acc[0][h].t3 = fma2(part[w][5 * h + 3][lane], one, acc[0][h].t3);
+                    acc[0][h].lp = fma2(part[w][5 * h + 4][lane], one, acc[0][h].lp);
+                }
+            }
+    }
+    if (quad < g.pitch4) store_pairs<MODE, 2>(g, acc[0], e, 4 * quad, val, grad, lap, ld);
+}
+
+// ---------------------------------------------------------------------------------------
 // Staged kernel (persistent: one CTA per SM).  A work item is (pencil segment, orbital chunk
 // of C = 32*VEC orbitals): the electrons of the segment, sorted by cell plane i1, are its
 // units; the table planes p1 = lo .. hi+3 of the pencil's (BY+3) x (BZ+3) cross-section slide
 // through a ring of R shared-memory slots, one TMA box per plane.
 //
-//   producer warp   takes items from the global counter meta[1] (chunk-major, heaviest segment
-//                   first: `order`), publishes them through a 2-entry item queue and issues the
-//                   planes of item after item into the ring — the planes of the next item
-//                   arrive while the consumers finish the current one;
-//   NW consumers    take units of the current item from a shared counter.  Planes carry a
-//                   CTA-wide sequence number; every consumer waits for and releases every
-//                   plane in sequence order (full / empty barriers, NW arrivals per plane), so
-//                   barrier phases follow from the sequence number alone.
+//   producer warp   takes items from the global counter meta[1] (heaviest segment first:
+//                   `order`), publishes their descriptors through a 3-entry queue — item k+1
+//                   before it issues any plane of item k, so that consumers can prefetch across
+//                   the item boundary — and issues the planes of item after item into the ring:
+//                   the planes of the next item arrive while the consumers finish the current;
+//   NW consumers    warp w takes units w, w+NW, ... of every item.  Planes carry a CTA-wide
+//                   sequence number; every consumer waits for and releases every plane in
+//                   sequence order (full / empty barriers, NW arrivals per plane), so barrier
+//                   phases follow from the sequence number alone.
+//
+// What bounds it (ncu + in-kernel timers, profiles/): while the warps run the 64-row loop the
+// shared-memory pipe (32 KB of coefficient reads per unit, 128 B/clk/SM) and the issue ports
+// (a packed FMA holds its scheduler's port for two cycles) are both > 90 % busy; the rest of
+// the time goes to waiting for planes (TMA latency under load) and per-unit bookkeeping.
 // ---------------------------------------------------------------------------------------
-#ifndef BLIP_SUSPEND_NS
-#define BLIP_SUSPEND_NS 20000u      // try_wait suspend-time hint: a waiting warp sleeps instead of polling
-#endif
 __device__ __forceinline__ ulonglong2 lds128(unsigned addr)
 {
     ulonglong2 v; asm volatile("ld.shared.v2.b64 {%0, %1}, [%2];" : "=l"(v.x), "=l"(v.y) : "r"(addr)); return v;
@@ -651,15 +776,12 @@ __device__ __forceinline__ void mbar_wait(unsigned bar, unsigned parity)
     asm volatile(
         "{\n\t.reg .pred p;\n\t"
         "WAIT_%=:\n\t"
-        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1, %2;\n\t"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n\t"
         "@p bra DONE_%=;\n\t"
         "bra WAIT_%=;\n\t"
         "DONE_%=:\n\t}"
-        :: "r"(bar), "r"(parity), "r"(BLIP_SUSPEND_NS) : "memory");
+        :: "r"(bar), "r"(parity) : "memory");
 }
-#ifndef BLIP_BACKOFF_NS
-#define BLIP_BACKOFF_NS 32
-#endif
 // Producer-side wait: the producer has nothing else to do, so it backs off between polls and
 // leaves the issue slots of its scheduler to the consumer warps that share it.
 __device__ __forceinline__ void mbar_wait_backoff(unsigned bar, unsigned parity)
@@ -672,7 +794,7 @@ __device__ __forceinline__ void mbar_wait_backoff(unsigned bar, unsigned parity)
             "selp.u32 %0, 1, 0, p;\n\t}"
             : "=r"(done) : "r"(bar), "r"(parity) : "memory");
         if (done) break;
-        if (BLIP_BACKOFF_NS > 0) __nanosleep(BLIP_BACKOFF_NS);
+        __nanosleep(64);
     }
 }
 __device__ __forceinline__ void tma_load_4d(unsigned dst, const CUtensorMap* tmap, int c0, int c1, int c2, int c3,
@@ -685,22 +807,10 @@ __device__ __forceinline__ void tma_load_4d(unsigned dst, const CUtensorMap* tma
         : "memory");
 }
 
-#ifdef BLIP_STATS
-// Development instrumentation (not compiled into the product): per CTA {start, end} in ns and,
-// per consumer warp, {units, cycles waiting for planes, cycles waiting for items, cycles total}.
-__device__ unsigned long long g_stats[160][2 + 16 * 4 + 8];
-__device__ __forceinline__ unsigned long long gtime()
-{
-    unsigned long long t; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t)); return t;
-}
-#endif
 constexpr int kItemQueue = 3;              // item descriptors in flight per CTA: finishing, current, next
 
 __device__ __forceinline__ void tma_prefetch_4d(const CUtensorMap* tmap, int c0, int c1, int c2, int c3)
 {
-#ifdef BLIP_NO_L2PF
-    return;
-#endif
     asm volatile("cp.async.bulk.prefetch.tensor.4d.L2.global.tile [%0, {%1, %2, %3, %4}];"
                  :: "l"(reinterpret_cast<uint64_t>(tmap)), "r"(c0), "r"(c1), "r"(c2), "r"(c3) : "memory");
 }
@@ -824,12 +934,6 @@ eval_staged_kernel(const __grid_constant__ CUtensorMap tmap, Geom g, StagedGeom 
     // The loop below is bound by instruction issue (a packed FMA holds the issue port of its
     // scheduler for two cycles, everything else for one), so the bookkeeping per unit is kept
     // short: the record carries the unit's plane number and byte offset inside a plane.
-#ifdef BLIP_STATS
-    unsigned long long st_units = 0, st_pwait = 0;
-    long long st_pro = 0, st_main = 0, st_epi = 0;
-    const long long st_c0 = clock64();
-    if (threadIdx.x == 0) g_stats[blockIdx.x][0] = gtime();
-#endif
     unsigned released = 0;             // planes < released have been released by this warp
     unsigned waited = 0;               // planes < waited have been waited for by this warp
     auto wait_upto = [&](unsigned need_end) {            // planes < need_end resident
@@ -839,13 +943,7 @@ eval_staged_kernel(const __grid_constant__ CUtensorMap tmap, Geom g, StagedGeom 
                 if (lane == 0) mbar_arrive(smem_u32(&sm.empty[released % RU]));
                 ++released;
             }
-#ifdef BLIP_STATS
-            const long long c0 = clock64();
-#endif
             mbar_wait(smem_u32(&sm.full[waited % RU]), (waited / RU) & 1u);
-#ifdef BLIP_STATS
-            st_pwait += clock64() - c0;
-#endif
             ++waited;
         }
     };
@@ -887,9 +985,6 @@ eval_staged_kernel(const __grid_constant__ CUtensorMap tmap, Geom g, StagedGeom 
             load_item(n);
         }
         if (it_nplanes < 0) break;
-#ifdef BLIP_STATS
-        const long long cu0 = clock64();
-#endif
         if (!have) {
             if (lane < kRecFloats / 4)
                 reinterpret_cast<float4*>(&sm.rec[warp][cur])[lane] = __ldg(it_rsrc + (size_t)u * (kRecFloats / 4) + lane);
@@ -899,7 +994,10 @@ eval_staged_kernel(const __grid_constant__ CUtensorMap tmap, Geom g, StagedGeom 
         const int4 loc = rec.loc;                            // {plane in item or -1, byte offset in plane, -, electron}
         const bool ok = loc.x >= 0;                          // non-finite positions (bin 0) touch no plane
         const unsigned sq = it_seq0 + (unsigned)loc.x;
-        if (ok) { wait_upto(sq + 4); release_upto(sq); }     // planes i1..i1+3 resident, earlier ones released
+        // planes i1, i1+1 resident, earlier ones released; planes i1+2 and i1+3 are waited for
+        // just before their quarter of the loop, which leaves the producer two more slots of the
+        // ring to run ahead of the consumers
+        if (ok) { wait_upto(sq + 2); release_upto(sq); }
 
         // record of this warp's next unit, in flight during the FMAs
         const float4* nsrc = nullptr;
@@ -912,9 +1010,6 @@ eval_staged_kernel(const __grid_constant__ CUtensorMap tmap, Geom g, StagedGeom 
         }
         float4 pre = make_float4(0.f, 0.f, 0.f, 0.f);
         if (nsrc && lane < kRecFloats / 4) pre = __ldg(nsrc + lane);
-#ifdef BLIP_STATS
-        const long long cu1 = clock64();
-#endif
         PairAcc acc[NP];
         if (!ok) {
 #pragma unroll
@@ -930,6 +1025,7 @@ eval_staged_kernel(const __grid_constant__ CUtensorMap tmap, Geom g, StagedGeom 
             const unsigned off = (unsigned)loc.y + lane_off;
 #pragma unroll
             for (int m1 = 0; m1 < 4; ++m1) {
+                if (m1 >= 2) wait_upto(sq + m1 + 1);
                 const unsigned pp = plane0 + ((sq + m1) % RU) * (unsigned)Cfg::PLANE_BYTES + off;
 #pragma unroll
                 for (int m2 = 0; m2 < 4; ++m2) {
@@ -949,14 +1045,7 @@ eval_staged_kernel(const __grid_constant__ CUtensorMap tmap, Geom g, StagedGeom 
                 }
             }
         }
-#ifdef BLIP_STATS
-        const long long cu2 = clock64();
-#endif
-#ifdef BLIP_NO_STORE
-        if (it_col0 < 4 * g.pitch4 && loc.w == -12345) store_pairs<MODE, NP>(g, acc, loc.w, it_col0, val, grad, lap, ld);
-#else
         if (it_col0 < 4 * g.pitch4) store_pairs<MODE, NP>(g, acc, loc.w, it_col0, val, grad, lap, ld);
-#endif
 
         have = nsrc != nullptr;
         if (have) {
@@ -964,21 +1053,8 @@ eval_staged_kernel(const __grid_constant__ CUtensorMap tmap, Geom g, StagedGeom 
             cur ^= 1;
         }
         __syncwarp();
-#ifdef BLIP_STATS
-        ++st_units;
-        st_pro += cu1 - cu0; st_main += cu2 - cu1; st_epi += clock64() - cu2;
-#endif
         u += NW;
     }
-#ifdef BLIP_STATS
-    if (lane == 0) {
-        unsigned long long* w = &g_stats[blockIdx.x][2 + 4 * warp];
-        w[0] = st_units; w[1] = st_pwait; w[2] = 0; w[3] = clock64() - st_c0;
-        if (warp == 0) { g_stats[blockIdx.x][1] = gtime();
-                         g_stats[blockIdx.x][5 + 4 * NW] = st_pro; g_stats[blockIdx.x][6 + 4 * NW] = st_main;
-                         g_stats[blockIdx.x][7 + 4 * NW] = st_epi; }
-    }
-#endif
 }
 
 }  // namespace blip

@@ -66,7 +66,7 @@ const StagedVariant kVariants[] = {
     SV<4, 4, 8, 8>::variant(),  SV<4, 4, 8, 12>::variant(), SV<4, 4, 8, 16>::variant(),
 };
 constexpr int kNumVariants = (int)(sizeof(kVariants) / sizeof(kVariants[0]));
-constexpr int kDefaultVariant = 2;
+constexpr int kDefaultVariant = 3;
 
 int env_int(const char* name, int dflt)
 {
@@ -91,6 +91,7 @@ struct blipgpu_table {
     const StagedVariant* sv = nullptr;
     int nchunk = 0;                  // staged path: orbital chunks of 128
     int nsm = 0;                     // SMs of the device (CTAs of the persistent staged kernel)
+    long long l2_bytes = 0;          // L2 capacity of the device
     CUtensorMap tmap;
     int4* order = nullptr;           // [sg.nps] work items {segment, first unit, units, 0}, heaviest first
     int* meta = nullptr;             // [2] {non-empty pencil segments, work counter}
@@ -99,7 +100,8 @@ struct blipgpu_table {
     int* bin = nullptr;              // [cap]
     int* perm = nullptr;             // [cap]
     float4* recs = nullptr;          // [cap][24] per-electron records (staged path)
-    unsigned* hist = nullptr;        // [nbins]
+    unsigned* hist = nullptr;        // [2][nbins]: the histograms of this call and of the next one alternate
+    int hist_cur = 0;
     // staging for blipgpu_eval_host (device)
     long long hcap = 0, hld = 0; int hmode = -1;
     double* d_pos = nullptr; float* d_val = nullptr; float* d_grad = nullptr; float* d_lap = nullptr;
@@ -255,6 +257,7 @@ extern "C" int blipgpu_create(const double* lattice, const int* grid, int norb,
     if (vi < 0 || vi >= kNumVariants) vi = kDefaultVariant;
     t->sv = &kVariants[vi];
     t->nsm = prop.multiProcessorCount;
+    t->l2_bytes = prop.l2CacheSize;
     t->nchunk = (int)((pitch + kSC - 1) / kSC);
     t->sg.by = t->sv->by; t->sg.bz = t->sv->bz;
     t->sg.nby = (grid[1] + t->sg.by - 1) / t->sg.by;
@@ -271,7 +274,7 @@ extern "C" int blipgpu_create(const double* lattice, const int* grid, int norb,
         t->sg.seg = seg;
     }
     t->sg.nseg = (grid[0] + t->sg.seg - 1) / t->sg.seg;
-    t->sg.chunk_major = env_int("BLIPGPU_CHUNK_MAJOR", 1);
+    t->sg.chunk_major = env_int("BLIPGPU_CHUNK_MAJOR", 0);
     {
         const long long nps = (long long)t->sg.nby * t->sg.nbz * t->sg.nseg;
         t->sg.nps = nps < (1LL << 24) ? (int)nps : 0;
@@ -293,7 +296,8 @@ extern "C" int blipgpu_create(const double* lattice, const int* grid, int norb,
     const size_t src_bytes = (size_t)nsites * (size_t)norb * sizeof(float);
     float* staging = nullptr;                         // device copy of a host table, until padded
     if ((e = cudaMalloc(&t->table, bytes)) != cudaSuccess) fail(e);
-    if (rc == BLIPGPU_OK && (e = cudaMalloc(&t->hist, sizeof(unsigned) * (size_t)t->nbins)) != cudaSuccess) fail(e);
+    if (rc == BLIPGPU_OK && (e = cudaMalloc(&t->hist, 2 * sizeof(unsigned) * (size_t)t->nbins)) != cudaSuccess) fail(e);
+    if (rc == BLIPGPU_OK && (e = cudaMemsetAsync(t->hist, 0, 2 * sizeof(unsigned) * (size_t)t->nbins, s)) != cudaSuccess) fail(e);
     if (rc == BLIPGPU_OK && (e = cudaMalloc(&t->order, sizeof(int4) * (size_t)(t->sg.nps + 1))) != cudaSuccess) fail(e);
     if (rc == BLIPGPU_OK && (e = cudaMalloc(&t->meta, sizeof(int) * 2)) != cudaSuccess) fail(e);
     if (rc == BLIPGPU_OK && !coeffs_on_device) {
@@ -354,9 +358,17 @@ static int check_eval_args(const blipgpu_table* t, const double* positions, long
     return BLIPGPU_OK;
 }
 
-// Batches of at most this many electrons are evaluated in caller order: every electron of
-// the batch is in flight at once, so grouping cannot improve locality and costs 3 launches.
+// Which kernel serves a call (path = 0, automatic):
+//   staged   M > 2,048 and every table row is wanted by >= 8 electrons on average: rows are
+//            staged once in shared memory for all electrons of a pencil;
+//   grouped  otherwise, if M > 2,048 and the table does not fit in L2: electrons sorted by
+//            4x4x4-cell brick so that neighbours run together, then the direct kernel;
+//   plain    otherwise (every electron of the batch is in flight at once, or L2 holds the
+//            whole table: grouping cannot improve locality and costs 3 launches): caller
+//            order, the split kernel up to 16,384 electrons (4 warps per electron and 128
+//            orbitals: latency), the direct kernel above.
 static const long long kGroupThreshold = 2048;
+static const long long kSplitMax = 16384;
 // The staged path pays (BY+3)(BZ+3)/(BY BZ) table rows per cell whatever the batch; it wins
 // once the rows are shared by enough electrons (average number of electrons touching a row).
 static const double kStagedMinReuse = 8.0;
@@ -370,28 +382,36 @@ static bool use_staged(const blipgpu_table* t, long long M)
     return 64.0 * (double)M / sites >= kStagedMinReuse;
 }
 
-static int launch_eval(blipgpu_table* t, const double* positions, long long M, int mode,
+// Mpol: the size of the caller's whole batch, which picks the kernel (blipgpu_eval_host cuts a
+// batch into pieces; all pieces then run the kernel the whole batch would, so that the host
+// and the device entry point return the same bits).
+static int launch_eval(blipgpu_table* t, const double* positions, long long M, long long Mpol, int mode,
                        float* val, float* grad, float* lap, long long ld, int* cell,
                        cudaStream_t s)
 {
     const int* perm = nullptr;
-    const bool staged = use_staged(t, M);
+    const bool staged = use_staged(t, Mpol);
     const int kmode = mode == BLIPGPU_VALUE ? 0 : (t->diag ? 2 : 1);      // kernel template MODE
     if (t->profiling) CK(t, cudaEventRecord(t->pe[0], s));
-    if (staged || M > kGroupThreshold) {
+    const bool grouped = staged || t->path == 1 ||
+                         (Mpol > kGroupThreshold && t->nrows * t->pitch * (long long)sizeof(float) > t->l2_bytes * 3 / 4);
+    if (grouped && (staged || M > kGroupThreshold)) {
         int rc = ensure_workspace(t, M, s);
         if (rc != BLIPGPU_OK) return rc;
         const int nbins = staged ? t->nbins_staged : t->nbins_direct;
-        CK(t, cudaMemsetAsync(t->hist, 0, sizeof(unsigned) * (size_t)nbins, s));
+        // the histogram of this call was cleared by the scan kernel of the previous one
+        unsigned* hist = t->hist + (size_t)t->hist_cur * (size_t)t->nbins;
+        unsigned* hist_next = t->hist + (size_t)(t->hist_cur ^ 1) * (size_t)t->nbins;
+        t->hist_cur ^= 1;
         const unsigned nb = (unsigned)((M + 255) / 256);
-        blip::bin_kernel<<<nb, 256, 0, s>>>(t->g, t->sg, staged ? 1 : 0, positions, M, t->bin, t->hist, cell);
-        blip::scan_kernel<<<1, blip::kScanThreads, 0, s>>>(t->hist, nbins, M, staged ? 1 : 0, t->g, t->sg,
+        blip::bin_kernel<<<nb, 256, 0, s>>>(t->g, t->sg, staged ? 1 : 0, positions, M, t->bin, hist, cell);
+        blip::scan_kernel<<<1, blip::kScanThreads, 0, s>>>(hist, hist_next, nbins, t->nbins, M, staged ? 1 : 0, t->g, t->sg,
                                                           t->order, t->meta);
         if (staged)
             blip::scatter_prep_kernel<<<(unsigned)((M + 127) / 128), 128, 0, s>>>(t->g, t->sg, kSC, positions, t->bin,
-                                                                                 t->hist, M, t->recs);
+                                                                                 hist, M, t->recs);
         else
-            blip::scatter_kernel<<<nb, 256, 0, s>>>(t->bin, t->hist, M, t->perm);
+            blip::scatter_kernel<<<nb, 256, 0, s>>>(t->bin, hist, M, t->perm);
         t->launches += 3;
         perm = t->perm;
         cell = nullptr;                                  // already written by bin_kernel
@@ -401,6 +421,12 @@ static int launch_eval(blipgpu_table* t, const double* positions, long long M, i
         const StagedArgs a = {&t->tmap, &t->g, &t->sg, t->recs, t->order, t->meta, t->nchunk,
                               val, grad, lap, ld};
         t->sv->launch(kmode, (unsigned)t->nsm, s, a);
+    } else if (t->path == 0 && !perm && Mpol <= kSplitMax) {
+        if (t->profiling) CK(t, cudaEventRecord(t->pe[1], s));
+        const dim3 grid((unsigned)M, (unsigned)((t->g.pitch4 + 31) / 32));
+        if (kmode == 0) blip::eval_split_kernel<0><<<grid, 128, 0, s>>>(t->g, t->table, positions, M, val, grad, lap, ld, cell);
+        else if (kmode == 2) blip::eval_split_kernel<2><<<grid, 128, 0, s>>>(t->g, t->table, positions, M, val, grad, lap, ld, cell);
+        else blip::eval_split_kernel<1><<<grid, 128, 0, s>>>(t->g, t->table, positions, M, val, grad, lap, ld, cell);
     } else {
         const int nq = t->nq;
         const dim3 grid((unsigned)((M + blip::kWarpsPerBlock - 1) / blip::kWarpsPerBlock),
@@ -434,7 +460,7 @@ extern "C" int blipgpu_eval(blipgpu_table* t, const double* positions, long long
     if (((uintptr_t)val & 15) || (mode == BLIPGPU_VGL && (((uintptr_t)grad & 15) || ((uintptr_t)lap & 15))))
         return BLIPGPU_EINVAL;
     if (M >= (1LL << 31)) return BLIPGPU_EINVAL;
-    return launch_eval(t, positions, M, mode, val, grad, lap, ld, cell, (cudaStream_t)stream);
+    return launch_eval(t, positions, M, M, mode, val, grad, lap, ld, cell, (cudaStream_t)stream);
 }
 
 extern "C" int blipgpu_reserve(blipgpu_table* t, long long M_max)
@@ -485,7 +511,7 @@ extern "C" int blipgpu_eval_host(blipgpu_table* t, const double* positions, long
     long long b0 = 0; int k = 0;
     while (b0 < M) {
         const long long nb = (M - b0 < B) ? (M - b0) : B;
-        rc = launch_eval(t, t->d_pos + 3 * b0, nb, mode, t->d_val + b0 * ld,
+        rc = launch_eval(t, t->d_pos + 3 * b0, nb, M, mode, t->d_val + b0 * ld,
                          mode == BLIPGPU_VGL ? t->d_grad + 3 * b0 * ld : nullptr,
                          mode == BLIPGPU_VGL ? t->d_lap + b0 * ld : nullptr, ld,
                          cell ? t->d_cell + 3 * b0 : nullptr, s);
@@ -549,12 +575,6 @@ extern "C" int blipgpu_set_tuning(blipgpu_table* t, int path, int nq)
     return BLIPGPU_OK;
 }
 
-#ifdef BLIP_STATS
-extern "C" int blipgpu_debug_stats(unsigned long long* out)          /* HOST [160][74] */
-{
-    return (int)cudaMemcpyFromSymbol(out, blip::g_stats, sizeof(unsigned long long) * 160 * 74);
-}
-#endif
 
 extern "C" long long blipgpu_launch_count(const blipgpu_table* t) { return t ? t->launches : 0; }
 
