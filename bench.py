@@ -54,7 +54,9 @@ def algorithmic_bytes(M, L, mode_vgl):
 
 
 def fma_count(M, L, mode_vgl):
-    return M * L * (320 if mode_vgl else 64)
+    """FMAs the kernels issue per evaluation: 16 columns x (12 for the z contraction + 7 folds) for
+    value + gradient + Laplacian, 16 x 5 for value only."""
+    return M * L * (304 if mode_vgl else 80)
 
 
 class ClockSampler:
@@ -271,12 +273,17 @@ def run_gpu(args):
     fp32_peak = 148 * 128 * 2 * sm_max * 1e6                          # FMA lanes x 2 flop x clock
     roofline = {
         "bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-        "traffic": None, "kernel": "blip::eval_kernel (gather + FMA, steps a-1..a-3, a-5)",
+        "traffic": None,
+        "kernel": {1: "blip::eval_direct_kernel", 2: "blip::eval_staged_kernel", 3: "blip::eval_split_kernel"}.get(
+            blip.blipgpu_last_path(handle), "?") + " (gather + FMA, steps a-2, a-3, a-5)",
         "kernel_ms": k_ms, "grouping_ms": g_ms, "kernel_share_of_step": k_ms / (k_ms + g_ms),
         "algorithmic_bytes": abytes, "bytes_per_eval": abytes / (M * L), "peak_source": peak_src,
         "fp32_fma_frac_of_nominal": 2 * fma_count(M, L, mode_vgl) / (k_ms * 1e-3) / fp32_peak,
-        "note": "algorithmic bytes count every gathered coefficient once per electron (R_gather, "
-                "SURVEY.md §8d); L2 reuse between neighbouring electrons lets achieved exceed the HBM peak",
+        "fp32_peak_tflops_nominal": fp32_peak / 1e12,
+        "note": "contract roofline of BASELINE.json north_star: every gathered coefficient (64 x 4 B) and every "
+                "output byte per evaluation at the measured HBM copy rate.  The staged kernel reads each table "
+                "row from HBM about 3 times instead of once per electron (see traffic), so achieved exceeds the "
+                "HBM peak; what binds it is the shared-memory pipe and the FP32 issue ports (DESIGN.md §6)",
     }
     traffic_file = os.path.join(ROOT, "profiles", "traffic.json")     # written from an ncu --set full capture
     if os.path.exists(traffic_file):

@@ -122,12 +122,21 @@ int blipgpu_info(const blipgpu_table* t, int* grid, int* norb, long long* pitch,
                  long long* table_bytes);
 
 /* blipgpu_set_tuning — expert knob; the defaults are chosen from the table and batch shape.
- *   path  0: automatic; 1: always the direct-gather kernel; 2: always the shared-memory
- *            staged kernel (EINVAL if this table cannot use it: fewer than 128 orbitals, a grid
- *            smaller than one staging box, or no TMA descriptor)
+ *   path  0: automatic (staged for dense batches; else the split kernel up to 16,384 positions
+ *            or the direct kernel, after grouping by cell brick when the table exceeds L2);
+ *         1: always the direct-gather kernel (grouped above 2,048 positions);
+ *         2: always the shared-memory staged kernel (EINVAL if this table cannot use it: fewer
+ *            than 128 orbitals, a grid smaller than one staging box, or no TMA descriptor)
  *   nq    direct kernel: quads of 4 orbitals per lane, 1..3; 0 restores the default.
- * Both kernels compute the same arithmetic sequence; results do not depend on the choice. */
+ * The direct and the staged kernel run the same arithmetic sequence and return the same bits;
+ * the split kernel adds the four plane partial sums last, so its results differ from theirs
+ * in the last bits (all are within the stated tolerances of the fp64 definition). */
 int blipgpu_set_tuning(blipgpu_table* t, int path, int nq);
+
+/* blipgpu_last_path — which gather+FMA kernel the last blipgpu_eval / blipgpu_eval_host of this
+ * handle launched: 1 direct (one warp per electron, rows from L2/HBM), 2 staged (table planes
+ * through shared memory), 3 split (four warps per electron, small batches); 0 before any call. */
+int blipgpu_last_path(const blipgpu_table* t);
 
 /* blipgpu_launch_count — number of kernels this handle has launched since creation (the
  * benchmark's "gpu_launches" evidence).  */

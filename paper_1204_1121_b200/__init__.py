@@ -35,6 +35,7 @@ SIGNATURES = {
     "blipgpu_destroy": (ctypes.c_int, [ctypes.c_void_p]),
     "blipgpu_info": (ctypes.c_int, [ctypes.c_void_p, _c_ip, _c_ip, _c_llp, _c_llp]),
     "blipgpu_set_tuning": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_int, ctypes.c_int]),
+    "blipgpu_last_path": (ctypes.c_int, [ctypes.c_void_p]),
     "blipgpu_launch_count": (ctypes.c_longlong, [ctypes.c_void_p]),
     "blipgpu_set_profiling": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_int]),
     "blipgpu_last_kernel_ms": (ctypes.c_int, [ctypes.c_void_p, _c_fp, _c_fp]),
@@ -130,6 +131,11 @@ def blipgpu_destroy(handle):
 def blipgpu_set_tuning(handle, path=0, nq=0):
     """path: 0 auto, 1 direct-gather kernel, 2 staged kernel; nq: direct kernel quads per lane (0 = default)."""
     _check(lib().blipgpu_set_tuning(handle, int(path), int(nq)), "blipgpu_set_tuning", handle)
+
+
+def blipgpu_last_path(handle):
+    """1 direct, 2 staged, 3 split: the gather+FMA kernel of the handle's last evaluation."""
+    return int(lib().blipgpu_last_path(handle))
 
 
 def blipgpu_launch_count(handle):

@@ -663,14 +663,14 @@ eval_direct_kernel(Geom g, const float4* __restrict__ table4, const double* __re
 // ---------------------------------------------------------------------------------------
 template <int MODE>
 __global__ void __launch_bounds__(128)
-eval_split_kernel(Geom g, const float4* __restrict__ table4, const double* __restrict__ pos, long long M,
-                  float* __restrict__ val, float* __restrict__ grad, float* __restrict__ lap,
+eval_split_kernel(Geom g, const float4* __restrict__ table4, const double* __restrict__ pos,
+                  const int* __restrict__ perm, long long M, float* __restrict__ val, float* __restrict__ grad, float* __restrict__ lap,
                   long long ld, int* __restrict__ cell_out)
 {
     __shared__ DirectScratch ws;
     __shared__ u64 part[3][5 * 2][32];                       // partial sums of warps 1..3
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    const int e = blockIdx.x;
+    const int e = perm ? perm[blockIdx.x] : (int)blockIdx.x;
     const ulonglong2* __restrict__ table = reinterpret_cast<const ulonglong2*>(table4);
     const int quad = blockIdx.y * 32 + lane;
     const unsigned off[1] = {(unsigned)min(quad, g.pitch4 - 1)};

@@ -113,6 +113,7 @@ struct blipgpu_table {
     int profiling = 0;
     cudaEvent_t pe[3] = {nullptr, nullptr, nullptr};   // call start, eval kernel start, end
     int last_cuda = 0;
+    int last_path = 0;               // gather+FMA kernel of the last eval: 1 direct, 2 staged, 3 split
     long long launches = 0;
 };
 
@@ -159,7 +160,7 @@ static int default_nq(int pitch4)
         const int v = std::atoi(env);
         if (v >= 1 && v <= 3) return v;
     }
-    return pitch4 <= 32 ? 1 : 2;
+    return pitch4 <= 32 ? 1 : (pitch4 < 96 ? 2 : 3);         // measured on the 1,536-orbital table: 3 > 1 > 2
 }
 
 static int ensure_workspace(blipgpu_table* t, long long M, cudaStream_t s)
@@ -421,13 +422,16 @@ static int launch_eval(blipgpu_table* t, const double* positions, long long M, l
         const StagedArgs a = {&t->tmap, &t->g, &t->sg, t->recs, t->order, t->meta, t->nchunk,
                               val, grad, lap, ld};
         t->sv->launch(kmode, (unsigned)t->nsm, s, a);
+        t->last_path = 2;
     } else if (t->path == 0 && !perm && Mpol <= kSplitMax) {
+        t->last_path = 3;
         if (t->profiling) CK(t, cudaEventRecord(t->pe[1], s));
         const dim3 grid((unsigned)M, (unsigned)((t->g.pitch4 + 31) / 32));
-        if (kmode == 0) blip::eval_split_kernel<0><<<grid, 128, 0, s>>>(t->g, t->table, positions, M, val, grad, lap, ld, cell);
-        else if (kmode == 2) blip::eval_split_kernel<2><<<grid, 128, 0, s>>>(t->g, t->table, positions, M, val, grad, lap, ld, cell);
-        else blip::eval_split_kernel<1><<<grid, 128, 0, s>>>(t->g, t->table, positions, M, val, grad, lap, ld, cell);
+        if (kmode == 0) blip::eval_split_kernel<0><<<grid, 128, 0, s>>>(t->g, t->table, positions, perm, M, val, grad, lap, ld, cell);
+        else if (kmode == 2) blip::eval_split_kernel<2><<<grid, 128, 0, s>>>(t->g, t->table, positions, perm, M, val, grad, lap, ld, cell);
+        else blip::eval_split_kernel<1><<<grid, 128, 0, s>>>(t->g, t->table, positions, perm, M, val, grad, lap, ld, cell);
     } else {
+        t->last_path = 1;
         const int nq = t->nq;
         const dim3 grid((unsigned)((M + blip::kWarpsPerBlock - 1) / blip::kWarpsPerBlock),
                         (unsigned)((t->g.pitch4 + 32 * nq - 1) / (32 * nq)));
@@ -575,6 +579,8 @@ extern "C" int blipgpu_set_tuning(blipgpu_table* t, int path, int nq)
     return BLIPGPU_OK;
 }
 
+
+extern "C" int blipgpu_last_path(const blipgpu_table* t) { return t ? t->last_path : 0; }
 
 extern "C" long long blipgpu_launch_count(const blipgpu_table* t) { return t ? t->launches : 0; }
 
