@@ -77,6 +77,14 @@ __device__ __forceinline__ bool cell_map_axis(const Geom& g, int a, double x, do
     return true;
 }
 
+// First statement of every kernel of a call: with programmatic stream serialization the kernel
+// may already be resident while its predecessor runs; this returns when the predecessor has
+// completed and flushed its writes (a no-op for a plain launch).
+__device__ __forceinline__ void wait_for_predecessor()
+{
+    asm volatile("griddepcontrol.wait;" ::: "memory");
+}
+
 __device__ __forceinline__ int brick_of(const Geom& g, int i0, int i1, int i2)
 {
     return ((i0 / kBrick) * g.nb[1] + (i1 / kBrick)) * g.nb[2] + (i2 / kBrick);
@@ -95,6 +103,7 @@ __global__ void __launch_bounds__(256)
 bin_kernel(Geom g, StagedGeom sg, int staged, const double* __restrict__ pos, long long M,
            int* __restrict__ bin, unsigned* __restrict__ hist, int* __restrict__ cell)
 {
+    wait_for_predecessor();
     long long e = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (e >= M) return;
     double x = pos[3 * e], y = pos[3 * e + 1], z = pos[3 * e + 2];
@@ -130,6 +139,7 @@ scan_kernel(unsigned* __restrict__ hist, unsigned* __restrict__ hist_next, int n
     __shared__ unsigned carry_s;
     __shared__ int nonempty;
     const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
+    wait_for_predecessor();
     if (tid == 0) { carry_s = 0; nonempty = 0; }
     for (int b = tid; b < nclear; b += kScanThreads) hist_next[b] = 0u;
     __syncthreads();
@@ -261,6 +271,7 @@ __global__ void __launch_bounds__(256)
 scatter_kernel(const int* __restrict__ bin, unsigned* __restrict__ offs, long long M,
                int* __restrict__ perm)
 {
+    wait_for_predecessor();
     long long e = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (e >= M) return;
     unsigned slot = atomicAdd(&offs[bin[e]], 1u);
@@ -400,6 +411,7 @@ scatter_prep_kernel(Geom g, StagedGeom sg, int tile_floats, const double* __rest
                     const int* __restrict__ bin, unsigned* __restrict__ offs, long long M,
                     float4* __restrict__ recs)
 {
+    wait_for_predecessor();
     const long long el = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (el >= M) return;
     const int e = (int)el;
@@ -864,6 +876,7 @@ eval_staged_kernel(const __grid_constant__ CUtensorMap tmap, Geom g, StagedGeom 
     constexpr unsigned RU = R;
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    wait_for_predecessor();
     if (threadIdx.x == 0) {
         for (int s = 0; s < R; ++s) { mbar_init(smem_u32(&sm.full[s]), 1); mbar_init(smem_u32(&sm.empty[s]), NW); }
         for (int s = 0; s < (int)IQ; ++s) { mbar_init(smem_u32(&sm.ifull[s]), 1); mbar_init(smem_u32(&sm.iempty[s]), NW); }

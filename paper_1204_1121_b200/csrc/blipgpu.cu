@@ -13,6 +13,22 @@
 // BY x BZ cells, ring of R table planes in shared memory, NW consumer warps.  All use 4 floats
 // per lane (128 orbitals per tile row).  The variant is fixed per table at creation.
 namespace {
+// Launch with programmatic stream serialization: the kernel may be set up on the device while
+// its predecessor in the stream still runs; it starts with griddepcontrol.wait, which returns
+// once the predecessor has completed and its writes are visible — stream order is kept, the
+// launch latency between the dependent kernels of one call is hidden.
+template <typename... KArgs, typename... Args>
+cudaError_t launch_pdl(void (*kernel)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t s, Args... args)
+{
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = grid; cfg.blockDim = block; cfg.dynamicSmemBytes = smem; cfg.stream = s;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = attr; cfg.numAttrs = 1;
+    return cudaLaunchKernelEx(&cfg, kernel, KArgs(args)...);
+}
+
 constexpr int kSVec = 4;
 constexpr int kSC = 32 * kSVec;
 
@@ -49,14 +65,14 @@ struct SV {
     {
         const size_t smem = sizeof(typename Cfg::Smem);
         if (mode == 0)
-            blip::eval_staged_kernel<0, kSVec, BY, BZ, R, NW><<<nctas, Cfg::THREADS, smem, s>>>(
-                *a.tmap, *a.g, *a.sg, a.recs, a.order, a.meta, a.nchunk, a.val, a.grad, a.lap, a.ld);
+            launch_pdl(blip::eval_staged_kernel<0, kSVec, BY, BZ, R, NW>, nctas, Cfg::THREADS, smem, s,
+                       *a.tmap, *a.g, *a.sg, a.recs, a.order, a.meta, a.nchunk, a.val, a.grad, a.lap, a.ld);
         else if (mode == 2)
-            blip::eval_staged_kernel<2, kSVec, BY, BZ, R, NW><<<nctas, Cfg::THREADS, smem, s>>>(
-                *a.tmap, *a.g, *a.sg, a.recs, a.order, a.meta, a.nchunk, a.val, a.grad, a.lap, a.ld);
+            launch_pdl(blip::eval_staged_kernel<2, kSVec, BY, BZ, R, NW>, nctas, Cfg::THREADS, smem, s,
+                       *a.tmap, *a.g, *a.sg, a.recs, a.order, a.meta, a.nchunk, a.val, a.grad, a.lap, a.ld);
         else
-            blip::eval_staged_kernel<1, kSVec, BY, BZ, R, NW><<<nctas, Cfg::THREADS, smem, s>>>(
-                *a.tmap, *a.g, *a.sg, a.recs, a.order, a.meta, a.nchunk, a.val, a.grad, a.lap, a.ld);
+            launch_pdl(blip::eval_staged_kernel<1, kSVec, BY, BZ, R, NW>, nctas, Cfg::THREADS, smem, s,
+                       *a.tmap, *a.g, *a.sg, a.recs, a.order, a.meta, a.nchunk, a.val, a.grad, a.lap, a.ld);
     }
     static constexpr StagedVariant variant() { return {BY, BZ, R, NW, sizeof(typename Cfg::Smem), &prepare, &launch}; }
 };
@@ -405,14 +421,14 @@ static int launch_eval(blipgpu_table* t, const double* positions, long long M, l
         unsigned* hist_next = t->hist + (size_t)(t->hist_cur ^ 1) * (size_t)t->nbins;
         t->hist_cur ^= 1;
         const unsigned nb = (unsigned)((M + 255) / 256);
-        blip::bin_kernel<<<nb, 256, 0, s>>>(t->g, t->sg, staged ? 1 : 0, positions, M, t->bin, hist, cell);
-        blip::scan_kernel<<<1, blip::kScanThreads, 0, s>>>(hist, hist_next, nbins, t->nbins, M, staged ? 1 : 0, t->g, t->sg,
-                                                          t->order, t->meta);
+        launch_pdl(blip::bin_kernel, nb, 256, 0, s, t->g, t->sg, staged ? 1 : 0, positions, M, t->bin, hist, cell);
+        launch_pdl(blip::scan_kernel, 1, blip::kScanThreads, 0, s, hist, hist_next, nbins, t->nbins, M, staged ? 1 : 0,
+                   t->g, t->sg, t->order, t->meta);
         if (staged)
-            blip::scatter_prep_kernel<<<(unsigned)((M + 127) / 128), 128, 0, s>>>(t->g, t->sg, kSC, positions, t->bin,
-                                                                                 hist, M, t->recs);
+            launch_pdl(blip::scatter_prep_kernel, (unsigned)((M + 127) / 128), 128, 0, s, t->g, t->sg, kSC, positions,
+                       (const int*)t->bin, hist, M, t->recs);
         else
-            blip::scatter_kernel<<<nb, 256, 0, s>>>(t->bin, hist, M, t->perm);
+            launch_pdl(blip::scatter_kernel, nb, 256, 0, s, (const int*)t->bin, hist, M, t->perm);
         t->launches += 3;
         perm = t->perm;
         cell = nullptr;                                  // already written by bin_kernel

@@ -85,6 +85,46 @@ def test_staged_path_matches_oracle_and_direct_path(torch_cuda, blip, grid, L, M
     t.close()
 
 
+def test_axis_aligned_lattice_mode(torch_cuda, blip):
+    """Lattice vectors along the Cartesian axes select the kernels' MODE 2 (diagonal J): staged,
+    direct and split kernels against the oracle, staged and direct bit-identical."""
+    grid, L, M = (11, 9, 14), 140, 5000
+    lat = ((7.0, 0.0, 0.0), (0.0, 8.5, 0.0), (0.0, 0.0, 9.25))
+    A, c, pos = workloads.small_case(grid, L, M, lat, seed=5, spread=2.0)
+    t = blip.BlipTable(A, grid, L, c)
+    out = {}
+    for path in (2, 1):
+        blip.blipgpu_set_tuning(t.handle, path=path)
+        out[path] = run_gpu(torch_cuda, blip, A, grid, c, pos, table=t)
+        assert blip.blipgpu_last_path(t.handle) == path
+        compare(A, grid, c, pos, out[path])
+    for a, b in zip(out[2], out[1]):
+        assert np.array_equal(a, b)
+    blip.blipgpu_set_tuning(t.handle, path=0)             # automatic: dense batch -> staged, small batch -> split
+    run_gpu(torch_cuda, blip, A, grid, c, pos, table=t)
+    assert blip.blipgpu_last_path(t.handle) == 2
+    compare(A, grid, c, pos[:150], run_gpu(torch_cuda, blip, A, grid, c, pos[:150], table=t))
+    assert blip.blipgpu_last_path(t.handle) == 3
+    t.close()
+
+
+def test_staged_path_with_more_work_items_than_the_sorter_takes(torch_cuda, blip):
+    """93 x 93 pencils (> 8,192 work items): the scan kernel leaves the items in id order and
+    the staged kernel skips the empty ones."""
+    grid, L, M = (4, 372, 372), 128, 20000
+    lat = ((3.0, 0.0, 0.0), (0.4, 90.0, 0.0), (0.1, 0.2, 95.0))
+    A, c, pos = workloads.small_case(grid, L, M, lat, seed=21, spread=1.0)
+    t = blip.BlipTable(A, grid, L, c)
+    blip.blipgpu_set_tuning(t.handle, path=2)
+    val, grad, lap, cell = run_gpu(torch_cuda, blip, A, grid, c, pos, table=t)
+    assert blip.blipgpu_last_path(t.handle) == 2
+    ocell, _ = oracle.cellmap(A, grid, pos)
+    assert np.array_equal(cell, ocell)
+    pick = np.arange(0, M, 7)
+    compare(A, grid, c, pos[pick], (val[pick], grad[pick], lap[pick], cell[pick]))
+    t.close()
+
+
 def test_staged_path_clustered_and_non_finite(torch_cuda, blip):
     """All electrons in a few cells (long unit lists per plane, most pencils empty), plus
     non-finite positions, through the staged kernel."""

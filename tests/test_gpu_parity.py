@@ -100,6 +100,7 @@ def test_config_tio2_full_size_sampled(torch_cuda, blip, tio2):
     cfg, A, c, table = tio2
     pos = workloads.positions(cfg)
     val, grad, lap, cell = run_gpu(torch_cuda, blip, A, cfg.grid, c, pos, table=table)
+    assert blip.blipgpu_last_path(table.handle) == 2        # the staged kernel, as in bench.py
     ocell, _ = oracle.cellmap(A, cfg.grid, pos)
     assert np.array_equal(cell, ocell)
     rng = np.random.default_rng(99)
@@ -118,6 +119,7 @@ def test_config_sweep(torch_cuda, blip, tio2, M, mode):
     pos = workloads.positions(cfg, M=M)
     compare(A, cfg.grid, c, pos, run_gpu(torch_cuda, blip, A, cfg.grid, c, pos, mode=mode, table=table),
             mode=mode)
+    assert blip.blipgpu_last_path(table.handle) == 3        # the split kernel
 
 
 # ------------------------------------------------------------------ config 5 (6.3 GB, triclinic)
