@@ -109,6 +109,32 @@ int blipgpu_eval(blipgpu_table* t, const double* positions, long long M, int mod
 int blipgpu_eval_host(blipgpu_table* t, const double* positions, long long M, int mode,
                       float* val, float* grad, float* lap, long long ld, int* cell, void* stream);
 
+/*
+ * blipgpu_eval_contract — evaluate and contract the orbital axis in the same pass (the step the
+ * paper names as next after the orbital evaluation: the determinant update needs
+ * sum_l psi_l(r'_j) (D^-1)_lj for the acceptance ratio of electron j, Eq. 11,
+ * 395-399 §VI.D).  For every position j and the caller's vector d_j:
+ *
+ *     out[j][0]    = sum_l psi_l(r_j) d[j][l]
+ *     out[j][1..3] = sum_l d psi_l / d r_i (r_j) d[j][l]   (i = x, y, z)        VGL only
+ *     out[j][4]    = sum_l nabla^2 psi_l (r_j) d[j][l]                          VGL only
+ *
+ * The [M][L] orbitals are never written: the 20 B per evaluation of output traffic of
+ * blipgpu_eval become 4 B of input.  Asynchronous on `stream` like blipgpu_eval.
+ *
+ *   positions DEVICE [M][3] fp64, as in blipgpu_eval;  mode BLIPGPU_VALUE (out[j][0] only) or VGL
+ *   d         DEVICE [M][ldd] fp32, 16-byte aligned; ldd >= L, ldd % 4 == 0; columns >= L are ignored
+ *   out       DEVICE [M][8] fp32, 16-byte aligned; entries 5..7 (1..7 for VALUE) are set to zero
+ *   cell      DEVICE [M][3] int32, optional
+ *
+ * Sums run in fp32: over the orbitals of a lane, the lanes of a warp, then one atomic add per
+ * 128-orbital tile, so the last bits depend on the order the tiles finish in.  A non-finite
+ * position gives NaN in out[j][0..4].  Errors: EINVAL (NULL pointer, M < 0, bad mode / ldd,
+ * misaligned d or out), ENOMEM, ECUDA.
+ */
+int blipgpu_eval_contract(blipgpu_table* t, const double* positions, long long M, int mode,
+                          const float* d, long long ldd, float* out, int* cell, void* stream);
+
 /* blipgpu_reserve — pre-size the grouping workspace for batches of up to M_max positions
  * (and the staging buffers of blipgpu_eval_host).  Optional.  Errors: EINVAL, ENOMEM, ECUDA. */
 int blipgpu_reserve(blipgpu_table* t, long long M_max);

@@ -110,3 +110,28 @@ def num_threads():
 
 def set_num_threads(t):
     lib().blip_oracle_set_num_threads(int(t))
+
+
+def contract(val, grad, lap, d):
+    """Orbital-axis contraction of oracle results with per-position vectors d [M][L]
+    (Eq. 11, 395-399 §VI.D: sum_l psi_l(r'_j) (D^-1)_lj), written out as the
+    definition, one position and one orbital at a time in fp64:
+        out[j] = (sum_l val[j][l] d[j][l],  sum_l grad[j][i][l] d[j][l] (i = x, y, z),  sum_l lap[j][l] d[j][l])
+    grad / lap may be None (value only: entries 1..4 stay zero).
+    Pins (tests/test_oracle_pins.py): a one-hot d selects one orbital; a constant table gives the sum of d."""
+    val = np.asarray(val, dtype=np.float64)
+    d = np.asarray(d, dtype=np.float64)
+    M, L = val.shape
+    out = np.zeros((M, 5), dtype=np.float64)
+    for j in range(M):
+        s = np.zeros(5)
+        for l in range(L):
+            w = d[j, l]
+            s[0] += val[j, l] * w
+            if grad is not None:
+                s[1] += grad[j, 0, l] * w
+                s[2] += grad[j, 1, l] * w
+                s[3] += grad[j, 2, l] * w
+                s[4] += lap[j, l] * w
+        out[j] = s
+    return out

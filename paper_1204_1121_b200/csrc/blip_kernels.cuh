@@ -568,6 +568,84 @@ __device__ __forceinline__ void store_pairs(const Geom& g, const PairAcc (&acc)[
     }
 }
 
+// Contraction epilogue (§VI.D, Eq. 11): instead of
+// storing the orbitals of electron e, contract them with the caller's vector d_e (column of
+// the inverse Slater matrix in the paper's use):
+//     out[e][0] += sum_l psi_l d_l,  out[e][1..3] += sum_l grad psi_l d_l,  out[e][4] += sum_l lap psi_l d_l
+// over the 2 NP orbitals of this lane (dq: their d values, zero past the last orbital), then
+// over the warp; one atomic add per quantity and (electron, orbital tile).
+template <int MODE, int NP>
+__device__ __forceinline__ void contract_pairs(const Geom& g, const PairAcc (&acc)[NP], const float (&dq)[2 * NP],
+                                               float (&sum)[5])
+{
+#pragma unroll
+    for (int p = 0; p < NP; ++p) {
+        const float2 v = unpack2(acc[p].val);
+        sum[0] = __fmaf_rn(v.x, dq[2 * p], __fmaf_rn(v.y, dq[2 * p + 1], sum[0]));
+        if (MODE != 0) {
+            const float2 a = unpack2(acc[p].t1), b = unpack2(acc[p].t2), c = unpack2(acc[p].t3), l = unpack2(acc[p].lp);
+            sum[1] = __fmaf_rn(a.x, dq[2 * p], __fmaf_rn(a.y, dq[2 * p + 1], sum[1]));
+            sum[2] = __fmaf_rn(b.x, dq[2 * p], __fmaf_rn(b.y, dq[2 * p + 1], sum[2]));
+            sum[3] = __fmaf_rn(c.x, dq[2 * p], __fmaf_rn(c.y, dq[2 * p + 1], sum[3]));
+            sum[4] = __fmaf_rn(l.x, dq[2 * p], __fmaf_rn(l.y, dq[2 * p + 1], sum[4]));
+        }
+    }
+}
+// Grid-space gradient -> Cartesian on the lane's partial sums (linear, so it commutes with the
+// sums over lanes and tiles), then the five sums are added over the warp with 9 shuffles: at
+// each of the first three steps a lane hands half of its values to its partner and keeps the
+// other half, so that lane 4 q ends up with the warp total of quantity q; one atomic add per
+// quantity into out[e][0..4].
+template <int MODE>
+__device__ __forceinline__ void contract_flush(const Geom& g, float (&sum)[5], int e, float* __restrict__ out, int lane)
+{
+    if (MODE == 0) {
+        float r = sum[0];
+#pragma unroll
+        for (int d = 16; d > 0; d >>= 1) r += __shfl_xor_sync(0xffffffffu, r, d);
+        if (lane == 0) atomicAdd(out + 8 * (size_t)e, r);
+        return;
+    }
+    float v[8];
+    v[0] = sum[0];
+    v[1] = __fmaf_rn(g.J[0], sum[1], __fmaf_rn(g.J[3], sum[2], __fmul_rn(g.J[6], sum[3])));
+    v[2] = __fmaf_rn(g.J[1], sum[1], __fmaf_rn(g.J[4], sum[2], __fmul_rn(g.J[7], sum[3])));
+    v[3] = __fmaf_rn(g.J[2], sum[1], __fmaf_rn(g.J[5], sum[2], __fmul_rn(g.J[8], sum[3])));
+    v[4] = sum[4]; v[5] = v[6] = v[7] = 0.f;
+    const bool h16 = lane & 16, h8 = lane & 8, h4 = lane & 4;
+    float w[4], x[2];
+#pragma unroll
+    for (int k = 0; k < 4; ++k) {                            // keep quantity k + 4 [lane bit 4]
+        const float give = h16 ? v[k] : v[k + 4], keep = h16 ? v[k + 4] : v[k];
+        w[k] = keep + __shfl_xor_sync(0xffffffffu, give, 16);
+    }
+#pragma unroll
+    for (int k = 0; k < 2; ++k) {                            // ... + 2 [bit 3]
+        const float give = h8 ? w[k] : w[k + 2], keep = h8 ? w[k + 2] : w[k];
+        x[k] = keep + __shfl_xor_sync(0xffffffffu, give, 8);
+    }
+    const float give = h4 ? x[0] : x[1], keep = h4 ? x[1] : x[0];
+    float r = keep + __shfl_xor_sync(0xffffffffu, give, 4);  // ... + [bit 2]: quantity lane >> 2
+    r += __shfl_xor_sync(0xffffffffu, r, 2);
+    r += __shfl_xor_sync(0xffffffffu, r, 1);
+    if ((lane & 3) == 0 && lane < 20) atomicAdd(out + 8 * (size_t)e + (lane >> 2), r);
+}
+// d values of the 4 orbitals starting at column col0 of electron e, zero at and past column L
+__device__ __forceinline__ float4 ldg_dvec(const float* __restrict__ dvec, long long ldd, int e, int col0)
+{
+    return __ldg(reinterpret_cast<const float4*>(dvec + (size_t)e * (size_t)ldd + col0));
+}
+__device__ __forceinline__ void mask_dvec(const float4& v, int col0, int L, float (&dq)[4])
+{
+    dq[0] = col0 < L ? v.x : 0.f; dq[1] = col0 + 1 < L ? v.y : 0.f;
+    dq[2] = col0 + 2 < L ? v.z : 0.f; dq[3] = col0 + 3 < L ? v.w : 0.f;
+}
+__device__ __forceinline__ void load_dvec(const float* __restrict__ dvec, long long ldd, int e, int col0, int L,
+                                          float (&dq)[4])
+{
+    mask_dvec(ldg_dvec(dvec, ldd, e, col0), col0, L, dq);
+}
+
 // ---------------------------------------------------------------------------------------
 // Direct kernel: warp = (electron, chunk of NQ*128 orbitals); lane owns NQ quads of 4
 // consecutive orbitals, quad q = (chunk*NQ + j)*32 + lane.  grid.x = groups of kWarpsPerBlock
@@ -610,7 +688,8 @@ __global__ void __launch_bounds__(kWarpsPerBlock * 32)
 eval_direct_kernel(Geom g, const float4* __restrict__ table4, const double* __restrict__ pos,
                    const int* __restrict__ perm, long long M,
                    float* __restrict__ val, float* __restrict__ grad, float* __restrict__ lap,
-                   long long ld, int* __restrict__ cell_out)
+                   long long ld, const float* __restrict__ dvec, long long ldd, float* __restrict__ cout,
+                   int* __restrict__ cell_out)
 {
     __shared__ DirectScratch scratch[kWarpsPerBlock];
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
@@ -661,6 +740,18 @@ eval_direct_kernel(Geom g, const float4* __restrict__ table4, const double* __re
             fold_column<MODE, NQ>(ws.rec, c + 1, wz, buf1, acc);
         }
     }
+    if (dvec) {
+        float sum[5] = {0.f, 0.f, 0.f, 0.f, 0.f};
+#pragma unroll
+        for (int j = 0; j < NQ; ++j)
+            if (quad[j] < g.pitch4) {
+                float dq[4];
+                load_dvec(dvec, ldd, e, 4 * quad[j], g.L, dq);
+                contract_pairs<MODE, 2>(g, acc[j], dq, sum);
+            }
+        contract_flush<MODE>(g, sum, e, cout, lane);
+        return;
+    }
 #pragma unroll
     for (int j = 0; j < NQ; ++j)
         if (quad[j] < g.pitch4) store_pairs<MODE, 2>(g, acc[j], e, 4 * quad[j], val, grad, lap, ld);
@@ -677,7 +768,8 @@ template <int MODE>
 __global__ void __launch_bounds__(128)
 eval_split_kernel(Geom g, const float4* __restrict__ table4, const double* __restrict__ pos,
                   const int* __restrict__ perm, long long M, float* __restrict__ val, float* __restrict__ grad, float* __restrict__ lap,
-                  long long ld, int* __restrict__ cell_out)
+                  long long ld, const float* __restrict__ dvec, long long ldd, float* __restrict__ cout,
+                  int* __restrict__ cell_out)
 {
     __shared__ DirectScratch ws;
     __shared__ u64 part[3][5 * 2][32];                       // partial sums of warps 1..3
@@ -737,6 +829,16 @@ eval_split_kernel(Geom g, const float4* __restrict__ table4, const double* __res
                     acc[0][h].lp = fma2(part[w][5 * h + 4][lane], one, acc[0][h].lp);
                 }
             }
+    }
+    if (dvec) {
+        float sum[5] = {0.f, 0.f, 0.f, 0.f, 0.f};
+        if (quad < g.pitch4) {
+            float dq[4];
+            load_dvec(dvec, ldd, e, 4 * quad, g.L, dq);
+            contract_pairs<MODE, 2>(g, acc[0], dq, sum);
+        }
+        contract_flush<MODE>(g, sum, e, cout, lane);
+        return;
     }
     if (quad < g.pitch4) store_pairs<MODE, 2>(g, acc[0], e, 4 * quad, val, grad, lap, ld);
 }
@@ -866,11 +968,12 @@ __global__ void __launch_bounds__((NW + 1) * 32, 1)
 eval_staged_kernel(const __grid_constant__ CUtensorMap tmap, Geom g, StagedGeom sg,
                    const float4* __restrict__ recs, const int4* __restrict__ order, int* __restrict__ meta,
                    int nchunk, float* __restrict__ val, float* __restrict__ grad, float* __restrict__ lap,
-                   long long ld)
+                   long long ld, const float* __restrict__ dvec, long long ldd, float* __restrict__ cout)
 {
     using Cfg = StagedCfg<VEC, BY, BZ, R, NW>;
     extern __shared__ __align__(128) unsigned char smem_raw[];
     typename Cfg::Smem& sm = *reinterpret_cast<typename Cfg::Smem*>(smem_raw);
+    static_assert(VEC == 4, "a lane owns 4 orbitals (one 128-bit load per row)");
     constexpr int NP = VEC / 2;
     constexpr unsigned IQ = kItemQueue;
     constexpr unsigned RU = R;
@@ -1023,6 +1126,8 @@ eval_staged_kernel(const __grid_constant__ CUtensorMap tmap, Geom g, StagedGeom 
         }
         float4 pre = make_float4(0.f, 0.f, 0.f, 0.f);
         if (nsrc && lane < kRecFloats / 4) pre = __ldg(nsrc + lane);
+        float4 dv = make_float4(0.f, 0.f, 0.f, 0.f);        // contraction mode: this lane's d values, in flight during the FMAs
+        if (dvec && it_col0 < 4 * g.pitch4) dv = ldg_dvec(dvec, ldd, loc.w, it_col0);
         PairAcc acc[NP];
         if (!ok) {
 #pragma unroll
@@ -1058,7 +1163,15 @@ eval_staged_kernel(const __grid_constant__ CUtensorMap tmap, Geom g, StagedGeom 
                 }
             }
         }
-        if (it_col0 < 4 * g.pitch4) store_pairs<MODE, NP>(g, acc, loc.w, it_col0, val, grad, lap, ld);
+        if (dvec) {
+            float sum[5] = {0.f, 0.f, 0.f, 0.f, 0.f};
+            if (it_col0 < 4 * g.pitch4) {
+                float dq[4];
+                mask_dvec(dv, it_col0, g.L, dq);
+                contract_pairs<MODE, NP>(g, acc, dq, sum);
+            }
+            contract_flush<MODE>(g, sum, loc.w, cout, lane);
+        } else if (it_col0 < 4 * g.pitch4) store_pairs<MODE, NP>(g, acc, loc.w, it_col0, val, grad, lap, ld);
 
         have = nsrc != nullptr;
         if (have) {

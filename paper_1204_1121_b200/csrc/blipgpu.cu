@@ -36,6 +36,7 @@ struct StagedArgs {
     const CUtensorMap* tmap; const blip::Geom* g; const blip::StagedGeom* sg; const float4* recs;
     const int4* order; int* meta; int nchunk;
     float* val; float* grad; float* lap; long long ld;
+    const float* dvec; long long ldd; float* cout;
 };
 
 struct StagedVariant {
@@ -66,13 +67,13 @@ struct SV {
         const size_t smem = sizeof(typename Cfg::Smem);
         if (mode == 0)
             launch_pdl(blip::eval_staged_kernel<0, kSVec, BY, BZ, R, NW>, nctas, Cfg::THREADS, smem, s,
-                       *a.tmap, *a.g, *a.sg, a.recs, a.order, a.meta, a.nchunk, a.val, a.grad, a.lap, a.ld);
+                       *a.tmap, *a.g, *a.sg, a.recs, a.order, a.meta, a.nchunk, a.val, a.grad, a.lap, a.ld, a.dvec, a.ldd, a.cout);
         else if (mode == 2)
             launch_pdl(blip::eval_staged_kernel<2, kSVec, BY, BZ, R, NW>, nctas, Cfg::THREADS, smem, s,
-                       *a.tmap, *a.g, *a.sg, a.recs, a.order, a.meta, a.nchunk, a.val, a.grad, a.lap, a.ld);
+                       *a.tmap, *a.g, *a.sg, a.recs, a.order, a.meta, a.nchunk, a.val, a.grad, a.lap, a.ld, a.dvec, a.ldd, a.cout);
         else
             launch_pdl(blip::eval_staged_kernel<1, kSVec, BY, BZ, R, NW>, nctas, Cfg::THREADS, smem, s,
-                       *a.tmap, *a.g, *a.sg, a.recs, a.order, a.meta, a.nchunk, a.val, a.grad, a.lap, a.ld);
+                       *a.tmap, *a.g, *a.sg, a.recs, a.order, a.meta, a.nchunk, a.val, a.grad, a.lap, a.ld, a.dvec, a.ldd, a.cout);
     }
     static constexpr StagedVariant variant() { return {BY, BZ, R, NW, sizeof(typename Cfg::Smem), &prepare, &launch}; }
 };
@@ -402,9 +403,11 @@ static bool use_staged(const blipgpu_table* t, long long M)
 // Mpol: the size of the caller's whole batch, which picks the kernel (blipgpu_eval_host cuts a
 // batch into pieces; all pieces then run the kernel the whole batch would, so that the host
 // and the device entry point return the same bits).
+// dvec != NULL: contraction mode (blipgpu_eval_contract): the orbitals are not stored but
+// contracted with dvec[e][.] into cout[e][0..4] (cleared by the caller of this function).
 static int launch_eval(blipgpu_table* t, const double* positions, long long M, long long Mpol, int mode,
                        float* val, float* grad, float* lap, long long ld, int* cell,
-                       cudaStream_t s)
+                       cudaStream_t s, const float* dvec = nullptr, long long ldd = 0, float* cout = nullptr)
 {
     const int* perm = nullptr;
     const bool staged = use_staged(t, Mpol);
@@ -436,16 +439,16 @@ static int launch_eval(blipgpu_table* t, const double* positions, long long M, l
     if (staged) {
         if (t->profiling) CK(t, cudaEventRecord(t->pe[1], s));
         const StagedArgs a = {&t->tmap, &t->g, &t->sg, t->recs, t->order, t->meta, t->nchunk,
-                              val, grad, lap, ld};
+                              val, grad, lap, ld, dvec, ldd, cout};
         t->sv->launch(kmode, (unsigned)t->nsm, s, a);
         t->last_path = 2;
     } else if (t->path == 0 && !perm && Mpol <= kSplitMax) {
         t->last_path = 3;
         if (t->profiling) CK(t, cudaEventRecord(t->pe[1], s));
         const dim3 grid((unsigned)M, (unsigned)((t->g.pitch4 + 31) / 32));
-        if (kmode == 0) blip::eval_split_kernel<0><<<grid, 128, 0, s>>>(t->g, t->table, positions, perm, M, val, grad, lap, ld, cell);
-        else if (kmode == 2) blip::eval_split_kernel<2><<<grid, 128, 0, s>>>(t->g, t->table, positions, perm, M, val, grad, lap, ld, cell);
-        else blip::eval_split_kernel<1><<<grid, 128, 0, s>>>(t->g, t->table, positions, perm, M, val, grad, lap, ld, cell);
+        if (kmode == 0) blip::eval_split_kernel<0><<<grid, 128, 0, s>>>(t->g, t->table, positions, perm, M, val, grad, lap, ld, dvec, ldd, cout, cell);
+        else if (kmode == 2) blip::eval_split_kernel<2><<<grid, 128, 0, s>>>(t->g, t->table, positions, perm, M, val, grad, lap, ld, dvec, ldd, cout, cell);
+        else blip::eval_split_kernel<1><<<grid, 128, 0, s>>>(t->g, t->table, positions, perm, M, val, grad, lap, ld, dvec, ldd, cout, cell);
     } else {
         t->last_path = 1;
         const int nq = t->nq;
@@ -455,7 +458,7 @@ static int launch_eval(blipgpu_table* t, const double* positions, long long M, l
         if (t->profiling) CK(t, cudaEventRecord(t->pe[1], s));
 #define BLIP_LAUNCH(MODE, NQ)                                                                         \
         blip::eval_direct_kernel<MODE, NQ><<<grid, block, 0, s>>>(t->g, t->table, positions, perm, M, \
-                                                                  val, grad, lap, ld, cell)
+                                                                  val, grad, lap, ld, dvec, ldd, cout, cell)
         if (kmode == 0) {
             if (nq == 1) BLIP_LAUNCH(0, 1); else if (nq == 2) BLIP_LAUNCH(0, 2); else BLIP_LAUNCH(0, 3);
         } else if (kmode == 2) {
@@ -481,6 +484,20 @@ extern "C" int blipgpu_eval(blipgpu_table* t, const double* positions, long long
         return BLIPGPU_EINVAL;
     if (M >= (1LL << 31)) return BLIPGPU_EINVAL;
     return launch_eval(t, positions, M, M, mode, val, grad, lap, ld, cell, (cudaStream_t)stream);
+}
+
+extern "C" int blipgpu_eval_contract(blipgpu_table* t, const double* positions, long long M, int mode,
+                                     const float* d, long long ldd, float* out, int* cell, void* stream)
+{
+    if (!t || M < 0) return BLIPGPU_EINVAL;
+    if (mode != BLIPGPU_VALUE && mode != BLIPGPU_VGL) return BLIPGPU_EINVAL;
+    if (ldd < t->L || (ldd % 4) != 0) return BLIPGPU_EINVAL;
+    if (M == 0) return BLIPGPU_OK;
+    if (!positions || !d || !out) return BLIPGPU_EINVAL;
+    if (((uintptr_t)d & 15) || ((uintptr_t)out & 15) || M >= (1LL << 31)) return BLIPGPU_EINVAL;
+    cudaStream_t s = (cudaStream_t)stream;
+    CK(t, cudaMemsetAsync(out, 0, sizeof(float) * 8 * (size_t)M, s));
+    return launch_eval(t, positions, M, M, mode, nullptr, nullptr, nullptr, t->pitch, cell, s, d, ldd, out);
 }
 
 extern "C" int blipgpu_reserve(blipgpu_table* t, long long M_max)

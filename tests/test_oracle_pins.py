@@ -487,3 +487,29 @@ def test_spacing_values_of_the_five_configs():
          for a in range(3)]
     assert np.abs(oracle.spacing(cfg.lattice, cfg.grid) - np.array(h)).max() < 1e-14
     assert abs(max(h) - 24.0 / 112.0) < 1e-15
+
+
+# ------------------------------------------------------------------ contraction
+def test_contract_one_hot_selects_an_orbital_and_constant_table_sums_d():
+    """oracle.contract against what fixes it: d = e_k returns orbital k of eval_fast; a constant
+    table c = kappa gives psi_l = kappa for every l (partition of unity), so out[0] = kappa sum(d)
+    and the derivative entries vanish; linear in d."""
+    rng = np.random.default_rng(5)
+    A, c, pos = workloads.small_case((6, 5, 7), 9, 12, ((5.0, 0.3, -0.2), (1.1, 4.0, 0.7), (-0.6, 0.9, 6.0)), seed=3)
+    val, grad, lap, _ = oracle.eval_fast(A, (6, 5, 7), c, pos)
+    for k in (0, 4, 8):
+        d = np.zeros((12, 9)); d[:, k] = 1.0
+        out = oracle.contract(val, grad, lap, d)
+        assert np.array_equal(out[:, 0], val[:, k]) and np.array_equal(out[:, 1:4], grad[:, :, k])
+        assert np.array_equal(out[:, 4], lap[:, k])
+    d1, d2 = rng.standard_normal((12, 9)), rng.standard_normal((12, 9))
+    lhs = oracle.contract(val, grad, lap, 2.0 * d1 - 3.0 * d2)
+    rhs = 2.0 * oracle.contract(val, grad, lap, d1) - 3.0 * oracle.contract(val, grad, lap, d2)
+    assert np.allclose(lhs, rhs, rtol=0, atol=1e-10)
+    kappa = np.full_like(c, 1.75)
+    v2, g2, l2, _ = oracle.eval_fast(A, (6, 5, 7), kappa, pos)
+    out = oracle.contract(v2, g2, l2, d1)
+    assert np.allclose(out[:, 0], 1.75 * d1.sum(axis=1), rtol=0, atol=1e-12)
+    assert np.abs(out[:, 1:]).max() < 1e-11
+    vo = oracle.contract(val, None, None, d1)
+    assert np.array_equal(vo[:, 0], oracle.contract(val, grad, lap, d1)[:, 0]) and not vo[:, 1:].any()

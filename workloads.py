@@ -120,3 +120,11 @@ def small_case(grid, norb, M, lattice_rows, seed=0, spread=3.0):
     c = rng.standard_normal((*[int(x) for x in grid], norb)).astype(np.float32)
     u = (rng.random((M, 3)) - 0.5) * 2.0 * spread
     return A, c, np.ascontiguousarray(u @ A)
+
+
+def contraction_vectors(M, norb, seed=4):
+    """Per-position vectors d_j [M][norb] fp32 for blipgpu_eval_contract: N(0, 1/norb) entries, the
+    scale of a column of the inverse of a well-conditioned norb x norb Slater matrix
+    (the paper's matrices are not available)."""
+    rng = np.random.default_rng(seed)
+    return (rng.standard_normal((int(M), int(norb)), dtype=np.float32) / np.float32(np.sqrt(norb)))
