@@ -948,7 +948,7 @@ struct StagedCfg {
     static constexpr int THREADS = (NW + 1) * 32;
     struct Smem {
         alignas(128) float plane[R][PLANE_FLOATS];
-        alignas(16) ElecRec rec[NW][2];
+        alignas(16) ElecRec rec[NW];                         // one record per consumer warp; the next one waits in registers
         alignas(16) WorkItem item[kItemQueue];
         alignas(8) u64 full[R];
         alignas(8) u64 empty[R];
@@ -1073,8 +1073,7 @@ eval_staged_kernel(const __grid_constant__ CUtensorMap tmap, Geom g, StagedGeom 
 
     unsigned n = 0;                    // current item
     unsigned u = (unsigned)warp;       // current unit of item n
-    bool have = false;                 // sm.rec[warp][cur] already holds the record of (n, u)
-    int cur = 0;
+    bool have = false;                 // sm.rec[warp] already holds the record of (n, u)
     int it_nplanes, it_col0 = 0;
     unsigned it_seq0 = 0, it_nunits = 0;
     const float4* it_rsrc = recs;
@@ -1103,10 +1102,10 @@ eval_staged_kernel(const __grid_constant__ CUtensorMap tmap, Geom g, StagedGeom 
         if (it_nplanes < 0) break;
         if (!have) {
             if (lane < kRecFloats / 4)
-                reinterpret_cast<float4*>(&sm.rec[warp][cur])[lane] = __ldg(it_rsrc + (size_t)u * (kRecFloats / 4) + lane);
+                reinterpret_cast<float4*>(&sm.rec[warp])[lane] = __ldg(it_rsrc + (size_t)u * (kRecFloats / 4) + lane);
             __syncwarp();
         }
-        const StagedRec& rec = reinterpret_cast<const StagedRec&>(sm.rec[warp][cur]);
+        const StagedRec& rec = reinterpret_cast<const StagedRec&>(sm.rec[warp]);
         const int4 loc = rec.loc;                            // {plane in item or -1, byte offset in plane, -, electron}
         const bool ok = loc.x >= 0;                          // non-finite positions (bin 0) touch no plane
         const unsigned sq = it_seq0 + (unsigned)loc.x;
@@ -1174,10 +1173,8 @@ eval_staged_kernel(const __grid_constant__ CUtensorMap tmap, Geom g, StagedGeom 
         } else if (it_col0 < 4 * g.pitch4) store_pairs<MODE, NP>(g, acc, loc.w, it_col0, val, grad, lap, ld);
 
         have = nsrc != nullptr;
-        if (have) {
-            if (lane < kRecFloats / 4) reinterpret_cast<float4*>(&sm.rec[warp][cur ^ 1])[lane] = pre;
-            cur ^= 1;
-        }
+        __syncwarp();                                        // every lane is done with this unit's record
+        if (have && lane < kRecFloats / 4) reinterpret_cast<float4*>(&sm.rec[warp])[lane] = pre;
         __syncwarp();
         u += NW;
     }
