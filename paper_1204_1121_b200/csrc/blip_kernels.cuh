@@ -1070,6 +1070,20 @@ eval_staged_kernel(const __grid_constant__ CUtensorMap tmap, Geom g, StagedGeom 
             ++released;
         }
     };
+    // Planes < end that this warp does not read (between two of its units, or to the end of an
+    // item): each is given back as soon as it has been waited for.  Holding them until the
+    // next wait forces it would let the producer issue plane q only when the consumers
+    // already stand waiting for it, i.e. put the full copy latency on every plane passed.
+    auto pass_upto = [&](unsigned end) {
+        release_upto(min(waited, end));
+#pragma unroll 1
+        while (waited < end) {
+            mbar_wait(smem_u32(&sm.full[waited % RU]), (waited / RU) & 1u);
+            if (lane == 0) mbar_arrive(smem_u32(&sm.empty[waited % RU]));
+            ++waited;
+            released = waited;
+        }
+    };
 
     unsigned n = 0;                    // current item
     unsigned u = (unsigned)warp;       // current unit of item n
@@ -1093,7 +1107,7 @@ eval_staged_kernel(const __grid_constant__ CUtensorMap tmap, Geom g, StagedGeom 
     const unsigned plane0 = smem_u32(&sm.plane[0][0]);
     while (true) {
         while (it_nplanes >= 0 && u >= it_nunits) {          // leave item n: pass all its planes
-            if (it_nplanes > 0) { wait_upto(it_seq0 + it_nplanes); release_upto(it_seq0 + it_nplanes); }
+            if (it_nplanes > 0) pass_upto(it_seq0 + it_nplanes);
             __syncwarp();
             if (lane == 0) mbar_arrive(smem_u32(&sm.iempty[n % IQ]));
             ++n; u = (unsigned)warp;
@@ -1112,7 +1126,7 @@ eval_staged_kernel(const __grid_constant__ CUtensorMap tmap, Geom g, StagedGeom 
         // planes i1, i1+1 resident, earlier ones released; planes i1+2 and i1+3 are waited for
         // just before their quarter of the loop, which leaves the producer two more slots of the
         // ring to run ahead of the consumers
-        if (ok) { wait_upto(sq + 2); release_upto(sq); }
+        if (ok) { pass_upto(sq); wait_upto(sq + 2); }
 
         // record of this warp's next unit, in flight during the FMAs
         const float4* nsrc = nullptr;

@@ -377,7 +377,7 @@ static int check_eval_args(const blipgpu_table* t, const double* positions, long
 }
 
 // Which kernel serves a call (path = 0, automatic):
-//   staged   M > 2,048 and every table row is wanted by >= 8 electrons on average: rows are
+//   staged   M > 2,048 and every table row is wanted by >= 6 electrons on average: rows are
 //            staged once in shared memory for all electrons of a pencil;
 //   grouped  otherwise, if M > 2,048 and the table does not fit in L2: electrons sorted by
 //            4x4x4-cell brick so that neighbours run together, then the direct kernel;
@@ -389,7 +389,7 @@ static const long long kGroupThreshold = 2048;
 static const long long kSplitMax = 16384;
 // The staged path pays (BY+3)(BZ+3)/(BY BZ) table rows per cell whatever the batch; it wins
 // once the rows are shared by enough electrons (average number of electrons touching a row).
-static const double kStagedMinReuse = 8.0;
+static const double kStagedMinReuse = 6.0;
 
 static bool use_staged(const blipgpu_table* t, long long M)
 {
