@@ -67,8 +67,8 @@ STAGED_CASES = [((9, 10, 13), 130, 3000, TRICLINIC), ((20, 7, 8), 128, 1200, SKE
 
 @pytest.mark.parametrize("grid,L,M,lat", STAGED_CASES)
 def test_staged_path_matches_oracle_and_direct_path(torch_cuda, blip, grid, L, M, lat):
-    """The staged kernel forced on grids that are ragged against the 4x8 pencil cross-section and
-    the 16-plane segments, orbital counts that are not a multiple of the 128-orbital tile, and
+    """The staged kernel forced on grids that are ragged against the 4x4 pencil cross-section,
+    orbital counts that are not a multiple of the 128-orbital tile, and
     pencils without electrons: parity with the oracle, and bit-identical to the direct kernel."""
     A, c, pos = workloads.small_case(grid, L, M, lat, seed=L + M, spread=3.0)
     t = blip.BlipTable(A, grid, L, c)
