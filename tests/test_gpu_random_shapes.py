@@ -1,0 +1,69 @@
+"""Seeded random shapes through every kernel (staged, direct, split; storing and contracting
+epilogues; both modes) against the oracle: grids 4..39 per axis, orbital counts around the
+4- and 128-orbital boundaries, batch sizes around the grouping and kernel-selection thresholds,
+axis-aligned and triclinic lattices, positions from a few cells to +-30 cells away, a few
+non-finite positions."""
+import numpy as np
+import pytest
+
+import oracle
+import workloads
+from test_gpu_parity import tolerances, torch_cuda, blip  # noqa: F401 (fixtures)
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.mark.parametrize("seed", range(24))
+def test_random_shape(torch_cuda, blip, seed):
+    torch = torch_cuda
+    rng = np.random.default_rng(1000 + seed)
+    grid = tuple(int(x) for x in rng.integers(4, 40, size=3))
+    L = int(rng.choice([1, 7, 64, 128, 129, 200, 256, 300, 513]))
+    M = int(rng.choice([1, 5, 33, 700, 2049, 5000, 20000]))
+    if rng.random() < 0.4:
+        lat = np.diag(rng.uniform(3, 12, size=3))
+    else:
+        lat = np.diag(rng.uniform(5, 12, size=3)) + rng.uniform(-1.5, 1.5, size=(3, 3))
+    path = int(rng.choice([0, 0, 1, 2]))
+    mode = int(rng.choice([0, 1, 1]))
+    contract = rng.random() < 0.3
+    spread = float(rng.choice([0.05, 1.0, 3.0, 30.0]))
+    A, c, pos = workloads.small_case(grid, L, M, lat, seed=seed, spread=spread)
+    if rng.random() < 0.3 and M > 3:
+        pos[rng.integers(0, M, size=2)] = np.nan
+    t = blip.BlipTable(A, grid, L, c)
+    if blip.lib().blipgpu_set_tuning(t.handle, path, 0) != blip.OK:      # staged path not available for this table
+        blip.blipgpu_set_tuning(t.handle, 0, 0)
+    dpos = torch.from_numpy(pos).cuda()
+    oval, ograd, olap, ocell = oracle.eval_fast(A, grid, c, pos, mode=mode)
+    tv, tg, tl = tolerances(A, grid, float(np.abs(c).max()))
+    good = ~np.isnan(oval).any(axis=1)
+    if contract:
+        d = rng.standard_normal((M, L)).astype(np.float32)
+        ldd = (L + 3) // 4 * 4
+        dd = torch.zeros((M, ldd), dtype=torch.float32, device="cuda")
+        dd[:, :L] = torch.from_numpy(d).cuda()
+        out = torch.empty((M, 8), dtype=torch.float32, device="cuda")
+        blip.blipgpu_eval_contract(t.handle, dpos, M, mode, dd, ldd, out)
+        torch.cuda.synchronize()
+        out = out.cpu().numpy()
+        assert np.isnan(out[~good, 0]).all()
+        if good.any():
+            ref = oracle.contract(oval[good], ograd[good] if mode else None, olap[good] if mode else None, d[good])
+            w = float(np.abs(d).sum(axis=1).max())
+            assert np.abs(out[good, 0] - ref[:, 0]).max() <= tv * w
+            if mode:
+                assert np.abs(out[good, 1:4] - ref[:, 1:4]).max() <= tg * w
+                assert np.abs(out[good, 4] - ref[:, 4]).max() <= tl * w
+    else:
+        val, grad, lap, cell = t.eval(dpos, mode=mode, want_cell=True)
+        torch.cuda.synchronize()
+        val = val.cpu().numpy()
+        assert np.array_equal(cell.cpu().numpy(), ocell)
+        assert np.isnan(val[~good]).all()
+        if good.any():
+            assert np.abs(val[good] - oval[good]).max() <= tv
+            if mode:
+                assert np.abs(grad.cpu().numpy()[good] - ograd[good]).max() <= tg
+                assert np.abs(lap.cpu().numpy()[good] - olap[good]).max() <= tl
+    t.close()
