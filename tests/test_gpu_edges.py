@@ -252,3 +252,35 @@ def test_argument_errors(torch_cuda, blip):
                           None, None, 8, None, None) == blip.EINVAL
     torch.cuda.synchronize()
     t.close()
+
+
+def test_distinct_handles_on_distinct_streams(torch_cuda, blip):
+    """include/blipgpu.h: "distinct handles are independent".  Three tables evaluated at the same
+    time on three streams (persistent staged kernels competing for the SMs) return the bits of
+    their stand-alone evaluation."""
+    torch = torch_cuda
+    cases = []
+    for k, (grid, L, M) in enumerate([((17, 12, 19), 257, 9000), ((9, 10, 13), 130, 30000), ((20, 7, 8), 128, 12000)]):
+        A, c, pos = workloads.small_case(grid, L, M, TRICLINIC, seed=k, spread=3.0)
+        t = blip.BlipTable(A, grid, L, c)
+        blip.blipgpu_set_tuning(t.handle, path=2)
+        dpos = torch.from_numpy(pos).cuda()
+        ref = [x.clone() for x in t.eval(dpos, mode=blip.VGL)[:3]]
+        cases.append((t, dpos, ref, torch.cuda.Stream()))
+    torch.cuda.synchronize()
+    for _ in range(5):
+        outs = []
+        for t, dpos, ref, st in cases:
+            with torch.cuda.stream(st):
+                M, ld = dpos.shape[0], t.ld
+                val = torch.empty((M, ld), dtype=torch.float32, device="cuda")
+                grad = torch.empty((M, 3, ld), dtype=torch.float32, device="cuda")
+                lap = torch.empty((M, ld), dtype=torch.float32, device="cuda")
+                blip.blipgpu_eval(t.handle, dpos, M, blip.VGL, val, grad, lap, ld, None, st)
+                outs.append((val, grad, lap))
+        torch.cuda.synchronize()
+        for (t, dpos, ref, st), o in zip(cases, outs):
+            L = ref[0].shape[1]
+            assert torch.equal(o[0][:, :L], ref[0]) and torch.equal(o[1][:, :, :L], ref[1]) and torch.equal(o[2][:, :L], ref[2])
+    for t, *_ in cases:
+        t.close()
