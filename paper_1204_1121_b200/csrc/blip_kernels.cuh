@@ -850,10 +850,11 @@ eval_split_kernel(Geom g, const float4* __restrict__ table4, const double* __res
 // through a ring of R shared-memory slots, one TMA box per plane.
 //
 //   producer warp   takes items from the global counter meta[1] (heaviest segment first:
-//                   `order`), publishes their descriptors through a 3-entry queue — item k+1
-//                   before it issues any plane of item k, so that consumers can prefetch across
-//                   the item boundary — and issues the planes of item after item into the ring:
-//                   the planes of the next item arrive while the consumers finish the current;
+//                   `order`), publishes their descriptors through a 3-entry queue — item k+1 as
+//                   soon as the last plane of item k is issued, so that consumers can prefetch
+//                   across the item boundary — and issues the planes of item after item into
+//                   the ring: the planes of the next item arrive while the consumers finish
+//                   the current one;
 //   NW consumers    warp w takes units w, w+NW, ... of every item.  Planes carry a CTA-wide
 //                   sequence number; every consumer waits for and releases every plane in
 //                   sequence order (full / empty barriers, NW arrivals per plane), so barrier
@@ -884,6 +885,16 @@ __device__ __forceinline__ void mbar_expect_tx(unsigned bar, unsigned bytes)
 __device__ __forceinline__ void mbar_arrive(unsigned bar)
 {
     asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" :: "r"(bar) : "memory");
+}
+__device__ __forceinline__ bool mbar_test(unsigned bar, unsigned parity)
+{
+    unsigned done;
+    asm volatile(
+        "{\n\t.reg .pred p;\n\t"
+        "mbarrier.test_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
+        "selp.u32 %0, 1, 0, p;\n\t}"
+        : "=r"(done) : "r"(bar), "r"(parity) : "memory");
+    return done != 0;
 }
 __device__ __forceinline__ void mbar_wait(unsigned bar, unsigned parity)
 {
@@ -957,12 +968,13 @@ struct StagedCfg {
     };
 };
 
-// Deadlock freedom of the two queues.  The producer publishes item k+1 before it issues any
-// plane of item k, and needs for that only the descriptor slot of item k-2, which every
-// consumer gives back when it leaves item k-2.  A consumer looks at the descriptor of item
-// k+1 (to prefetch its first record) only while it works on a unit of item k, i.e. after it
-// has left item k-1 and released all planes of it; so whatever a consumer waits for never
-// depends on something that consumer still holds.
+// Deadlock freedom of the two queues.  The producer takes and publishes item k+1 once every
+// plane of item k is issued; for that it needs ring slots, which consumers give back as they
+// move through item k, and the descriptor slot of item k-2, which every consumer gives back
+// when it leaves item k-2.  A consumer waits for the descriptor of item k+1 only after it has
+// left item k and released all of its planes; while it still works on a unit of item k it
+// only looks whether the descriptor is there yet (to prefetch its first record of item k+1).
+// So whatever a consumer waits for never depends on something that consumer still holds.
 template <int MODE, int VEC, int BY, int BZ, int R, int NW>
 __global__ void __launch_bounds__((NW + 1) * 32, 1)
 eval_staged_kernel(const __grid_constant__ CUtensorMap tmap, Geom g, StagedGeom sg,
@@ -1025,7 +1037,6 @@ eval_staged_kernel(const __grid_constant__ CUtensorMap tmap, Geom g, StagedGeom 
             unsigned seq = 0;
             Desc cur = fetch(0);
             for (unsigned k = 0; cur.nplanes >= 0; ++k) {
-                const Desc nxt = fetch(k + 1);
                 for (int j = 0; j < cur.nplanes; ++j, ++seq) {
                     const unsigned slot = seq % RU, round = seq / RU;
                     if (j + R < cur.nplanes)
@@ -1036,7 +1047,10 @@ eval_staged_kernel(const __grid_constant__ CUtensorMap tmap, Geom g, StagedGeom 
                     tma_load_4d(smem_u32(&sm.plane[slot][0]), &tmap, cur.chunk * Cfg::C, cur.bz * BZ, cur.by * BY,
                                 cur.lo + j, bar);
                 }
-                cur = nxt;
+                // the next item is taken from the global queue only now, when the consumers are
+                // within a ring of the end of this one: a CTA never sits on a queued item while
+                // another CTA runs dry
+                cur = fetch(k + 1);
             }
         }
         return;
@@ -1132,10 +1146,14 @@ eval_staged_kernel(const __grid_constant__ CUtensorMap tmap, Geom g, StagedGeom 
         const float4* nsrc = nullptr;
         if (u + NW < it_nunits) nsrc = it_rsrc + (size_t)(u + NW) * (kRecFloats / 4);
         else {
-            mbar_wait(smem_u32(&sm.ifull[(n + 1) % IQ]), ((n + 1) / IQ) & 1u);     // published before item n's planes
-            const WorkItem& nx = sm.item[(n + 1) % IQ];
-            if (nx.nplanes >= 0 && (unsigned)warp < nx.nunits)
-                nsrc = recs + (size_t)(nx.u0 + (unsigned)warp) * (kRecFloats / 4);
+            // the next item, if the producer has published it already (it does so once all planes
+            // of this one are issued; waiting for it here, with this unit's planes pinned, could
+            // starve the producer of ring slots)
+            if (mbar_test(smem_u32(&sm.ifull[(n + 1) % IQ]), ((n + 1) / IQ) & 1u)) {
+                const WorkItem& nx = sm.item[(n + 1) % IQ];
+                if (nx.nplanes >= 0 && (unsigned)warp < nx.nunits)
+                    nsrc = recs + (size_t)(nx.u0 + (unsigned)warp) * (kRecFloats / 4);
+            }
         }
         float4 pre = make_float4(0.f, 0.f, 0.f, 0.f);
         if (nsrc && lane < kRecFloats / 4) pre = __ldg(nsrc + lane);
