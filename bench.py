@@ -364,6 +364,7 @@ def run_gpu(args):
             line["sweep"] = run_sweep(torch, blip, handle, cfg, dpos, stream)
         if mode_vgl and not args.no_contract:
             line["contract"] = run_contract(torch, blip, handle, cfg, hpos, dpos, stream, args)
+            line["f64"] = run_f64(torch, blip, handle, cfg, dpos, stream)
     blip.blipgpu_destroy(handle)
     if dist is not None:
         dist.barrier()
@@ -409,6 +410,27 @@ def run_contract(torch, blip, handle, cfg, hpos, dpos, stream, args):
             "e2e_ms_per_step": 1e3 * dt, "e2e_evals_per_s": M * L / dt, "h2d_bytes_per_step": int(ppos.numel() * 8),
             "d2h_bytes_per_step": int(M * 8 * 4), "checksum": float(pout[:, 0].double().sum()),
             "note": "d [M][L] fp32 resident on the device (151 MB read per step instead of 755 MB written)"}
+
+
+def run_f64(torch, blip, handle, cfg, dpos, stream):
+    """blipgpu_eval_f64 (fp64 weights, accumulation, outputs) on one walker's
+    worth of positions — the paper's local-energy call."""
+    M, L = min(int(dpos.shape[0]), max(1, cfg.electrons)), cfg.norb
+    ld = (L + 3) // 4 * 4
+    val = torch.empty((M, ld), dtype=torch.float64, device="cuda")
+    grad = torch.empty((M, 3, ld), dtype=torch.float64, device="cuda")
+    lap = torch.empty((M, ld), dtype=torch.float64, device="cuda")
+    for _ in range(3):
+        blip.blipgpu_eval_f64(handle, dpos, M, blip.VGL, val, grad, lap, ld, None, stream)
+    torch.cuda.synchronize()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record(stream)
+    for _ in range(20):
+        blip.blipgpu_eval_f64(handle, dpos, M, blip.VGL, val, grad, lap, ld, None, stream)
+    e1.record(stream)
+    torch.cuda.synchronize()
+    ms = e0.elapsed_time(e1) / 20
+    return {"api": "blipgpu_eval_f64", "positions": M, "ms_per_call": ms, "evals_per_s": M * L / (ms * 1e-3), "dtype": "f64"}
 
 
 def run_sweep(torch, blip, handle, cfg, dpos, stream):

@@ -135,6 +135,26 @@ int blipgpu_eval_host(blipgpu_table* t, const double* positions, long long M, in
 int blipgpu_eval_contract(blipgpu_table* t, const double* positions, long long M, int mode,
                           const float* d, long long ldd, float* out, int* cell, void* stream);
 
+/*
+ * blipgpu_eval_f64 — the same evaluation with fp64 weights, fp64 accumulation and fp64 outputs
+ * from the resident fp32 table.  The paper keeps the local-energy evaluation in double
+ * precision on the CPU because the bias of single-precision orbitals in the energy is
+ * untested, and uses the fp32 values only for accept/reject; this entry
+ * point lets that occasional call stay on the device.  Results agree with the fp64 definition
+ * to rounding (~1e-14 relative to max|c| x weights).  It is the accuracy path, not the fast
+ * one: one CTA per (position, 128 orbitals), no grouping, about 1/2 the FMA rate.
+ *
+ *   positions DEVICE [M][3] fp64;  mode BLIPGPU_VALUE or BLIPGPU_VGL
+ *   val  DEVICE [M][ld] fp64;  grad DEVICE [M][3][ld] fp64;  lap DEVICE [M][ld] fp64 (VGL only)
+ *   ld   row pitch in doubles, >= L, multiple of 4; outputs 16-byte aligned
+ *   cell DEVICE [M][3] int32, optional
+ *
+ * Non-finite positions give NaN outputs and cell = -1.  Asynchronous on `stream`.
+ * Errors: EINVAL (as blipgpu_eval), ECUDA.
+ */
+int blipgpu_eval_f64(blipgpu_table* t, const double* positions, long long M, int mode,
+                     double* val, double* grad, double* lap, long long ld, int* cell, void* stream);
+
 /* blipgpu_reserve — pre-size the grouping workspace for batches of up to M_max positions
  * (and the staging buffers of blipgpu_eval_host).  Optional.  Errors: EINVAL, ENOMEM, ECUDA. */
 int blipgpu_reserve(blipgpu_table* t, long long M_max);
@@ -161,7 +181,8 @@ int blipgpu_set_tuning(blipgpu_table* t, int path, int nq);
 
 /* blipgpu_last_path — which gather+FMA kernel the last blipgpu_eval / blipgpu_eval_host of this
  * handle launched: 1 direct (one warp per electron, rows from L2/HBM), 2 staged (table planes
- * through shared memory), 3 split (four warps per electron, small batches); 0 before any call. */
+ * through shared memory), 3 split (four warps per electron, small batches), 4 the fp64 kernel of blipgpu_eval_f64; 0 before
+ * any call. */
 int blipgpu_last_path(const blipgpu_table* t);
 
 /* blipgpu_launch_count — number of kernels this handle has launched since creation (the

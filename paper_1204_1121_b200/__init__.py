@@ -34,6 +34,9 @@ SIGNATURES = {
     "blipgpu_eval_contract": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_void_p, ctypes.c_longlong, ctypes.c_int,
                                              ctypes.c_void_p, ctypes.c_longlong, ctypes.c_void_p,
                                              ctypes.c_void_p, ctypes.c_void_p]),
+    "blipgpu_eval_f64": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_void_p, ctypes.c_longlong, ctypes.c_int,
+                                        ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p,
+                                        ctypes.c_longlong, ctypes.c_void_p, ctypes.c_void_p]),
     "blipgpu_reserve": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_longlong]),
     "blipgpu_destroy": (ctypes.c_int, [ctypes.c_void_p]),
     "blipgpu_info": (ctypes.c_int, [ctypes.c_void_p, _c_ip, _c_ip, _c_llp, _c_llp]),
@@ -127,6 +130,12 @@ def blipgpu_eval_contract(handle, positions, M, mode, d, ldd, out, cell=None, st
     rc = lib().blipgpu_eval_contract(handle, _ptr(positions), int(M), int(mode), _ptr(d), int(ldd), _ptr(out),
                                      _ptr(cell), _stream_ptr(stream))
     _check(rc, "blipgpu_eval_contract", handle)
+
+
+def blipgpu_eval_f64(handle, positions, M, mode, val, grad, lap, ld, cell=None, stream=None):
+    rc = lib().blipgpu_eval_f64(handle, _ptr(positions), int(M), int(mode), _ptr(val), _ptr(grad), _ptr(lap),
+                                int(ld), _ptr(cell), _stream_ptr(stream))
+    _check(rc, "blipgpu_eval_f64", handle)
 
 
 def blipgpu_reserve(handle, M_max):

@@ -8,7 +8,7 @@ ROOT = os.path.dirname(HERE)
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libblipgpu.so")
 SOURCES = [os.path.join(CSRC, "blipgpu.cu")]
-DEPS = SOURCES + [os.path.join(CSRC, "blip_kernels.cuh"), os.path.join(ROOT, "include", "blipgpu.h")]
+DEPS = SOURCES + [os.path.join(CSRC, "blip_kernels.cuh"), os.path.join(CSRC, "blip_f64.cuh"), os.path.join(ROOT, "include", "blipgpu.h")]
 
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",

@@ -3,6 +3,7 @@
 // step of the hot path itself runs in the kernels of blip_kernels.cuh.
 #include "blipgpu.h"
 #include "blip_kernels.cuh"
+#include "blip_f64.cuh"
 
 #include <cmath>
 #include <cstdlib>
@@ -94,6 +95,7 @@ int env_int(const char* name, int dflt)
 
 struct blipgpu_table {
     blip::Geom g;
+    blip::Geom64 g64;                // J and Q in fp64, for blipgpu_eval_f64
     blip::StagedGeom sg;
     int L = 0;
     long long pitch = 0;             // floats per table row (multiple of 4)
@@ -256,6 +258,7 @@ extern "C" int blipgpu_create(const double* lattice, const int* grid, int norb,
         for (int i = 0; i < 3; ++i) {
             Jd[a][i] = (double)grid[a] * t->g.G[3 * i + a];
             t->g.J[3 * a + i] = (float)Jd[a][i];
+            t->g64.J[3 * a + i] = Jd[a][i];
         }
     }
     t->diag = 1;
@@ -263,9 +266,10 @@ extern "C" int blipgpu_create(const double* lattice, const int* grid, int norb,
         for (int i = 0; i < 3; ++i)
             if (a != i && Jd[a][i] != 0.0) t->diag = 0;
     const int qa[6] = {0, 1, 2, 0, 0, 1}, qb[6] = {0, 1, 2, 1, 2, 2};
-    for (int k = 0; k < 6; ++k)
-        t->g.Q[k] = (float)(Jd[qa[k]][0] * Jd[qb[k]][0] + Jd[qa[k]][1] * Jd[qb[k]][1]
-                            + Jd[qa[k]][2] * Jd[qb[k]][2]);
+    for (int k = 0; k < 6; ++k) {
+        t->g64.Q[k] = Jd[qa[k]][0] * Jd[qb[k]][0] + Jd[qa[k]][1] * Jd[qb[k]][1] + Jd[qa[k]][2] * Jd[qb[k]][2];
+        t->g.Q[k] = (float)t->g64.Q[k];
+    }
     t->L = norb;
     t->pitch = pitch;
     t->nrows = nrows;
@@ -498,6 +502,29 @@ extern "C" int blipgpu_eval_contract(blipgpu_table* t, const double* positions, 
     cudaStream_t s = (cudaStream_t)stream;
     CK(t, cudaMemsetAsync(out, 0, sizeof(float) * 8 * (size_t)M, s));
     return launch_eval(t, positions, M, M, mode, nullptr, nullptr, nullptr, t->pitch, cell, s, d, ldd, out);
+}
+
+extern "C" int blipgpu_eval_f64(blipgpu_table* t, const double* positions, long long M, int mode,
+                                double* val, double* grad, double* lap, long long ld, int* cell, void* stream)
+{
+    if (!t || M < 0) return BLIPGPU_EINVAL;
+    if (mode != BLIPGPU_VALUE && mode != BLIPGPU_VGL) return BLIPGPU_EINVAL;
+    if (ld < t->L || (ld % 4) != 0) return BLIPGPU_EINVAL;
+    if (M == 0) return BLIPGPU_OK;
+    if (!positions || !val || (mode == BLIPGPU_VGL && (!grad || !lap))) return BLIPGPU_EINVAL;
+    if (((uintptr_t)val & 15) || (mode == BLIPGPU_VGL && (((uintptr_t)grad & 15) || ((uintptr_t)lap & 15))))
+        return BLIPGPU_EINVAL;
+    if (M >= (1LL << 31)) return BLIPGPU_EINVAL;
+    cudaStream_t s = (cudaStream_t)stream;
+    const dim3 grid((unsigned)M, (unsigned)((t->g.pitch4 + 31) / 32));
+    if (mode == BLIPGPU_VALUE)
+        blip::eval_f64_kernel<0><<<grid, 128, 0, s>>>(t->g, t->g64, t->table, positions, M, val, grad, lap, ld, cell);
+    else
+        blip::eval_f64_kernel<1><<<grid, 128, 0, s>>>(t->g, t->g64, t->table, positions, M, val, grad, lap, ld, cell);
+    t->launches += 1;
+    t->last_path = 4;
+    CK(t, cudaGetLastError());
+    return BLIPGPU_OK;
 }
 
 extern "C" int blipgpu_reserve(blipgpu_table* t, long long M_max)
