@@ -297,6 +297,21 @@ def run_gpu(args):
     abytes = algorithmic_bytes(M, L, mode_vgl)
     achieved = abytes / (k_ms * 1e-3) / 1e9
     fp32_peak = 148 * 128 * 2 * sm_max * 1e6                          # FMA lanes x 2 flop x clock
+    fp32_meas = blip.blipgpu_probe_fp32(handle, stream) * 1e12        # packed-FMA rate measured in this run
+    # R_compulsory: distinct table rows the batch touches, once, plus the outputs
+    cellbuf = torch.empty((M, 3), dtype=torch.int32, device="cuda")
+    blip.blipgpu_eval(handle, dpos, M, mode, val, grad, lap, ld, cellbuf, stream)
+    torch.cuda.synchronize()
+    n = torch.tensor(list(cfg.grid), device="cuda", dtype=torch.int64)
+    off = torch.arange(-1, 3, device="cuda", dtype=torch.int64)
+    ci = cellbuf.to(torch.int64)
+    k0 = (ci[:, 0:1] + off) % n[0]
+    k1 = (ci[:, 1:2] + off) % n[1]
+    k2 = (ci[:, 2:3] + off) % n[2]
+    rows = ((k0[:, :, None, None] * n[1] + k1[:, None, :, None]) * n[2] + k2[:, None, None, :]).reshape(-1)
+    distinct_rows = int(torch.unique(rows).numel())
+    del rows, k0, k1, k2, ci, cellbuf
+    comp_bytes = distinct_rows * L * 4 + M * L * (20 if mode_vgl else 4)
     roofline = {
         "bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
         "traffic": None,
@@ -306,6 +321,10 @@ def run_gpu(args):
         "algorithmic_bytes": abytes, "bytes_per_eval": abytes / (M * L), "peak_source": peak_src,
         "fp32_fma_frac_of_nominal": 2 * fma_count(M, L, mode_vgl) / (k_ms * 1e-3) / fp32_peak,
         "fp32_peak_tflops_nominal": fp32_peak / 1e12,
+        "fp32_peak_tflops_measured": fp32_meas / 1e12,
+        "fp32_fma_frac_of_measured": 2 * fma_count(M, L, mode_vgl) / (k_ms * 1e-3) / fp32_meas,
+        "distinct_rows": distinct_rows, "compulsory_bytes": comp_bytes,
+        "compulsory_hbm_frac": comp_bytes / (k_ms * 1e-3) / 1e9 / peak,
         "note": "contract roofline of BASELINE.json north_star: every gathered coefficient (64 x 4 B) and every "
                 "output byte per evaluation at the measured HBM copy rate.  The staged kernel reads each table "
                 "row from HBM about 3 times instead of once per electron (see traffic), so achieved exceeds the "

@@ -179,6 +179,12 @@ int blipgpu_info(const blipgpu_table* t, int* grid, int* norb, long long* pitch,
  * in the last bits (all are within the stated tolerances of the fp64 definition). */
 int blipgpu_set_tuning(blipgpu_table* t, int path, int nq);
 
+/* blipgpu_probe_fp32 — measures the device's packed-FP32 FMA rate with a register-only kernel
+ * (3 launches on `stream`, the last one timed; synchronises) and returns it in TFLOP/s in
+ * *tflops (HOST).  For the benchmark's FP32 roofline, measured in the same run at the clocks
+ * the run sees.  Errors: EINVAL, ENOMEM, ECUDA. */
+int blipgpu_probe_fp32(blipgpu_table* t, double* tflops, void* stream);
+
 /* blipgpu_last_path — which gather+FMA kernel the last blipgpu_eval / blipgpu_eval_host of this
  * handle launched: 1 direct (one warp per electron, rows from L2/HBM), 2 staged (table planes
  * through shared memory), 3 split (four warps per electron, small batches), 4 the fp64 kernel of blipgpu_eval_f64; 0 before

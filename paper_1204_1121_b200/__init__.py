@@ -41,6 +41,7 @@ SIGNATURES = {
     "blipgpu_destroy": (ctypes.c_int, [ctypes.c_void_p]),
     "blipgpu_info": (ctypes.c_int, [ctypes.c_void_p, _c_ip, _c_ip, _c_llp, _c_llp]),
     "blipgpu_set_tuning": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_int, ctypes.c_int]),
+    "blipgpu_probe_fp32": (ctypes.c_int, [ctypes.c_void_p, _c_dp, ctypes.c_void_p]),
     "blipgpu_last_path": (ctypes.c_int, [ctypes.c_void_p]),
     "blipgpu_launch_count": (ctypes.c_longlong, [ctypes.c_void_p]),
     "blipgpu_set_profiling": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_int]),
@@ -149,6 +150,13 @@ def blipgpu_destroy(handle):
 def blipgpu_set_tuning(handle, path=0, nq=0):
     """path: 0 auto, 1 direct-gather kernel, 2 staged kernel; nq: direct kernel quads per lane (0 = default)."""
     _check(lib().blipgpu_set_tuning(handle, int(path), int(nq)), "blipgpu_set_tuning", handle)
+
+
+def blipgpu_probe_fp32(handle, stream=None):
+    """Measured packed-FP32 FMA rate of the device, TFLOP/s."""
+    v = ctypes.c_double()
+    _check(lib().blipgpu_probe_fp32(handle, ctypes.byref(v), _stream_ptr(stream)), "blipgpu_probe_fp32", handle)
+    return v.value
 
 
 def blipgpu_last_path(handle):

@@ -1212,4 +1212,29 @@ eval_staged_kernel(const __grid_constant__ CUtensorMap tmap, Geom g, StagedGeom 
     }
 }
 
+// ---------------------------------------------------------------------------------------
+// FP32 peak probe for the benchmark (the FP32 roofline is measured in the same
+// run): every thread runs `iters` rounds of 16 independent packed FMAs on registers.
+// ---------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(512)
+fp32_probe_kernel(float* __restrict__ out, int iters, float seed)
+{
+    u64 acc[16];
+#pragma unroll
+    for (int i = 0; i < 16; ++i) acc[i] = dup2(seed * (float)(i + 1 + threadIdx.x));
+    const u64 x = dup2(0.999f);
+    const float w = 1.0f + seed;
+#pragma unroll 1
+    for (int it = 0; it < iters; ++it) {
+#pragma unroll
+        for (int r = 0; r < 4; ++r)
+#pragma unroll
+            for (int i = 0; i < 16; ++i) acc[i] = fma2(acc[i], dup2(w), x);
+    }
+    float s = 0.f;
+#pragma unroll
+    for (int i = 0; i < 16; ++i) { const float2 v = unpack2(acc[i]); s += v.x + v.y; }
+    out[(size_t)blockIdx.x * blockDim.x + threadIdx.x] = s;
+}
+
 }  // namespace blip

@@ -640,6 +640,34 @@ extern "C" int blipgpu_set_tuning(blipgpu_table* t, int path, int nq)
 }
 
 
+extern "C" int blipgpu_probe_fp32(blipgpu_table* t, double* tflops, void* stream)
+{
+    if (!t || !tflops) return BLIPGPU_EINVAL;
+    cudaStream_t s = (cudaStream_t)stream;
+    const int blocks = t->nsm * 4, threads = 512, iters = 4096;
+    float* out = nullptr;
+    CK(t, cudaMalloc(&out, sizeof(float) * (size_t)blocks * threads));
+    cudaEvent_t e0 = nullptr, e1 = nullptr;
+    int rc = BLIPGPU_OK;
+    float ms = 0.f;
+    cudaError_t e = cudaEventCreate(&e0);
+    if (e == cudaSuccess) e = cudaEventCreate(&e1);
+    for (int rep = 0; rep < 3 && e == cudaSuccess; ++rep) {          // the last of three runs is timed
+        e = cudaEventRecord(e0, s);
+        blip::fp32_probe_kernel<<<blocks, threads, 0, s>>>(out, iters, 1e-9f);
+        if (e == cudaSuccess) e = cudaEventRecord(e1, s);
+        if (e == cudaSuccess) e = cudaEventSynchronize(e1);
+        if (e == cudaSuccess) e = cudaEventElapsedTime(&ms, e0, e1);
+    }
+    if (e != cudaSuccess) { t->last_cuda = (int)e; (void)cudaGetLastError(); rc = BLIPGPU_ECUDA; }
+    else *tflops = 2.0 * 2.0 * 64.0 * (double)iters * (double)blocks * threads / (ms * 1e-3) / 1e12;
+    if (e0) cudaEventDestroy(e0);
+    if (e1) cudaEventDestroy(e1);
+    cudaFree(out);
+    t->launches += 3;
+    return rc;
+}
+
 extern "C" int blipgpu_last_path(const blipgpu_table* t) { return t ? t->last_path : 0; }
 
 extern "C" long long blipgpu_launch_count(const blipgpu_table* t) { return t ? t->launches : 0; }
