@@ -975,7 +975,7 @@ struct StagedCfg {
 // left item k and released all of its planes; while it still works on a unit of item k it
 // only looks whether the descriptor is there yet (to prefetch its first record of item k+1).
 // So whatever a consumer waits for never depends on something that consumer still holds.
-template <int MODE, int VEC, int BY, int BZ, int R, int NW>
+template <int MODE, bool CONTRACT, int VEC, int BY, int BZ, int R, int NW>
 __global__ void __launch_bounds__((NW + 1) * 32, 1)
 eval_staged_kernel(const __grid_constant__ CUtensorMap tmap, Geom g, StagedGeom sg,
                    const float4* __restrict__ recs, const int4* __restrict__ order, int* __restrict__ meta,
@@ -1066,21 +1066,22 @@ eval_staged_kernel(const __grid_constant__ CUtensorMap tmap, Geom g, StagedGeom 
     // short: the record carries the unit's plane number and byte offset inside a plane.
     unsigned released = 0;             // planes < released have been released by this warp
     unsigned waited = 0;               // planes < waited have been waited for by this warp
+    const unsigned full0 = smem_u32(&sm.full[0]), empty0 = smem_u32(&sm.empty[0]);
     auto wait_upto = [&](unsigned need_end) {            // planes < need_end resident
 #pragma unroll 1
         while (waited < need_end) {
             if (released + RU <= waited) {
-                if (lane == 0) mbar_arrive(smem_u32(&sm.empty[released % RU]));
+                if (lane == 0) mbar_arrive(empty0 + 8u * (released % RU));
                 ++released;
             }
-            mbar_wait(smem_u32(&sm.full[waited % RU]), (waited / RU) & 1u);
+            mbar_wait(full0 + 8u * (waited % RU), (waited / RU) & 1u);
             ++waited;
         }
     };
     auto release_upto = [&](unsigned release_end) {      // planes < release_end no longer needed by this warp
 #pragma unroll 1
         while (released < release_end) {
-            if (lane == 0) mbar_arrive(smem_u32(&sm.empty[released % RU]));
+            if (lane == 0) mbar_arrive(empty0 + 8u * (released % RU));
             ++released;
         }
     };
@@ -1092,8 +1093,8 @@ eval_staged_kernel(const __grid_constant__ CUtensorMap tmap, Geom g, StagedGeom 
         release_upto(min(waited, end));
 #pragma unroll 1
         while (waited < end) {
-            mbar_wait(smem_u32(&sm.full[waited % RU]), (waited / RU) & 1u);
-            if (lane == 0) mbar_arrive(smem_u32(&sm.empty[waited % RU]));
+            mbar_wait(full0 + 8u * (waited % RU), (waited / RU) & 1u);
+            if (lane == 0) mbar_arrive(empty0 + 8u * (waited % RU));
             ++waited;
             released = waited;
         }
@@ -1158,12 +1159,26 @@ eval_staged_kernel(const __grid_constant__ CUtensorMap tmap, Geom g, StagedGeom 
         float4 pre = make_float4(0.f, 0.f, 0.f, 0.f);
         if (nsrc && lane < kRecFloats / 4) pre = __ldg(nsrc + lane);
         float4 dv = make_float4(0.f, 0.f, 0.f, 0.f);        // contraction mode: this lane's d values, in flight during the FMAs
-        if (dvec && it_col0 < 4 * g.pitch4) dv = ldg_dvec(dvec, ldd, loc.w, it_col0);
-        PairAcc acc[NP];
-        if (!ok) {
+        if (CONTRACT && it_col0 < 4 * g.pitch4) dv = ldg_dvec(dvec, ldd, loc.w, it_col0);
+        // a-5: store the unit's results, or contract them with d (blipgpu_eval_contract)
+        auto emit = [&](const PairAcc (&a)[NP]) {
+            if (CONTRACT) {
+                float sum[5] = {0.f, 0.f, 0.f, 0.f, 0.f};
+                if (it_col0 < 4 * g.pitch4) {
+                    float dq[4];
+                    mask_dvec(dv, it_col0, g.L, dq);
+                    contract_pairs<MODE, NP>(g, a, dq, sum);
+                }
+                contract_flush<MODE>(g, sum, loc.w, cout, lane);
+            } else if (it_col0 < 4 * g.pitch4) store_pairs<MODE, NP>(g, a, loc.w, it_col0, val, grad, lap, ld);
+        };
+        if (!ok) {                                           // non-finite position (rare): NaN out, no plane touched
+            PairAcc nanacc[NP];
 #pragma unroll
-            for (int p = 0; p < NP; ++p) set_nan(acc[p]);
+            for (int p = 0; p < NP; ++p) set_nan(nanacc[p]);
+            emit(nanacc);
         } else {
+            PairAcc acc[NP];
 #pragma unroll
             for (int p = 0; p < NP; ++p) acc[p].val = acc[p].t1 = acc[p].t2 = acc[p].t3 = acc[p].lp = 0ull;
             float wz[3][4];
@@ -1193,16 +1208,8 @@ eval_staged_kernel(const __grid_constant__ CUtensorMap tmap, Geom g, StagedGeom 
                     }
                 }
             }
+            emit(acc);
         }
-        if (dvec) {
-            float sum[5] = {0.f, 0.f, 0.f, 0.f, 0.f};
-            if (it_col0 < 4 * g.pitch4) {
-                float dq[4];
-                mask_dvec(dv, it_col0, g.L, dq);
-                contract_pairs<MODE, NP>(g, acc, dq, sum);
-            }
-            contract_flush<MODE>(g, sum, loc.w, cout, lane);
-        } else if (it_col0 < 4 * g.pitch4) store_pairs<MODE, NP>(g, acc, loc.w, it_col0, val, grad, lap, ld);
 
         have = nsrc != nullptr;
         __syncwarp();                                        // every lane is done with this unit's record

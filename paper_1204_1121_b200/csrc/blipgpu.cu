@@ -50,31 +50,36 @@ struct StagedVariant {
 template <int BY, int BZ, int R, int NW>
 struct SV {
     using Cfg = blip::StagedCfg<kSVec, BY, BZ, R, NW>;
+    template <int MODE, bool CONTRACT>
+    static cudaError_t prep1()
+    {
+        return cudaFuncSetAttribute(blip::eval_staged_kernel<MODE, CONTRACT, kSVec, BY, BZ, R, NW>,
+                                    cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(typename Cfg::Smem));
+    }
     static cudaError_t prepare()
     {
-        const int smem = (int)sizeof(typename Cfg::Smem);
-        cudaError_t e = cudaFuncSetAttribute(blip::eval_staged_kernel<0, kSVec, BY, BZ, R, NW>,
-                                             cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
-        if (e == cudaSuccess)
-            e = cudaFuncSetAttribute(blip::eval_staged_kernel<1, kSVec, BY, BZ, R, NW>,
-                                     cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
-        if (e == cudaSuccess)
-            e = cudaFuncSetAttribute(blip::eval_staged_kernel<2, kSVec, BY, BZ, R, NW>,
-                                     cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+        cudaError_t e = prep1<0, false>();
+        if (e == cudaSuccess) e = prep1<1, false>();
+        if (e == cudaSuccess) e = prep1<2, false>();
+        if (e == cudaSuccess) e = prep1<0, true>();
+        if (e == cudaSuccess) e = prep1<1, true>();
+        if (e == cudaSuccess) e = prep1<2, true>();
         return e;
+    }
+    template <int MODE, bool CONTRACT>
+    static void launch1(unsigned nctas, cudaStream_t s, const StagedArgs& a)
+    {
+        launch_pdl(blip::eval_staged_kernel<MODE, CONTRACT, kSVec, BY, BZ, R, NW>, nctas, Cfg::THREADS,
+                   sizeof(typename Cfg::Smem), s, *a.tmap, *a.g, *a.sg, a.recs, a.order, a.meta, a.nchunk, a.val, a.grad,
+                   a.lap, a.ld, a.dvec, a.ldd, a.cout);
     }
     static void launch(int mode, unsigned nctas, cudaStream_t s, const StagedArgs& a)
     {
-        const size_t smem = sizeof(typename Cfg::Smem);
-        if (mode == 0)
-            launch_pdl(blip::eval_staged_kernel<0, kSVec, BY, BZ, R, NW>, nctas, Cfg::THREADS, smem, s,
-                       *a.tmap, *a.g, *a.sg, a.recs, a.order, a.meta, a.nchunk, a.val, a.grad, a.lap, a.ld, a.dvec, a.ldd, a.cout);
-        else if (mode == 2)
-            launch_pdl(blip::eval_staged_kernel<2, kSVec, BY, BZ, R, NW>, nctas, Cfg::THREADS, smem, s,
-                       *a.tmap, *a.g, *a.sg, a.recs, a.order, a.meta, a.nchunk, a.val, a.grad, a.lap, a.ld, a.dvec, a.ldd, a.cout);
-        else
-            launch_pdl(blip::eval_staged_kernel<1, kSVec, BY, BZ, R, NW>, nctas, Cfg::THREADS, smem, s,
-                       *a.tmap, *a.g, *a.sg, a.recs, a.order, a.meta, a.nchunk, a.val, a.grad, a.lap, a.ld, a.dvec, a.ldd, a.cout);
+        if (a.dvec) {
+            if (mode == 0) launch1<0, true>(nctas, s, a); else if (mode == 2) launch1<2, true>(nctas, s, a); else launch1<1, true>(nctas, s, a);
+        } else {
+            if (mode == 0) launch1<0, false>(nctas, s, a); else if (mode == 2) launch1<2, false>(nctas, s, a); else launch1<1, false>(nctas, s, a);
+        }
     }
     static constexpr StagedVariant variant() { return {BY, BZ, R, NW, sizeof(typename Cfg::Smem), &prepare, &launch}; }
 };
