@@ -1067,15 +1067,11 @@ eval_staged_kernel(const __grid_constant__ CUtensorMap tmap, Geom g, StagedGeom 
     unsigned released = 0;             // planes < released have been released by this warp
     unsigned waited = 0;               // planes < waited have been waited for by this warp
     const unsigned full0 = smem_u32(&sm.full[0]), empty0 = smem_u32(&sm.empty[0]);
-    auto wait_upto = [&](unsigned need_end) {            // planes < need_end resident
-#pragma unroll 1
-        while (waited < need_end) {
-            if (released + RU <= waited) {
-                if (lane == 0) mbar_arrive(empty0 + 8u * (released % RU));
-                ++released;
-            }
-            mbar_wait(full0 + 8u * (waited % RU), (waited / RU) & 1u);
-            ++waited;
+    // plane q of the current unit (q - released < R, so nothing is due for release first)
+    auto wait_plane = [&](unsigned q) {
+        if (waited <= q) {
+            mbar_wait(full0 + 8u * (q % RU), (q / RU) & 1u);
+            waited = q + 1;
         }
     };
     auto release_upto = [&](unsigned release_end) {      // planes < release_end no longer needed by this warp
@@ -1141,7 +1137,7 @@ eval_staged_kernel(const __grid_constant__ CUtensorMap tmap, Geom g, StagedGeom 
         // planes i1, i1+1 resident, earlier ones released; planes i1+2 and i1+3 are waited for
         // just before their quarter of the loop, which leaves the producer two more slots of the
         // ring to run ahead of the consumers
-        if (ok) { pass_upto(sq); wait_upto(sq + 2); }
+        if (ok) { pass_upto(sq); wait_plane(sq); wait_plane(sq + 1); }
 
         // record of this warp's next unit, in flight during the FMAs
         const float4* nsrc = nullptr;
@@ -1189,7 +1185,8 @@ eval_staged_kernel(const __grid_constant__ CUtensorMap tmap, Geom g, StagedGeom 
             const unsigned off = (unsigned)loc.y + lane_off;
 #pragma unroll
             for (int m1 = 0; m1 < 4; ++m1) {
-                if (m1 >= 2) wait_upto(sq + m1 + 1);
+                // planes i1+2, i1+3 just before their quarter of the loop
+                if (m1 >= 2) wait_plane(sq + m1);
                 const unsigned pp = plane0 + ((sq + m1) % RU) * (unsigned)Cfg::PLANE_BYTES + off;
 #pragma unroll
                 for (int m2 = 0; m2 < 4; ++m2) {
