@@ -89,7 +89,7 @@ const StagedVariant kVariants[] = {
     SV<4, 4, 8, 8>::variant(),  SV<4, 4, 8, 12>::variant(), SV<4, 4, 8, 16>::variant(),
 };
 constexpr int kNumVariants = (int)(sizeof(kVariants) / sizeof(kVariants[0]));
-constexpr int kDefaultVariant = 3;
+constexpr int kDefaultVariant = 4;
 
 int env_int(const char* name, int dflt)
 {
