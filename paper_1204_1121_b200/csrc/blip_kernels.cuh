@@ -886,6 +886,15 @@ __device__ __forceinline__ void mbar_arrive(unsigned bar)
 {
     asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" :: "r"(bar) : "memory");
 }
+// arrival by lane 0 only, predicated inside the instruction (no branch, no reconvergence point)
+__device__ __forceinline__ void mbar_arrive_lane0(unsigned bar, int lane)
+{
+    asm volatile(
+        "{\n\t.reg .pred p;\n\t"
+        "setp.eq.s32 p, %1, 0;\n\t"
+        "@p mbarrier.arrive.shared::cta.b64 _, [%0];\n\t}"
+        :: "r"(bar), "r"(lane) : "memory");
+}
 __device__ __forceinline__ bool mbar_test(unsigned bar, unsigned parity)
 {
     unsigned done;
@@ -1077,7 +1086,7 @@ eval_staged_kernel(const __grid_constant__ CUtensorMap tmap, Geom g, StagedGeom 
     auto release_upto = [&](unsigned release_end) {      // planes < release_end no longer needed by this warp
 #pragma unroll 1
         while (released < release_end) {
-            if (lane == 0) mbar_arrive(empty0 + 8u * (released % RU));
+            mbar_arrive_lane0(empty0 + 8u * (released % RU), lane);
             ++released;
         }
     };
@@ -1087,11 +1096,14 @@ eval_staged_kernel(const __grid_constant__ CUtensorMap tmap, Geom g, StagedGeom 
     // already stand waiting for it, i.e. put the full copy latency on every plane passed.
     auto pass_upto = [&](unsigned end) {
         release_upto(min(waited, end));
+        if (waited < end) {
 #pragma unroll 1
-        while (waited < end) {
-            mbar_wait(full0 + 8u * (waited % RU), (waited / RU) & 1u);
-            if (lane == 0) mbar_arrive(empty0 + 8u * (waited % RU));
-            ++waited;
+            do {
+                const unsigned sl = 8u * (waited % RU);
+                mbar_wait(full0 + sl, (waited / RU) & 1u);
+                mbar_arrive_lane0(empty0 + sl, lane);
+                ++waited;
+            } while (waited < end);
             released = waited;
         }
     };
