@@ -59,6 +59,23 @@ def fma_count(M, L, mode_vgl):
     return M * L * (304 if mode_vgl else 80)
 
 
+def max_over_ranks(dist, x, device):
+    """Timing rule of the contract: a multi-rank number is the MAX over ranks.  `dist` is
+    torch.distributed (None for a single process); works with nccl (GPU) and gloo (CPU tests)."""
+    if dist is None:
+        return float(x)
+    import torch
+    t = torch.tensor([float(x)], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def whole_job_value(positions_per_rank, norb, world, ms_per_step):
+    """Weak scaling: every rank evaluates its own walkers on its replica of the table, so the job's
+    evaluations per step are world x (positions per rank) x orbitals, over the slowest rank's time."""
+    return positions_per_rank * norb * world / (ms_per_step * 1e-3)
+
+
 class ClockSampler:
     """Samples SM clock and throttle reasons during the timed region (NVML in a thread)."""
 
@@ -275,13 +292,10 @@ def run_gpu(args):
             ms_total = sum(a.elapsed_time(b) for a, b in pairs)
             del scratch
     launches = blip.blipgpu_launch_count(handle) - n0
-    if dist is not None:
-        tmax = torch.tensor([ms_total], dtype=torch.float64, device="cuda")
-        dist.all_reduce(tmax, op=dist.ReduceOp.MAX)
-        ms_total = float(tmax.item())
+    ms_total = max_over_ranks(dist, ms_total, "cuda")
     ms_step = ms_total / args.steps
     evals_step = M * L * world
-    value = evals_step / (ms_step * 1e-3)
+    value = whole_job_value(M, L, world, ms_step)
 
     # ---- dominant kernel (gather + FMA) timed by the library's own events on the same stream
     blip.blipgpu_set_profiling(handle, 1)
@@ -358,10 +372,7 @@ def run_gpu(args):
             blip.blipgpu_eval_host(handle, ppos, M, mode, pval, pgrad, plap, ld, None, stream)
         barrier()
         dt = time.perf_counter() - t0
-        if dist is not None:
-            tm = torch.tensor([dt], dtype=torch.float64, device="cuda")
-            dist.all_reduce(tm, op=dist.ReduceOp.MAX)
-            dt = float(tm.item())
+        dt = max_over_ranks(dist, dt, "cuda")
         e2e = {"value": evals_step * e2e_steps / dt, "unit": UNIT, "h2d_bytes_per_step": int(ppos.numel() * 8),
                "d2h_bytes_per_step": int(M * ld * 4 * (5 if mode_vgl else 1)), "steps": e2e_steps,
                "ms_per_step": 1e3 * dt / e2e_steps, "api": "blipgpu_eval_host (pinned host buffers)",
