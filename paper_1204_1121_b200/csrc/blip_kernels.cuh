@@ -42,6 +42,7 @@ struct Geom {
     float Q[6];         // (J J^T): Q00 Q11 Q22 Q01 Q02 Q12
     int L;              // orbitals
     int pitch4;         // table row pitch in float4 (= ceil(L/4))
+    int diag;           // J diagonal (lattice vectors along the Cartesian axes): the kernels' MODE 2
 };
 
 // Geometry of the staged path: pencils of BY x BZ cells running along axis 1, cut into
@@ -371,8 +372,10 @@ __device__ __forceinline__ void column_weights(const Geom& g, const AX& ax, int 
     float la = __fmul_rn(g.Q[0], __fmul_rn(c0, a1));
     la = __fmaf_rn(g.Q[1], __fmul_rn(a0, c1), la);
     la = __fmaf_rn(__fmul_rn(2.0f, g.Q[3]), __fmul_rn(b0, b1), la);
-    cw = make_float4(p00, p10, p01, la);
     lb = __fmul_rn(2.0f, __fmaf_rn(g.Q[4], p10, __fmul_rn(g.Q[5], p01)));
+    // diagonal J (MODE 2, where Lb = 0): the gradient weights carry J, so that the accumulators
+    // are the Cartesian components and the epilogue has nothing left to multiply
+    cw = g.diag ? make_float4(p00, __fmul_rn(g.J[0], p10), __fmul_rn(g.J[4], p01), la) : make_float4(p00, p10, p01, la);
 }
 
 // Warp-cooperative a-1 + a-2 for electron `e` into `rec` (shared memory).  `ax` is per-warp
@@ -398,7 +401,8 @@ __device__ __forceinline__ void warp_prepare(const Geom& g, const double* __rest
         rec.cw[lane] = cw; rec.lb[lane] = lb;
     } else if (lane < 28) {
         const int k = (lane - 16) >> 2, m = lane & 3;
-        rec.wz[k][m] = (k == 2) ? __fmul_rn(g.Q[2], ax[2][2][m]) : ax[2][k][m];
+        rec.wz[k][m] = (k == 2) ? __fmul_rn(g.Q[2], ax[2][2][m])
+                     : (k == 1 && g.diag) ? __fmul_rn(g.J[8], ax[2][1][m]) : ax[2][k][m];
     }
     __syncwarp();
 }
@@ -437,7 +441,10 @@ scatter_prep_kernel(Geom g, StagedGeom sg, int tile_floats, const double* __rest
 #pragma unroll
     for (int k = 0; k < 4; ++k) out[16 + k] = make_float4(lb[4 * k], lb[4 * k + 1], lb[4 * k + 2], lb[4 * k + 3]);
     out[20] = make_float4(ax[2][0][0], ax[2][0][1], ax[2][0][2], ax[2][0][3]);
-    out[21] = make_float4(ax[2][1][0], ax[2][1][1], ax[2][1][2], ax[2][1][3]);
+    const float jz = g.diag ? g.J[8] : 1.0f;                 // see column_weights
+    out[21] = g.diag ? make_float4(__fmul_rn(jz, ax[2][1][0]), __fmul_rn(jz, ax[2][1][1]), __fmul_rn(jz, ax[2][1][2]),
+                                   __fmul_rn(jz, ax[2][1][3]))
+                     : make_float4(ax[2][1][0], ax[2][1][1], ax[2][1][2], ax[2][1][3]);
     out[22] = make_float4(__fmul_rn(g.Q[2], ax[2][2][0]), __fmul_rn(g.Q[2], ax[2][2][1]),
                           __fmul_rn(g.Q[2], ax[2][2][2]), __fmul_rn(g.Q[2], ax[2][2][3]));
     // StagedRec::loc: plane within the pencil segment, byte offset of row (i2, i3) in a plane of
@@ -534,10 +541,10 @@ __device__ __forceinline__ void store_pairs(const Geom& g, const PairAcc (&acc)[
             const float ta[2] = {a.x, a.y}, tb[2] = {b.x, b.y}, tc[2] = {c.x, c.y};
 #pragma unroll
             for (int h = 0; h < 2; ++h) {
-                if (MODE == 2) {
-                    gx[2 * p + h] = __fmul_rn(g.J[0], ta[h]);
-                    gy[2 * p + h] = __fmul_rn(g.J[4], tb[h]);
-                    gz[2 * p + h] = __fmul_rn(g.J[8], tc[h]);
+                if (MODE == 2) {                             // J is already in the weights
+                    gx[2 * p + h] = ta[h];
+                    gy[2 * p + h] = tb[h];
+                    gz[2 * p + h] = tc[h];
                 } else {
                     gx[2 * p + h] = __fmaf_rn(g.J[0], ta[h], __fmaf_rn(g.J[3], tb[h], __fmul_rn(g.J[6], tc[h])));
                     gy[2 * p + h] = __fmaf_rn(g.J[1], ta[h], __fmaf_rn(g.J[4], tb[h], __fmul_rn(g.J[7], tc[h])));
@@ -608,9 +615,13 @@ __device__ __forceinline__ void contract_flush(const Geom& g, float (&sum)[5], i
     }
     float v[8];
     v[0] = sum[0];
-    v[1] = __fmaf_rn(g.J[0], sum[1], __fmaf_rn(g.J[3], sum[2], __fmul_rn(g.J[6], sum[3])));
-    v[2] = __fmaf_rn(g.J[1], sum[1], __fmaf_rn(g.J[4], sum[2], __fmul_rn(g.J[7], sum[3])));
-    v[3] = __fmaf_rn(g.J[2], sum[1], __fmaf_rn(g.J[5], sum[2], __fmul_rn(g.J[8], sum[3])));
+    if (MODE == 2) {                                         // J is already in the weights
+        v[1] = sum[1]; v[2] = sum[2]; v[3] = sum[3];
+    } else {
+        v[1] = __fmaf_rn(g.J[0], sum[1], __fmaf_rn(g.J[3], sum[2], __fmul_rn(g.J[6], sum[3])));
+        v[2] = __fmaf_rn(g.J[1], sum[1], __fmaf_rn(g.J[4], sum[2], __fmul_rn(g.J[7], sum[3])));
+        v[3] = __fmaf_rn(g.J[2], sum[1], __fmaf_rn(g.J[5], sum[2], __fmul_rn(g.J[8], sum[3])));
+    }
     v[4] = sum[4]; v[5] = v[6] = v[7] = 0.f;
     const bool h16 = lane & 16, h8 = lane & 8, h4 = lane & 4;
     float w[4], x[2];

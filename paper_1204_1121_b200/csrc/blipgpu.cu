@@ -270,6 +270,7 @@ extern "C" int blipgpu_create(const double* lattice, const int* grid, int norb,
     for (int a = 0; a < 3; ++a)
         for (int i = 0; i < 3; ++i)
             if (a != i && Jd[a][i] != 0.0) t->diag = 0;
+    t->g.diag = t->diag;
     const int qa[6] = {0, 1, 2, 0, 0, 1}, qb[6] = {0, 1, 2, 1, 2, 2};
     for (int k = 0; k < 6; ++k) {
         t->g64.Q[k] = Jd[qa[k]][0] * Jd[qb[k]][0] + Jd[qa[k]][1] * Jd[qb[k]][1] + Jd[qa[k]][2] * Jd[qb[k]][2];
