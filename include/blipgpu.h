@@ -22,8 +22,11 @@
  * innermost ("l ... sequential memory access").
  *
  * Every pointer argument says HOST or DEVICE.  Nothing throws; every call returns a code.
- * There is no CPU fallback: without a CUDA device of compute capability 10.x the library
- * fails with BLIPGPU_EARCH / BLIPGPU_ECUDA.
+ * There is no CPU fallback: without a CUDA device of compute capability 10.0 (B200; the
+ * library holds sm_100a code only) it fails with BLIPGPU_EARCH / BLIPGPU_ECUDA.
+ *
+ * This header is the whole boundary.  Test and benchmark instrumentation
+ * (forcing a kernel, launch counts, kernel timers, the FP32 probe) is in blipgpu_dev.h.
  */
 #ifndef BLIPGPU_H
 #define BLIPGPU_H
@@ -43,7 +46,7 @@ typedef struct blipgpu_table blipgpu_table;       /* opaque handle: table + work
 #define BLIPGPU_EINVAL  (-1)                      /* bad argument (see each call)          */
 #define BLIPGPU_ENOMEM  (-2)                      /* host or device allocation failed      */
 #define BLIPGPU_ECUDA   (-3)                      /* CUDA runtime error: blipgpu_last_cuda_error */
-#define BLIPGPU_EARCH   (-4)                      /* current device is not sm_100 class    */
+#define BLIPGPU_EARCH   (-4)                      /* current device is not compute capability 10.0 */
 
 /*
  * blipgpu_create — load a coefficient table onto the current CUDA device.
@@ -89,6 +92,9 @@ int blipgpu_create(const double* lattice, const int* grid, int norb, const float
  * detecting it would need a synchronisation).  Output pointers must be 16-byte aligned.
  * One handle serves one stream at a time (it owns the grouping workspace); if the
  * workspace must grow the call synchronises `stream` once — blipgpu_reserve avoids that.
+ * The call keeps no state on the host between calls and leaves its device workspace as it
+ * found it, so once the workspace is reserved it may be captured in a CUDA graph and
+ * replayed.
  * Errors: EINVAL (NULL required pointer, M < 0, unknown mode, bad ld, misaligned output),
  * ENOMEM, ECUDA.
  */
@@ -98,10 +104,10 @@ int blipgpu_eval(blipgpu_table* t, const double* positions, long long M, int mod
 /*
  * blipgpu_eval_host — the same evaluation with HOST buffers: the paper's per-step data flow
  * (trial positions host->device, orbital values device->host; Fig. 4,
- * 336-343 Table XI).  Copies positions in, evaluates batch by batch and copies results out,
- * overlapping the device->host copies of one batch with the evaluation of the next; returns
- * after everything has landed (synchronises `stream`).  Pinned host buffers make the copies
- * asynchronous; pageable ones work but serialise.
+ * 336-343 Table XI).  Copies positions in, evaluates the whole batch with the kernels
+ * blipgpu_eval would use (same bits) and copies the results out; returns after everything has
+ * landed (synchronises `stream`).  The device->host copy dominates (20 B per evaluation over
+ * PCIe); pinned host buffers run it at the link rate, pageable ones work but are slower.
  *
  *   positions HOST [M][3] fp64;  val/grad/lap HOST, shapes and `ld` as in blipgpu_eval
  *   (no alignment requirement);  cell HOST [M][3] int32, optional.
@@ -155,8 +161,10 @@ int blipgpu_eval_contract(blipgpu_table* t, const double* positions, long long M
 int blipgpu_eval_f64(blipgpu_table* t, const double* positions, long long M, int mode,
                      double* val, double* grad, double* lap, long long ld, int* cell, void* stream);
 
-/* blipgpu_reserve — pre-size the grouping workspace for batches of up to M_max positions
- * (and the staging buffers of blipgpu_eval_host).  Optional.  Errors: EINVAL, ENOMEM, ECUDA. */
+/* blipgpu_reserve — pre-size the grouping workspace (bins, permutation, per-electron records)
+ * for batches of up to M_max positions, so that blipgpu_eval never has to grow it (growing
+ * synchronises the stream once).  Optional.  The device staging buffers of blipgpu_eval_host
+ * are sized by that call itself.  Errors: EINVAL, ENOMEM, ECUDA. */
 int blipgpu_reserve(blipgpu_table* t, long long M_max);
 
 /* blipgpu_destroy — free the table and workspace.  destroy(NULL) is a no-op returning OK. */
@@ -166,44 +174,6 @@ int blipgpu_destroy(blipgpu_table* t);
  * Any out pointer may be NULL. */
 int blipgpu_info(const blipgpu_table* t, int* grid, int* norb, long long* pitch,
                  long long* table_bytes);
-
-/* blipgpu_set_tuning — expert knob; the defaults are chosen from the table and batch shape.
- *   path  0: automatic (staged for dense batches; else the split kernel up to 16,384 positions
- *            or the direct kernel, after grouping by cell brick when the table exceeds L2);
- *         1: always the direct-gather kernel (grouped above 2,048 positions);
- *         2: always the shared-memory staged kernel (EINVAL if this table cannot use it: fewer
- *            than 128 orbitals, a grid smaller than one staging box, or no TMA descriptor)
- *   nq    direct kernel: quads of 4 orbitals per lane, 1..3; 0 restores the default.
- * The direct and the staged kernel run the same arithmetic sequence and return the same bits;
- * the split kernel adds the four plane partial sums last, so its results differ from theirs
- * in the last bits (all are within the stated tolerances of the fp64 definition). */
-int blipgpu_set_tuning(blipgpu_table* t, int path, int nq);
-
-/* blipgpu_probe_fp32 — measures the device's packed-FP32 FMA rate with a register-only kernel
- * (3 launches on `stream`, the last one timed; synchronises) and returns it in TFLOP/s in
- * *tflops (HOST).  For the benchmark's FP32 roofline, measured in the same run at the clocks
- * the run sees.  Errors: EINVAL, ENOMEM, ECUDA. */
-int blipgpu_probe_fp32(blipgpu_table* t, double* tflops, void* stream);
-
-/* blipgpu_last_path — which gather+FMA kernel the last blipgpu_eval / blipgpu_eval_host of this
- * handle launched: 1 direct (one warp per electron, rows from L2/HBM), 2 staged (table planes
- * through shared memory), 3 split (four warps per electron, small batches), 4 the fp64 kernel of blipgpu_eval_f64; 0 before
- * any call. */
-int blipgpu_last_path(const blipgpu_table* t);
-
-/* blipgpu_launch_count — number of kernels this handle has launched since creation (the
- * benchmark's "gpu_launches" evidence).  */
-long long blipgpu_launch_count(const blipgpu_table* t);
-
-/* blipgpu_set_profiling — on != 0: every following blipgpu_eval also records CUDA events on
- * its stream at the start of the call, before and after the gather+FMA kernel (no
- * synchronisation is added).  Off by default. */
-int blipgpu_set_profiling(blipgpu_table* t, int on);
-
-/* blipgpu_last_kernel_ms — waits for the last profiled blipgpu_eval and returns the device
- * time (ms) of its grouping kernels (step a-4) and of its gather+FMA kernel (steps a-1..a-3,
- * a-5).  HOST out pointers, either may be NULL.  EINVAL if profiling is off or nothing ran. */
-int blipgpu_last_kernel_ms(blipgpu_table* t, float* group_ms, float* eval_ms);
 
 /* blipgpu_strerror — static string for a return code. */
 const char* blipgpu_strerror(int code);

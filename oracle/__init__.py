@@ -135,3 +135,23 @@ def contract(val, grad, lap, d):
                 s[4] += lap[j, l] * w
         out[j] = s
     return out
+
+
+def contract_rows(val, grad, lap, d):
+    """The same contraction as `contract`, one position at a time with numpy's fp64 dot product as
+    the library primitive for the sum over l (Eq. 11: sum_l psi_l(r'_j) (D^-1)_lj).
+    For full-size comparisons, where the pure-Python double loop of `contract` would take minutes.
+    Pin (tests/test_oracle_pins.py): equal to `contract` on a seeded case to fp64 rounding, and the
+    one-hot / constant-table pins of `contract`."""
+    val = np.asarray(val, dtype=np.float64)
+    d = np.asarray(d, dtype=np.float64)
+    M = val.shape[0]
+    out = np.zeros((M, 5), dtype=np.float64)
+    for j in range(M):
+        out[j, 0] = np.dot(val[j], d[j])
+        if grad is not None:
+            out[j, 1] = np.dot(grad[j, 0], d[j])
+            out[j, 2] = np.dot(grad[j, 1], d[j])
+            out[j, 3] = np.dot(grad[j, 2], d[j])
+            out[j, 4] = np.dot(lap[j], d[j])
+    return out

@@ -7,8 +7,9 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 ROOT = os.path.dirname(HERE)
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libblipgpu.so")
-SOURCES = [os.path.join(CSRC, "blipgpu.cu")]
-DEPS = SOURCES + [os.path.join(CSRC, "blip_kernels.cuh"), os.path.join(CSRC, "blip_f64.cuh"), os.path.join(ROOT, "include", "blipgpu.h")]
+SOURCES = [os.path.join(CSRC, "blipgpu.cu"), os.path.join(CSRC, "blipgpu_dev.cu")]
+DEPS = SOURCES + [os.path.join(CSRC, f) for f in sorted(os.listdir(CSRC)) if f.endswith((".cuh", ".h"))] + [
+    os.path.join(ROOT, "include", "blipgpu.h"), os.path.join(ROOT, "include", "blipgpu_dev.h")]
 
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",

@@ -12,11 +12,6 @@
 
 namespace blip {
 
-struct Geom64 {
-    double J[9];        // J[a][i] = n_a G[i][a]
-    double Q[6];        // J J^T: Q00 Q11 Q22 Q01 Q02 Q12
-};
-
 // cell map of one axis with the fraction kept in fp64 (same pinned sequence as cell_map_axis)
 __device__ __forceinline__ bool cell_map_axis_d(const Geom& g, int a, double x, double y, double z,
                                                 int& i, double& f)

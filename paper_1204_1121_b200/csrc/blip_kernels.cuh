@@ -22,40 +22,9 @@
 // written in the symmetric B(x) form and the sum is contracted z axis first, the oracle uses
 // the expanded per-site pieces and keeps all 10 grid-space accumulators.
 #pragma once
-#include <cuda.h>
-#include <cuda_runtime.h>
-#include <stdint.h>
+#include "blip_types.h"
 
 namespace blip {
-
-constexpr int kWarpsPerBlock = 8;          // direct kernel: 8 electrons per CTA
-constexpr int kBrick = 4;                  // direct path grouping: bricks of 4x4x4 cells
-constexpr int kScanThreads = 1024;
-constexpr int kRecFloats = 96;             // per-electron record (ElecRec), 384 bytes
-
-struct Geom {
-    double G[9];        // inverse lattice, u = r.G (row vector), fp64 for the index map
-    int n[3];           // grid points per axis
-    int np[3];          // padded table extent per axis, n + 3
-    int nb[3];          // direct path: bricks per axis
-    float J[9];         // J[a][i] = n_a G[i][a] = d t_a / d r_i
-    float Q[6];         // (J J^T): Q00 Q11 Q22 Q01 Q02 Q12
-    int L;              // orbitals
-    int pitch4;         // table row pitch in float4 (= ceil(L/4))
-    int diag;           // J diagonal (lattice vectors along the Cartesian axes): the kernels' MODE 2
-};
-
-// Geometry of the staged path: pencils of BY x BZ cells running along axis 1, cut into
-// segments of `seg` cell planes.  Sort key of an electron = (pencil, i1).
-struct StagedGeom {
-    int by, bz;         // cross-section of a pencil in cells (template constants of the kernel)
-    int nby, nbz;       // pencils per axis
-    int seg;            // cell planes per segment
-    int nseg;           // segments per pencil = ceil(n1 / seg)
-    int nps;            // pencil segments = nby * nbz * nseg (the work items, per orbital chunk)
-    int chunk_major;    // order of the work items (see eval_staged_kernel)
-};
-constexpr int kMaxSortedItems = 8192;      // pencil segments the scan kernel can order by load
 
 // ---------------------------------------------------------------------------------------
 // a-1: cell map.  The IEEE sequence is pinned so that the integer
@@ -120,19 +89,21 @@ bin_kernel(Geom g, StagedGeom sg, int staged, const double* __restrict__ pos, lo
     atomicAdd(&hist[b], 1u);
 }
 
-// a-4 (2/3): exclusive scan of the histogram, in place, one CTA; it also clears `hist_next`,
-// the histogram of the next call (the two alternate, so no separate memset is needed).  For
-// the staged path it orders the work items (pencil segments) by decreasing electron count —
-// the persistent staged kernel takes items from a shared counter, so heavy items first keeps
-// the tail short (longest-processing-time-first) — and resets that counter.
+// a-4 (2/3): exclusive scan of the histogram into `offs`, one CTA.  `hist` is all zero on entry
+// to every call (blipgpu_create clears it once) and this kernel, its only reader, puts it back
+// to zero as it reads it: a call leaves no state behind for the next one, so a call captured
+// in a CUDA graph can be replayed any number of times.  For the staged path it also orders
+// the work items (pencil segments) by decreasing electron count — the persistent staged kernel
+// takes items from a shared counter, so heavy items first keeps the tail short
+// (longest-processing-time-first) — and resets that counter.
+//   offs[b]           start of bin b in the sorted order (the scatter kernels advance it)
 //   order[0 .. nps)   {pencil segment id, first unit, units, 0}; units are indices into the
-//                     sorted records.  sg.chunk_major: x-slab by x-slab, heaviest first inside a
-//                     slab; else heaviest first overall; in id order if nps > kMaxSortedItems
+//                     sorted records; heaviest first, in id order if nps > kMaxSortedItems
 //   meta[0]           number of leading entries of `order` that hold electrons
 //   meta[1]           work counter of the staged kernel, reset to 0
 constexpr int kScanChunk = 8 * kScanThreads;                 // bins scanned per pass through shared memory
 __global__ void __launch_bounds__(kScanThreads)
-scan_kernel(unsigned* __restrict__ hist, unsigned* __restrict__ hist_next, int nbins, int nclear, long long M, int staged,
+scan_kernel(unsigned* __restrict__ hist, unsigned* __restrict__ offs, int nbins, long long M, int staged,
             Geom g, StagedGeom sg, int4* __restrict__ order, int* __restrict__ meta)
 {
     __shared__ unsigned buf[kScanChunk];                     // one chunk of the histogram; later the sort keys
@@ -142,14 +113,15 @@ scan_kernel(unsigned* __restrict__ hist, unsigned* __restrict__ hist_next, int n
     const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
     wait_for_predecessor();
     if (tid == 0) { carry_s = 0; nonempty = 0; }
-    for (int b = tid; b < nclear; b += kScanThreads) hist_next[b] = 0u;
     __syncthreads();
     for (int base = 0; base < nbins; base += kScanChunk) {
         const int n = min(kScanChunk, nbins - base);
 #pragma unroll
         for (int k = 0; k < 8; ++k) {                        // coalesced, 8 independent loads per thread
             const int i = tid + k * kScanThreads;
-            buf[i] = (i < n) ? hist[base + i] : 0u;
+            unsigned v = 0u;
+            if (i < n) { v = hist[base + i]; hist[base + i] = 0u; }
+            buf[i] = v;
         }
         __syncthreads();
         unsigned v[8], s = 0;
@@ -181,20 +153,20 @@ scan_kernel(unsigned* __restrict__ hist, unsigned* __restrict__ hist_next, int n
 #pragma unroll
         for (int k = 0; k < 8; ++k) {
             const int i = tid + k * kScanThreads;
-            if (i < n) hist[base + i] = buf[i];
+            if (i < n) offs[base + i] = buf[i];
         }
         __syncthreads();
     }
     if (!staged) return;
-    // hist[b] = start of bin b (written above by this block, visible after the barrier)
+    // offs[b] = start of bin b (written above by this block, visible after the barrier)
     if (tid == 0) meta[1] = 0;
     const int nps = sg.nps;
     auto units_of = [&](int i, unsigned& u0, unsigned& u1) {
         const int pencil = i / sg.nseg, segi = i - pencil * sg.nseg;
         const int p0 = segi * sg.seg, p1 = min(p0 + sg.seg, g.n[0]);
         const int bin0 = pencil * g.n[0] + p0, bin1 = pencil * g.n[0] + p1;         // [bin0, bin1)
-        u0 = hist[bin0];
-        u1 = (bin1 < nbins) ? hist[bin1] : (unsigned)M;
+        u0 = offs[bin0];
+        u1 = (bin1 < nbins) ? offs[bin1] : (unsigned)M;
     };
     if (nps > kMaxSortedItems) {
         for (int i = tid; i < nps; i += kScanThreads) {
@@ -214,17 +186,9 @@ scan_kernel(unsigned* __restrict__ hist, unsigned* __restrict__ hist_next, int n
         if (i < nps) {
             unsigned u0, u1;
             units_of(i, u0, u1);
-            if (sg.chunk_major) {
-                // slab-major: all segments of x-slab 0 first (heaviest first inside the slab), then
-                // slab 1, ... — the CTAs in flight share one slab of one chunk of the table in L2
-                const unsigned segi = (unsigned)(i % sg.nseg);
-                key = ((127u - min(segi, 127u)) << 25) | (min(u1 - u0, 4095u) << 13) | (unsigned)i;
-                mine += 1;
-            } else {
-                const unsigned cnt = min(u1 - u0, (1u << 19) - 1u);
-                key = (cnt << 13) | (unsigned)i;
-                mine += (cnt != 0);
-            }
+            const unsigned cnt = min(u1 - u0, (1u << 19) - 1u);
+            key = (cnt << 13) | (unsigned)i;
+            mine += (cnt != 0);
         }
         keys[i] = key;
     }
@@ -1035,10 +999,9 @@ eval_staged_kernel(const __grid_constant__ CUtensorMap tmap, Geom g, StagedGeom 
                 WorkItem& it = sm.item[q];
                 Desc d = {-1, 0, 0, 0, 0};
                 if (w < nitems) {
-                    // heaviest segment first, its chunks side by side (sg.chunk_major: all segments
-                    // of chunk 0, then chunk 1, ... — better L2 locality, longer tail)
-                    d.chunk = sg.chunk_major ? w / nps : w % nchunk;
-                    const int4 o = __ldg(order + (sg.chunk_major ? w - d.chunk * nps : w / nchunk));
+                    // heaviest segment first, its chunks side by side
+                    d.chunk = w % nchunk;
+                    const int4 o = __ldg(order + w / nchunk);
                     const int pencil = o.x / sg.nseg, segi = o.x - pencil * sg.nseg;
                     d.lo = segi * sg.seg;
                     const int hi = min(d.lo + sg.seg, g.n[0]) - 1;
@@ -1237,31 +1200,6 @@ eval_staged_kernel(const __grid_constant__ CUtensorMap tmap, Geom g, StagedGeom 
         __syncwarp();
         u += NW;
     }
-}
-
-// ---------------------------------------------------------------------------------------
-// FP32 peak probe for the benchmark (the FP32 roofline is measured in the same
-// run): every thread runs `iters` rounds of 16 independent packed FMAs on registers.
-// ---------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(512)
-fp32_probe_kernel(float* __restrict__ out, int iters, float seed)
-{
-    u64 acc[16];
-#pragma unroll
-    for (int i = 0; i < 16; ++i) acc[i] = dup2(seed * (float)(i + 1 + threadIdx.x));
-    const u64 x = dup2(0.999f);
-    const float w = 1.0f + seed;
-#pragma unroll 1
-    for (int it = 0; it < iters; ++it) {
-#pragma unroll
-        for (int r = 0; r < 4; ++r)
-#pragma unroll
-            for (int i = 0; i < 16; ++i) acc[i] = fma2(acc[i], dup2(w), x);
-    }
-    float s = 0.f;
-#pragma unroll
-    for (int i = 0; i < 16; ++i) { const float2 v = unpack2(acc[i]); s += v.x + v.y; }
-    out[(size_t)blockIdx.x * blockDim.x + threadIdx.x] = s;
 }
 
 }  // namespace blip

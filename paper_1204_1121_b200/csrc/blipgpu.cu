@@ -2,6 +2,8 @@
 // Argument checking, the fp64 inverse lattice, device memory and kernel launches; every
 // step of the hot path itself runs in the kernels of blip_kernels.cuh.
 #include "blipgpu.h"
+#include "blipgpu_dev.h"
+#include "blip_host.h"
 #include "blip_kernels.cuh"
 #include "blip_f64.cuh"
 
@@ -10,9 +12,6 @@
 #include <cstring>
 #include <new>
 
-// Staged kernel variants (template constants of blip::eval_staged_kernel): pencil cross-section
-// BY x BZ cells, ring of R table planes in shared memory, NW consumer warps.  All use 4 floats
-// per lane (128 orbitals per tile row).  The variant is fixed per table at creation.
 namespace {
 // Launch with programmatic stream serialization: the kernel may be set up on the device while
 // its predecessor in the stream still runs; it starts with griddepcontrol.wait, which returns
@@ -30,8 +29,13 @@ cudaError_t launch_pdl(void (*kernel)(KArgs...), dim3 grid, dim3 block, size_t s
     return cudaLaunchKernelEx(&cfg, kernel, KArgs(args)...);
 }
 
-constexpr int kSVec = 4;
+// The staged kernel as shipped (blip::eval_staged_kernel template constants): 4 orbitals per
+// lane (128 per tile row), pencils of 4 x 4 cells, a ring of 8 table planes in shared memory,
+// 16 consumer warps.  The other shapes that were measured (4 x 8 pencils with a 5-plane ring;
+// 8 and 12 warps) lost and are not built (profiles/r1_v3.md).
+constexpr int kSVec = 4, kSBY = 4, kSBZ = 4, kSRing = 8, kSWarps = 16;
 constexpr int kSC = 32 * kSVec;
+using StagedShape = blip::StagedCfg<kSVec, kSBY, kSBZ, kSRing, kSWarps>;
 
 struct StagedArgs {
     const CUtensorMap* tmap; const blip::Geom* g; const blip::StagedGeom* sg; const float4* recs;
@@ -40,118 +44,43 @@ struct StagedArgs {
     const float* dvec; long long ldd; float* cout;
 };
 
-struct StagedVariant {
-    int by, bz, ring, warps;
-    size_t smem;
-    cudaError_t (*prepare)();
-    void (*launch)(int mode, unsigned nctas, cudaStream_t s, const StagedArgs& a);
-};
-
-template <int BY, int BZ, int R, int NW>
-struct SV {
-    using Cfg = blip::StagedCfg<kSVec, BY, BZ, R, NW>;
-    template <int MODE, bool CONTRACT>
-    static cudaError_t prep1()
-    {
-        return cudaFuncSetAttribute(blip::eval_staged_kernel<MODE, CONTRACT, kSVec, BY, BZ, R, NW>,
-                                    cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(typename Cfg::Smem));
-    }
-    static cudaError_t prepare()
-    {
-        cudaError_t e = prep1<0, false>();
-        if (e == cudaSuccess) e = prep1<1, false>();
-        if (e == cudaSuccess) e = prep1<2, false>();
-        if (e == cudaSuccess) e = prep1<0, true>();
-        if (e == cudaSuccess) e = prep1<1, true>();
-        if (e == cudaSuccess) e = prep1<2, true>();
-        return e;
-    }
-    template <int MODE, bool CONTRACT>
-    static void launch1(unsigned nctas, cudaStream_t s, const StagedArgs& a)
-    {
-        launch_pdl(blip::eval_staged_kernel<MODE, CONTRACT, kSVec, BY, BZ, R, NW>, nctas, Cfg::THREADS,
-                   sizeof(typename Cfg::Smem), s, *a.tmap, *a.g, *a.sg, a.recs, a.order, a.meta, a.nchunk, a.val, a.grad,
-                   a.lap, a.ld, a.dvec, a.ldd, a.cout);
-    }
-    static void launch(int mode, unsigned nctas, cudaStream_t s, const StagedArgs& a)
-    {
-        if (a.dvec) {
-            if (mode == 0) launch1<0, true>(nctas, s, a); else if (mode == 2) launch1<2, true>(nctas, s, a); else launch1<1, true>(nctas, s, a);
-        } else {
-            if (mode == 0) launch1<0, false>(nctas, s, a); else if (mode == 2) launch1<2, false>(nctas, s, a); else launch1<1, false>(nctas, s, a);
-        }
-    }
-    static constexpr StagedVariant variant() { return {BY, BZ, R, NW, sizeof(typename Cfg::Smem), &prepare, &launch}; }
-};
-
-const StagedVariant kVariants[] = {
-    SV<4, 8, 5, 8>::variant(),  SV<4, 8, 5, 12>::variant(),
-    SV<4, 4, 8, 8>::variant(),  SV<4, 4, 8, 12>::variant(), SV<4, 4, 8, 16>::variant(),
-};
-constexpr int kNumVariants = (int)(sizeof(kVariants) / sizeof(kVariants[0]));
-constexpr int kDefaultVariant = 4;
-
-int env_int(const char* name, int dflt)
+template <int MODE, bool CONTRACT>
+cudaError_t staged_prepare1()
 {
-    const char* v = std::getenv(name);
-    return v ? std::atoi(v) : dflt;
+    return cudaFuncSetAttribute(blip::eval_staged_kernel<MODE, CONTRACT, kSVec, kSBY, kSBZ, kSRing, kSWarps>,
+                                cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(StagedShape::Smem));
+}
+cudaError_t staged_prepare()
+{
+    cudaError_t e = staged_prepare1<0, false>();
+    if (e == cudaSuccess) e = staged_prepare1<1, false>();
+    if (e == cudaSuccess) e = staged_prepare1<2, false>();
+    if (e == cudaSuccess) e = staged_prepare1<0, true>();
+    if (e == cudaSuccess) e = staged_prepare1<1, true>();
+    if (e == cudaSuccess) e = staged_prepare1<2, true>();
+    return e;
+}
+template <int MODE, bool CONTRACT>
+cudaError_t staged_launch1(unsigned nctas, cudaStream_t s, const StagedArgs& a)
+{
+    return launch_pdl(blip::eval_staged_kernel<MODE, CONTRACT, kSVec, kSBY, kSBZ, kSRing, kSWarps>, nctas,
+                      StagedShape::THREADS, sizeof(StagedShape::Smem), s, *a.tmap, *a.g, *a.sg, a.recs, a.order, a.meta,
+                      a.nchunk, a.val, a.grad, a.lap, a.ld, a.dvec, a.ldd, a.cout);
+}
+cudaError_t staged_launch(int mode, unsigned nctas, cudaStream_t s, const StagedArgs& a)
+{
+    if (a.dvec) {
+        if (mode == 0) return staged_launch1<0, true>(nctas, s, a);
+        if (mode == 2) return staged_launch1<2, true>(nctas, s, a);
+        return staged_launch1<1, true>(nctas, s, a);
+    }
+    if (mode == 0) return staged_launch1<0, false>(nctas, s, a);
+    if (mode == 2) return staged_launch1<2, false>(nctas, s, a);
+    return staged_launch1<1, false>(nctas, s, a);
 }
 }
-
-struct blipgpu_table {
-    blip::Geom g;
-    blip::Geom64 g64;                // J and Q in fp64, for blipgpu_eval_f64
-    blip::StagedGeom sg;
-    int L = 0;
-    long long pitch = 0;             // floats per table row (multiple of 4)
-    long long nrows = 0;             // rows of the padded table, (n1+3)(n2+3)(n3+3)
-    float4* table = nullptr;         // device, ghost-padded [n1+3][n2+3][n3+3][pitch/4]
-    int nbins = 0;                   // max(bricks, staged bins)
-    int nbins_direct = 0, nbins_staged = 0;
-    int nq = 1;                      // direct kernel: quads of 4 orbitals per lane (1..3)
-    int diag = 0;                    // lattice vectors along the Cartesian axes: J diagonal (kernel MODE 2)
-    int path = 0;                    // 0 auto, 1 direct, 2 staged
-    int staged_ok = 0;               // TMA descriptor built and the grid is large enough
-    const StagedVariant* sv = nullptr;
-    int nchunk = 0;                  // staged path: orbital chunks of 128
-    int nsm = 0;                     // SMs of the device (CTAs of the persistent staged kernel)
-    long long l2_bytes = 0;          // L2 capacity of the device
-    CUtensorMap tmap;
-    int4* order = nullptr;           // [sg.nps] work items {segment, first unit, units, 0}, heaviest first
-    int* meta = nullptr;             // [2] {non-empty pencil segments, work counter}
-    // grouping workspace (device)
-    long long cap = 0;               // electrons the workspace holds
-    int* bin = nullptr;              // [cap]
-    int* perm = nullptr;             // [cap]
-    float4* recs = nullptr;          // [cap][24] per-electron records (staged path)
-    unsigned* hist = nullptr;        // [2][nbins]: the histograms of this call and of the next one alternate
-    int hist_cur = 0;
-    // staging for blipgpu_eval_host (device)
-    long long hcap = 0, hld = 0; int hmode = -1;
-    double* d_pos = nullptr; float* d_val = nullptr; float* d_grad = nullptr; float* d_lap = nullptr;
-    int* d_cell = nullptr;
-    cudaStream_t copy_stream = nullptr;
-    cudaEvent_t ev[2] = {nullptr, nullptr};
-    cudaEvent_t ev_in = nullptr;
-    // optional timing of the kernels of the last blipgpu_eval (blipgpu_set_profiling)
-    int profiling = 0;
-    cudaEvent_t pe[3] = {nullptr, nullptr, nullptr};   // call start, eval kernel start, end
-    int last_cuda = 0;
-    int last_path = 0;               // gather+FMA kernel of the last eval: 1 direct, 2 staged, 3 split
-    long long launches = 0;
-};
 
 static thread_local int g_create_cuda_error = 0;
-
-#define CK(t, call)                                                        \
-    do {                                                                   \
-        cudaError_t e_ = (call);                                           \
-        if (e_ != cudaSuccess) {                                           \
-            (t)->last_cuda = (int)e_;                                      \
-            (void)cudaGetLastError();                                      \
-            return e_ == cudaErrorMemoryAllocation ? BLIPGPU_ENOMEM : BLIPGPU_ECUDA; \
-        }                                                                  \
-    } while (0)
 
 // Inverse lattice by cofactors, G = adj(A)/det — the pinned fp64 sequence of DESIGN.md
 // "Index map" (each cofactor p*q - r*s, det = (A00 C00 + A01 C01) + A02 C02, true division).
@@ -178,12 +107,8 @@ static bool inverse_lattice(const double* A, double* G)
 
 // Quads per lane: a warp covers nq*128 orbitals of one electron.  Larger nq amortises the
 // per-column weight reads and address arithmetic over more FMAs at the cost of registers.
-static int default_nq(int pitch4)
+int blip_default_nq(int pitch4)
 {
-    if (const char* env = std::getenv("BLIPGPU_NQ")) {
-        const int v = std::atoi(env);
-        if (v >= 1 && v <= 3) return v;
-    }
     return pitch4 <= 32 ? 1 : (pitch4 < 96 ? 2 : 3);         // measured on the 1,536-orbital table: 3 > 1 > 2
 }
 
@@ -220,7 +145,7 @@ static bool build_tensor_map(blipgpu_table* t)
     const cuuint64_t dims[4] = {(cuuint64_t)t->pitch, (cuuint64_t)t->g.np[2], (cuuint64_t)t->g.np[1],
                                 (cuuint64_t)t->g.np[0]};
     const cuuint64_t strides[3] = {pitchB, pitchB * t->g.np[2], pitchB * t->g.np[2] * t->g.np[1]};
-    const cuuint32_t box[4] = {(cuuint32_t)kSC, (cuuint32_t)(t->sv->bz + 3), (cuuint32_t)(t->sv->by + 3), 1u};
+    const cuuint32_t box[4] = {(cuuint32_t)kSC, (cuuint32_t)(kSBZ + 3), (cuuint32_t)(kSBY + 3), 1u};
     const cuuint32_t estr[4] = {1u, 1u, 1u, 1u};
     const CUresult r = ((encode_fn)fn)(&t->tmap, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 4, t->table, dims, strides, box,
                                        estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
@@ -250,7 +175,13 @@ extern "C" int blipgpu_create(const double* lattice, const int* grid, int norb,
     cudaDeviceProp prop;
     if (ce == cudaSuccess) ce = cudaGetDeviceProperties(&prop, dev);
     if (ce != cudaSuccess) { g_create_cuda_error = (int)ce; (void)cudaGetLastError(); return BLIPGPU_ECUDA; }
-    if (prop.major != 10) return BLIPGPU_EARCH;      // sm_100a code only; no fallback
+    // The library holds sm_100a code only ('a' targets are not forward compatible, so 10.3 etc.
+    // cannot run it); no fallback.  The attribute query fails when the device has no image.
+    if (prop.major != 10 || prop.minor != 0) return BLIPGPU_EARCH;
+    {
+        cudaFuncAttributes fa;
+        if (cudaFuncGetAttributes(&fa, blip::bin_kernel) != cudaSuccess) { (void)cudaGetLastError(); return BLIPGPU_EARCH; }
+    }
 
     blipgpu_table* t = new (std::nothrow) blipgpu_table();
     if (!t) return BLIPGPU_ENOMEM;
@@ -281,28 +212,20 @@ extern "C" int blipgpu_create(const double* lattice, const int* grid, int norb,
     t->nrows = nrows;
     t->g.L = norb;
     t->g.pitch4 = (int)(pitch / 4);
-    int vi = env_int("BLIPGPU_SCFG", kDefaultVariant);
-    if (vi < 0 || vi >= kNumVariants) vi = kDefaultVariant;
-    t->sv = &kVariants[vi];
     t->nsm = prop.multiProcessorCount;
     t->l2_bytes = prop.l2CacheSize;
     t->nchunk = (int)((pitch + kSC - 1) / kSC);
-    t->sg.by = t->sv->by; t->sg.bz = t->sv->bz;
+    t->sg.by = kSBY; t->sg.bz = kSBZ;
     t->sg.nby = (grid[1] + t->sg.by - 1) / t->sg.by;
     t->sg.nbz = (grid[2] + t->sg.bz - 1) / t->sg.bz;
     // pencil segments: whole pencils unless that leaves fewer than ~4 work items per SM
     {
-        int seg = env_int("BLIPGPU_SEG", 0);
-        if (seg <= 0) {
-            seg = grid[0];
-            const long long pencils = (long long)t->sg.nby * t->sg.nbz * t->nchunk;
-            while (seg > 16 && pencils * ((grid[0] + seg - 1) / seg) < 4LL * t->nsm) seg = (seg + 1) / 2;
-        }
-        if (seg > grid[0]) seg = grid[0];
+        int seg = grid[0];
+        const long long pencils = (long long)t->sg.nby * t->sg.nbz * t->nchunk;
+        while (seg > 16 && pencils * ((grid[0] + seg - 1) / seg) < 4LL * t->nsm) seg = (seg + 1) / 2;
         t->sg.seg = seg;
     }
     t->sg.nseg = (grid[0] + t->sg.seg - 1) / t->sg.seg;
-    t->sg.chunk_major = env_int("BLIPGPU_CHUNK_MAJOR", 0);
     {
         const long long nps = (long long)t->sg.nby * t->sg.nbz * t->sg.nseg;
         t->sg.nps = nps < (1LL << 24) ? (int)nps : 0;
@@ -311,7 +234,7 @@ extern "C" int blipgpu_create(const double* lattice, const int* grid, int norb,
     const long long sbins = (long long)t->sg.nby * t->sg.nbz * grid[0];
     t->nbins_staged = (sbins < (1LL << 30) && t->sg.nps > 0) ? (int)sbins : 0;
     t->nbins = t->nbins_direct > t->nbins_staged ? t->nbins_direct : t->nbins_staged;
-    t->nq = default_nq(t->g.pitch4);
+    t->nq = blip_default_nq(t->g.pitch4);
 
     cudaStream_t s = (cudaStream_t)stream;
     int rc = BLIPGPU_OK;
@@ -324,8 +247,9 @@ extern "C" int blipgpu_create(const double* lattice, const int* grid, int norb,
     const size_t src_bytes = (size_t)nsites * (size_t)norb * sizeof(float);
     float* staging = nullptr;                         // device copy of a host table, until padded
     if ((e = cudaMalloc(&t->table, bytes)) != cudaSuccess) fail(e);
-    if (rc == BLIPGPU_OK && (e = cudaMalloc(&t->hist, 2 * sizeof(unsigned) * (size_t)t->nbins)) != cudaSuccess) fail(e);
-    if (rc == BLIPGPU_OK && (e = cudaMemsetAsync(t->hist, 0, 2 * sizeof(unsigned) * (size_t)t->nbins, s)) != cudaSuccess) fail(e);
+    if (rc == BLIPGPU_OK && (e = cudaMalloc(&t->hist, sizeof(unsigned) * (size_t)t->nbins)) != cudaSuccess) fail(e);
+    if (rc == BLIPGPU_OK && (e = cudaMalloc(&t->offs, sizeof(unsigned) * (size_t)t->nbins)) != cudaSuccess) fail(e);
+    if (rc == BLIPGPU_OK && (e = cudaMemsetAsync(t->hist, 0, sizeof(unsigned) * (size_t)t->nbins, s)) != cudaSuccess) fail(e);
     if (rc == BLIPGPU_OK && (e = cudaMalloc(&t->order, sizeof(int4) * (size_t)(t->sg.nps + 1))) != cudaSuccess) fail(e);
     if (rc == BLIPGPU_OK && (e = cudaMalloc(&t->meta, sizeof(int) * 2)) != cudaSuccess) fail(e);
     if (rc == BLIPGPU_OK && !coeffs_on_device) {
@@ -340,17 +264,13 @@ extern "C" int blipgpu_create(const double* lattice, const int* grid, int norb,
         if (e != cudaSuccess) fail(e);
     }
     if (staging) cudaFree(staging);
-    if (rc == BLIPGPU_OK && (e = cudaStreamCreateWithFlags(&t->copy_stream, cudaStreamNonBlocking)) != cudaSuccess) fail(e);
-    for (int k = 0; k < 2 && rc == BLIPGPU_OK; ++k)
-        if ((e = cudaEventCreateWithFlags(&t->ev[k], cudaEventDisableTiming)) != cudaSuccess) fail(e);
-    if (rc == BLIPGPU_OK && (e = cudaEventCreateWithFlags(&t->ev_in, cudaEventDisableTiming)) != cudaSuccess) fail(e);
     if (rc == BLIPGPU_OK) {
         // staged path: needs a full tile row (pitch >= C), a grid at least as large as one box,
         // the opt-in shared memory size, and the TMA descriptor
-        const bool fits = t->pitch >= kSC && t->g.np[1] >= t->sv->by + 3 && t->g.np[2] >= t->sv->bz + 3 &&
-                          t->nbins_staged > 0 && (size_t)prop.sharedMemPerBlockOptin >= t->sv->smem;
+        const bool fits = t->pitch >= kSC && t->g.np[1] >= kSBY + 3 && t->g.np[2] >= kSBZ + 3 &&
+                          t->nbins_staged > 0 && (size_t)prop.sharedMemPerBlockOptin >= sizeof(StagedShape::Smem);
         if (fits && build_tensor_map(t)) {
-            e = t->sv->prepare();
+            e = staged_prepare();
             if (e == cudaSuccess) t->staged_ok = 1; else (void)cudaGetLastError();
         }
     }
@@ -362,13 +282,10 @@ extern "C" int blipgpu_create(const double* lattice, const int* grid, int norb,
 extern "C" int blipgpu_destroy(blipgpu_table* t)
 {
     if (!t) return BLIPGPU_OK;
-    cudaFree(t->table); cudaFree(t->bin); cudaFree(t->perm); cudaFree(t->recs); cudaFree(t->hist);
-    cudaFree(t->order); cudaFree(t->meta);
+    cudaFree(t->table); cudaFree(t->bin); cudaFree(t->perm); cudaFree(t->recs); cudaFree(t->hist); cudaFree(t->offs);
+    cudaFree(t->order); cudaFree(t->meta); cudaFree(t->kvec);
     cudaFree(t->d_pos); cudaFree(t->d_val); cudaFree(t->d_grad); cudaFree(t->d_lap); cudaFree(t->d_cell);
-    if (t->copy_stream) cudaStreamDestroy(t->copy_stream);
-    for (int k = 0; k < 2; ++k) if (t->ev[k]) cudaEventDestroy(t->ev[k]);
     for (int k = 0; k < 3; ++k) if (t->pe[k]) cudaEventDestroy(t->pe[k]);
-    if (t->ev_in) cudaEventDestroy(t->ev_in);
     (void)cudaGetLastError();
     delete t;
     return BLIPGPU_OK;
@@ -410,38 +327,40 @@ static bool use_staged(const blipgpu_table* t, long long M)
     return 64.0 * (double)M / sites >= kStagedMinReuse;
 }
 
-// Mpol: the size of the caller's whole batch, which picks the kernel (blipgpu_eval_host cuts a
-// batch into pieces; all pieces then run the kernel the whole batch would, so that the host
-// and the device entry point return the same bits).
 // dvec != NULL: contraction mode (blipgpu_eval_contract): the orbitals are not stored but
 // contracted with dvec[e][.] into cout[e][0..4] (cleared by the caller of this function).
-static int launch_eval(blipgpu_table* t, const double* positions, long long M, long long Mpol, int mode,
+static int launch_eval(blipgpu_table* t, const double* positions, long long M, int mode,
                        float* val, float* grad, float* lap, long long ld, int* cell,
                        cudaStream_t s, const float* dvec = nullptr, long long ldd = 0, float* cout = nullptr)
 {
     const int* perm = nullptr;
-    const bool staged = use_staged(t, Mpol);
+    const bool staged = use_staged(t, M);
     const int kmode = mode == BLIPGPU_VALUE ? 0 : (t->diag ? 2 : 1);      // kernel template MODE
     if (t->profiling) CK(t, cudaEventRecord(t->pe[0], s));
     const bool grouped = staged || t->path == 1 ||
-                         (Mpol > kGroupThreshold && t->nrows * t->pitch * (long long)sizeof(float) > t->l2_bytes * 3 / 4);
+                         (M > kGroupThreshold && t->nrows * t->pitch * (long long)sizeof(float) > t->l2_bytes * 3 / 4);
     if (grouped && (staged || M > kGroupThreshold)) {
         int rc = ensure_workspace(t, M, s);
         if (rc != BLIPGPU_OK) return rc;
         const int nbins = staged ? t->nbins_staged : t->nbins_direct;
-        // the histogram of this call was cleared by the scan kernel of the previous one
-        unsigned* hist = t->hist + (size_t)t->hist_cur * (size_t)t->nbins;
-        unsigned* hist_next = t->hist + (size_t)(t->hist_cur ^ 1) * (size_t)t->nbins;
-        t->hist_cur ^= 1;
+        // t->hist is zero here: blipgpu_create cleared it and the scan kernel of every call puts
+        // back to zero what it reads, so the call is self-contained in stream order (no host-side
+        // state: a captured call can be replayed).  Only a launch failure half-way leaves it dirty.
+        if (t->hist_dirty) {
+            CK(t, cudaMemsetAsync(t->hist, 0, sizeof(unsigned) * (size_t)t->nbins, s));
+            t->hist_dirty = 0;
+        }
         const unsigned nb = (unsigned)((M + 255) / 256);
-        launch_pdl(blip::bin_kernel, nb, 256, 0, s, t->g, t->sg, staged ? 1 : 0, positions, M, t->bin, hist, cell);
-        launch_pdl(blip::scan_kernel, 1, blip::kScanThreads, 0, s, hist, hist_next, nbins, t->nbins, M, staged ? 1 : 0,
-                   t->g, t->sg, t->order, t->meta);
+        CK(t, launch_pdl(blip::bin_kernel, nb, 256, 0, s, t->g, t->sg, staged ? 1 : 0, positions, M, t->bin, t->hist, cell));
+        t->hist_dirty = 1;
+        CK(t, launch_pdl(blip::scan_kernel, 1, blip::kScanThreads, 0, s, t->hist, t->offs, nbins, M, staged ? 1 : 0,
+                         t->g, t->sg, t->order, t->meta));
+        t->hist_dirty = 0;
         if (staged)
-            launch_pdl(blip::scatter_prep_kernel, (unsigned)((M + 127) / 128), 128, 0, s, t->g, t->sg, kSC, positions,
-                       (const int*)t->bin, hist, M, t->recs);
+            CK(t, launch_pdl(blip::scatter_prep_kernel, (unsigned)((M + 127) / 128), 128, 0, s, t->g, t->sg, kSC, positions,
+                             (const int*)t->bin, t->offs, M, t->recs));
         else
-            launch_pdl(blip::scatter_kernel, nb, 256, 0, s, (const int*)t->bin, hist, M, t->perm);
+            CK(t, launch_pdl(blip::scatter_kernel, nb, 256, 0, s, (const int*)t->bin, t->offs, M, t->perm));
         t->launches += 3;
         perm = t->perm;
         cell = nullptr;                                  // already written by bin_kernel
@@ -450,9 +369,9 @@ static int launch_eval(blipgpu_table* t, const double* positions, long long M, l
         if (t->profiling) CK(t, cudaEventRecord(t->pe[1], s));
         const StagedArgs a = {&t->tmap, &t->g, &t->sg, t->recs, t->order, t->meta, t->nchunk,
                               val, grad, lap, ld, dvec, ldd, cout};
-        t->sv->launch(kmode, (unsigned)t->nsm, s, a);
+        CK(t, staged_launch(kmode, (unsigned)t->nsm, s, a));
         t->last_path = 2;
-    } else if (t->path == 0 && !perm && Mpol <= kSplitMax) {
+    } else if (t->path == 0 && !perm && M <= kSplitMax) {
         t->last_path = 3;
         if (t->profiling) CK(t, cudaEventRecord(t->pe[1], s));
         const dim3 grid((unsigned)M, (unsigned)((t->g.pitch4 + 31) / 32));
@@ -493,7 +412,7 @@ extern "C" int blipgpu_eval(blipgpu_table* t, const double* positions, long long
     if (((uintptr_t)val & 15) || (mode == BLIPGPU_VGL && (((uintptr_t)grad & 15) || ((uintptr_t)lap & 15))))
         return BLIPGPU_EINVAL;
     if (M >= (1LL << 31)) return BLIPGPU_EINVAL;
-    return launch_eval(t, positions, M, M, mode, val, grad, lap, ld, cell, (cudaStream_t)stream);
+    return launch_eval(t, positions, M, mode, val, grad, lap, ld, cell, (cudaStream_t)stream);
 }
 
 extern "C" int blipgpu_eval_contract(blipgpu_table* t, const double* positions, long long M, int mode,
@@ -507,7 +426,7 @@ extern "C" int blipgpu_eval_contract(blipgpu_table* t, const double* positions, 
     if (((uintptr_t)d & 15) || ((uintptr_t)out & 15) || M >= (1LL << 31)) return BLIPGPU_EINVAL;
     cudaStream_t s = (cudaStream_t)stream;
     CK(t, cudaMemsetAsync(out, 0, sizeof(float) * 8 * (size_t)M, s));
-    return launch_eval(t, positions, M, M, mode, nullptr, nullptr, nullptr, t->pitch, cell, s, d, ldd, out);
+    return launch_eval(t, positions, M, mode, nullptr, nullptr, nullptr, t->pitch, cell, s, d, ldd, out);
 }
 
 extern "C" int blipgpu_eval_f64(blipgpu_table* t, const double* positions, long long M, int mode,
@@ -547,11 +466,10 @@ static int ensure_host_staging(blipgpu_table* t, long long M, int mode, long lon
     const bool fits = M <= t->hcap && ld == t->hld && (mode <= t->hmode) && (!want_cell || t->d_cell);
     if (fits) return BLIPGPU_OK;
     CK(t, cudaStreamSynchronize(s));
-    CK(t, cudaStreamSynchronize(t->copy_stream));
     cudaFree(t->d_pos); cudaFree(t->d_val); cudaFree(t->d_grad); cudaFree(t->d_lap); cudaFree(t->d_cell);
     t->d_pos = nullptr; t->d_val = t->d_grad = t->d_lap = nullptr; t->d_cell = nullptr;
     t->hcap = 0; t->hmode = -1;
-    const long long cap = M > t->hcap ? M : t->hcap;
+    const long long cap = M;
     CK(t, cudaMalloc(&t->d_pos, sizeof(double) * 3 * (size_t)cap));
     CK(t, cudaMalloc(&t->d_val, sizeof(float) * (size_t)cap * (size_t)ld));
     if (mode == BLIPGPU_VGL) {
@@ -573,32 +491,22 @@ extern "C" int blipgpu_eval_host(blipgpu_table* t, const double* positions, long
     cudaStream_t s = (cudaStream_t)stream;
     rc = ensure_host_staging(t, M, mode, ld, cell != nullptr, s);
     if (rc != BLIPGPU_OK) return rc;
+    // positions in, ONE evaluation of the whole batch (the same kernels, hence the same bits, as
+    // blipgpu_eval on device buffers; the staged kernel streams the table once), results out.
+    // The device->host copy of psi dominates (the largest transfer in the paper's Table XI too,
+    // PAPER.md:343): 20 B per evaluation over PCIe against < 1 ms of kernel time, so there is
+    // nothing to gain from cutting the batch into pieces to overlap the two.
     CK(t, cudaMemcpyAsync(t->d_pos, positions, sizeof(double) * 3 * (size_t)M, cudaMemcpyHostToDevice, s));
-    // Batches: evaluate batch b on `s`, then copy its results out on the copy stream while
-    // batch b+1 is evaluated (the device->host copy of psi is the largest transfer in the
-    // paper's Table XI).
-    const long long B = 8192;
-    long long b0 = 0; int k = 0;
-    while (b0 < M) {
-        const long long nb = (M - b0 < B) ? (M - b0) : B;
-        rc = launch_eval(t, t->d_pos + 3 * b0, nb, M, mode, t->d_val + b0 * ld,
-                         mode == BLIPGPU_VGL ? t->d_grad + 3 * b0 * ld : nullptr,
-                         mode == BLIPGPU_VGL ? t->d_lap + b0 * ld : nullptr, ld,
-                         cell ? t->d_cell + 3 * b0 : nullptr, s);
-        if (rc != BLIPGPU_OK) return rc;
-        CK(t, cudaEventRecord(t->ev[k], s));
-        CK(t, cudaStreamWaitEvent(t->copy_stream, t->ev[k], 0));
-        const size_t rowb = sizeof(float) * (size_t)ld;
-        CK(t, cudaMemcpyAsync(val + b0 * ld, t->d_val + b0 * ld, rowb * (size_t)nb, cudaMemcpyDeviceToHost, t->copy_stream));
-        if (mode == BLIPGPU_VGL) {
-            CK(t, cudaMemcpyAsync(grad + 3 * b0 * ld, t->d_grad + 3 * b0 * ld, 3 * rowb * (size_t)nb, cudaMemcpyDeviceToHost, t->copy_stream));
-            CK(t, cudaMemcpyAsync(lap + b0 * ld, t->d_lap + b0 * ld, rowb * (size_t)nb, cudaMemcpyDeviceToHost, t->copy_stream));
-        }
-        if (cell)
-            CK(t, cudaMemcpyAsync(cell + 3 * b0, t->d_cell + 3 * b0, sizeof(int) * 3 * (size_t)nb, cudaMemcpyDeviceToHost, t->copy_stream));
-        b0 += nb; k ^= 1;
+    rc = launch_eval(t, t->d_pos, M, mode, t->d_val, mode == BLIPGPU_VGL ? t->d_grad : nullptr,
+                     mode == BLIPGPU_VGL ? t->d_lap : nullptr, ld, cell ? t->d_cell : nullptr, s);
+    if (rc != BLIPGPU_OK) return rc;
+    const size_t rowb = sizeof(float) * (size_t)ld;
+    CK(t, cudaMemcpyAsync(val, t->d_val, rowb * (size_t)M, cudaMemcpyDeviceToHost, s));
+    if (mode == BLIPGPU_VGL) {
+        CK(t, cudaMemcpyAsync(grad, t->d_grad, 3 * rowb * (size_t)M, cudaMemcpyDeviceToHost, s));
+        CK(t, cudaMemcpyAsync(lap, t->d_lap, rowb * (size_t)M, cudaMemcpyDeviceToHost, s));
     }
-    CK(t, cudaStreamSynchronize(t->copy_stream));
+    if (cell) CK(t, cudaMemcpyAsync(cell, t->d_cell, sizeof(int) * 3 * (size_t)M, cudaMemcpyDeviceToHost, s));
     CK(t, cudaStreamSynchronize(s));
     return BLIPGPU_OK;
 }
@@ -613,70 +521,6 @@ extern "C" int blipgpu_info(const blipgpu_table* t, int* grid, int* norb, long l
     if (table_bytes) *table_bytes = t->nrows * t->pitch * (long long)sizeof(float);   // ghost-padded
     return BLIPGPU_OK;
 }
-
-extern "C" int blipgpu_set_profiling(blipgpu_table* t, int on)
-{
-    if (!t) return BLIPGPU_EINVAL;
-    if (on)
-        for (int k = 0; k < 3; ++k)
-            if (!t->pe[k]) CK(t, cudaEventCreate(&t->pe[k]));
-    t->profiling = on ? 1 : 0;
-    return BLIPGPU_OK;
-}
-
-extern "C" int blipgpu_last_kernel_ms(blipgpu_table* t, float* group_ms, float* eval_ms)
-{
-    if (!t || !t->profiling || !t->pe[2]) return BLIPGPU_EINVAL;
-    CK(t, cudaEventSynchronize(t->pe[2]));
-    float a = 0.f, b = 0.f;
-    CK(t, cudaEventElapsedTime(&a, t->pe[0], t->pe[1]));
-    CK(t, cudaEventElapsedTime(&b, t->pe[1], t->pe[2]));
-    if (group_ms) *group_ms = a;
-    if (eval_ms) *eval_ms = b;
-    return BLIPGPU_OK;
-}
-
-extern "C" int blipgpu_set_tuning(blipgpu_table* t, int path, int nq)
-{
-    if (!t || path < 0 || path > 2 || nq < 0 || nq > 3) return BLIPGPU_EINVAL;
-    if (path == 2 && !t->staged_ok) return BLIPGPU_EINVAL;
-    t->path = path;
-    t->nq = nq ? nq : default_nq(t->g.pitch4);
-    return BLIPGPU_OK;
-}
-
-
-extern "C" int blipgpu_probe_fp32(blipgpu_table* t, double* tflops, void* stream)
-{
-    if (!t || !tflops) return BLIPGPU_EINVAL;
-    cudaStream_t s = (cudaStream_t)stream;
-    const int blocks = t->nsm * 4, threads = 512, iters = 4096;
-    float* out = nullptr;
-    CK(t, cudaMalloc(&out, sizeof(float) * (size_t)blocks * threads));
-    cudaEvent_t e0 = nullptr, e1 = nullptr;
-    int rc = BLIPGPU_OK;
-    float ms = 0.f;
-    cudaError_t e = cudaEventCreate(&e0);
-    if (e == cudaSuccess) e = cudaEventCreate(&e1);
-    for (int rep = 0; rep < 3 && e == cudaSuccess; ++rep) {          // the last of three runs is timed
-        e = cudaEventRecord(e0, s);
-        blip::fp32_probe_kernel<<<blocks, threads, 0, s>>>(out, iters, 1e-9f);
-        if (e == cudaSuccess) e = cudaEventRecord(e1, s);
-        if (e == cudaSuccess) e = cudaEventSynchronize(e1);
-        if (e == cudaSuccess) e = cudaEventElapsedTime(&ms, e0, e1);
-    }
-    if (e != cudaSuccess) { t->last_cuda = (int)e; (void)cudaGetLastError(); rc = BLIPGPU_ECUDA; }
-    else *tflops = 2.0 * 2.0 * 64.0 * (double)iters * (double)blocks * threads / (ms * 1e-3) / 1e12;
-    if (e0) cudaEventDestroy(e0);
-    if (e1) cudaEventDestroy(e1);
-    cudaFree(out);
-    t->launches += 3;
-    return rc;
-}
-
-extern "C" int blipgpu_last_path(const blipgpu_table* t) { return t ? t->last_path : 0; }
-
-extern "C" long long blipgpu_launch_count(const blipgpu_table* t) { return t ? t->launches : 0; }
 
 extern "C" const char* blipgpu_strerror(int code)
 {

@@ -1,0 +1,33 @@
+"""Build tests/harness/blip_harness (plain C, gcc) against paper_1204_1121_b200/libblipgpu.so and
+the CUDA runtime.  Used by tests/test_gpu_harness.py, by bench.py's per-call latency rows and
+by the compute-sanitizer runs recorded under profiles/."""
+import os
+import subprocess
+import sys
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+ROOT = os.path.dirname(os.path.dirname(HERE))
+SRC = os.path.join(HERE, "blip_harness.c")
+EXE = os.path.join(HERE, "blip_harness")
+CUDA = os.environ.get("CUDA_HOME", "/usr/local/cuda")
+
+
+def build(force=False):
+    if ROOT not in sys.path:
+        sys.path.insert(0, ROOT)
+    from paper_1204_1121_b200 import _build
+    lib = _build.build()
+    libdir = os.path.dirname(lib)
+    deps = [SRC, lib, os.path.join(ROOT, "include", "blipgpu.h"), os.path.join(ROOT, "include", "blipgpu_dev.h")]
+    if not force and os.path.exists(EXE) and all(os.path.getmtime(EXE) >= os.path.getmtime(d) for d in deps):
+        return EXE
+    cmd = ["gcc", "-O2", "-std=c11", "-D_POSIX_C_SOURCE=200809L", "-Wall", "-Wextra", "-I", os.path.join(ROOT, "include"),
+           "-I", os.path.join(CUDA, "include"), "-o", EXE, SRC, "-L", libdir, "-lblipgpu",
+           "-L", os.path.join(CUDA, "lib64"), "-lcudart", "-lm",
+           "-Wl,-rpath," + libdir, "-Wl,-rpath," + os.path.join(CUDA, "lib64")]
+    subprocess.run(cmd, check=True)
+    return EXE
+
+
+if __name__ == "__main__":
+    print(build(force=True))

@@ -13,10 +13,16 @@ import paper_1204_1121_b200 as blip
 ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 
 
-def declared_symbols():
-    text = open(os.path.join(ROOT, "include", "blipgpu.h")).read()
-    text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
-    return sorted(set(re.findall(r"\b(blipgpu_[a-z0-9_]+)\s*\(", text)))
+def declared_symbols(header=None):
+    """Function names declared in include/*.h (comments stripped)."""
+    names = set()
+    for h in sorted(os.listdir(os.path.join(ROOT, "include"))):
+        if not h.endswith(".h") or (header and h != header):
+            continue
+        text = open(os.path.join(ROOT, "include", h)).read()
+        text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
+        names |= set(re.findall(r"\b(blipgpu_[a-z0-9_]+)\s*\(", text))
+    return sorted(names)
 
 
 def test_header_symbols_are_exported_and_bound():
@@ -27,6 +33,15 @@ def test_header_symbols_are_exported_and_bound():
     for n in names:
         assert hasattr(L, n), f"{n} declared in blipgpu.h but not exported"
     assert sorted(blip.SIGNATURES) == names
+    # the boundary proper carries no test / benchmark instrumentation
+    boundary = set(declared_symbols("blipgpu.h"))
+    assert not boundary & {"blipgpu_set_tuning", "blipgpu_probe_fp32", "blipgpu_set_profiling",
+                           "blipgpu_last_kernel_ms", "blipgpu_launch_count", "blipgpu_last_path"}
+
+
+def test_library_reads_no_environment_knobs():
+    for f in os.listdir(os.path.join(ROOT, "paper_1204_1121_b200", "csrc")):
+        assert "getenv" not in open(os.path.join(ROOT, "paper_1204_1121_b200", "csrc", f)).read(), f
 
 
 def test_strerror_is_total():

@@ -225,6 +225,81 @@ def test_eval_host_matches_eval(torch_cuda, blip):
     t.close()
 
 
+def test_eval_host_staged_path_large_batch(torch_cuda, blip):
+    """blipgpu_eval_host on the staged path with more than 8,192 positions: one evaluation of the
+    whole batch, the bits of blipgpu_eval."""
+    torch = torch_cuda
+    grid, L, M = (17, 12, 19), 257, 20000
+    A, c, pos = workloads.small_case(grid, L, M, TRICLINIC, seed=14, spread=3.0)
+    ld = 260
+    t = blip.BlipTable(A, grid, L, c)
+    blip.blipgpu_set_tuning(t.handle, path=2)
+    dev = run_gpu(torch, blip, A, grid, c, pos, table=t)
+    hpos = torch.from_numpy(pos).pin_memory()
+    hval = torch.empty((M, ld), dtype=torch.float32).pin_memory()
+    hgrad = torch.empty((M, 3, ld), dtype=torch.float32).pin_memory()
+    hlap = torch.empty((M, ld), dtype=torch.float32).pin_memory()
+    n0 = t.launch_count()
+    blip.blipgpu_eval_host(t.handle, hpos, M, blip.VGL, hval, hgrad, hlap, ld, None)
+    assert t.launch_count() - n0 == 4 and blip.blipgpu_last_path(t.handle) == 2
+    assert np.array_equal(hval.numpy()[:, :L], dev[0])
+    assert np.array_equal(hgrad.numpy()[:, :, :L], dev[1])
+    assert np.array_equal(hlap.numpy()[:, :L], dev[2])
+    # grouped direct path, 8,192 < M <= 10,240 (the remainder used to run another kernel)
+    blip.blipgpu_set_tuning(t.handle, path=1)
+    dev = run_gpu(torch, blip, A, grid, c, pos[:9000], table=t)
+    blip.blipgpu_eval_host(t.handle, hpos, 9000, blip.VGL, hval, hgrad, hlap, ld, None)
+    assert np.array_equal(hval.numpy()[:9000, :L], dev[0]) and np.array_equal(hlap.numpy()[:9000, :L], dev[2])
+    t.close()
+
+
+@pytest.mark.parametrize("path", [1, 2])
+def test_grouped_call_replayed_from_a_cuda_graph(torch_cuda, blip, path):
+    """A grouped / staged blipgpu_eval (M > 2,048: bin, scan, scatter, evaluate) keeps no state
+    between calls, so it can be captured in a CUDA graph and replayed: three calls (an odd number)
+    on two batches are captured once and replayed five times; every replay returns the bits of
+    the eager calls, and eager calls after the replays still do."""
+    torch = torch_cuda
+    grid, L = (17, 12, 19), 257
+    A, c, pos = workloads.small_case(grid, L, 9000, TRICLINIC, seed=15, spread=3.0)
+    t = blip.BlipTable(A, grid, L, c)
+    blip.blipgpu_set_tuning(t.handle, path=path)
+    blip.blipgpu_reserve(t.handle, 9000)
+    da, db = torch.from_numpy(pos).cuda(), torch.from_numpy(pos[:5000][::-1].copy()).cuda()
+    ld = t.ld
+
+    def bufs(M):
+        return (torch.zeros((M, ld), dtype=torch.float32, device="cuda"), torch.zeros((M, 3, ld), dtype=torch.float32, device="cuda"),
+                torch.zeros((M, ld), dtype=torch.float32, device="cuda"))
+
+    ref_a, ref_b = bufs(9000), bufs(5000)
+    blip.blipgpu_eval(t.handle, da, 9000, blip.VGL, *ref_a, ld)
+    blip.blipgpu_eval(t.handle, db, 5000, blip.VGL, *ref_b, ld)
+    torch.cuda.synchronize()
+    out_a, out_b, out_c = bufs(9000), bufs(5000), bufs(9000)
+    side = torch.cuda.Stream()
+    side.wait_stream(torch.cuda.current_stream())
+    graph = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(graph, stream=side):
+        blip.blipgpu_eval(t.handle, da, 9000, blip.VGL, *out_a, ld, None, side)
+        blip.blipgpu_eval(t.handle, db, 5000, blip.VGL, *out_b, ld, None, side)
+        blip.blipgpu_eval(t.handle, da, 9000, blip.VGL, *out_c, ld, None, side)
+    for _ in range(5):
+        for o in (*out_a, *out_b, *out_c):
+            o.zero_()
+        graph.replay()
+        torch.cuda.synchronize()
+        for r, o in zip((*ref_a, *ref_b, *ref_a), (*out_a, *out_b, *out_c)):
+            assert torch.equal(r, o)
+    again = bufs(9000)
+    blip.blipgpu_eval(t.handle, da, 9000, blip.VGL, *again, ld)
+    torch.cuda.synchronize()
+    for r, o in zip(ref_a, again):
+        assert torch.equal(r, o)
+    del graph
+    t.close()
+
+
 def test_argument_errors(torch_cuda, blip):
     torch = torch_cuda
     A, c, pos = workloads.small_case((4, 4, 4), 6, 8, SKEW, seed=2)

@@ -1,0 +1,40 @@
+"""The plain-C caller tests/harness/blip_harness.c (no Python between the caller and the C ABI):
+it builds against include/blipgpu.h as a C11 translation unit, its self-test of every kernel
+passes, and its per-call latency rows (BASELINE.json configs[3], PAPER.md:268 kernel (1)) are
+well-formed."""
+import json
+import os
+import subprocess
+import sys
+
+import pytest
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+sys.path.insert(0, os.path.join(ROOT, "tests", "harness"))
+import build as harness_build  # noqa: E402
+
+
+def test_harness_builds_as_plain_c():
+    exe = harness_build.build(force=True)
+    assert os.access(exe, os.X_OK)
+    r = subprocess.run([exe], capture_output=True, text=True)
+    assert r.returncode == 64 and "usage" in r.stderr
+
+
+@pytest.mark.gpu
+def test_harness_selftest():
+    r = subprocess.run([harness_build.build(), "selftest"], capture_output=True, text=True, timeout=600)
+    assert r.returncode == 0, r.stdout + r.stderr
+    assert "selftest: 0 failure(s)" in r.stdout
+    assert "kernel=2" in r.stdout and "kernel=1" in r.stdout and "kernel=3" in r.stdout
+
+
+@pytest.mark.gpu
+def test_harness_latency_rows():
+    r = subprocess.run([harness_build.build(), "latency", "60"], capture_output=True, text=True, timeout=900)
+    assert r.returncode == 0, r.stdout + r.stderr
+    line = json.loads(r.stdout.strip().splitlines()[-1])
+    rows = line["rows"]
+    assert [x["M"] for x in rows if x["mode"] == "vgl"] == [1, 8, 32, 128, 512, 1536]
+    for x in rows:
+        assert x["kernel"] == 3 and 0.5 < x["us_back_to_back"] < 5e3 and x["us_call_and_wait_median"] >= x["us_p10"]

@@ -24,6 +24,14 @@ def test_random_shape(torch_cuda, blip, seed):
         lat = np.diag(rng.uniform(3, 12, size=3))
     else:
         lat = np.diag(rng.uniform(5, 12, size=3)) + rng.uniform(-1.5, 1.5, size=(3, 3))
+    # DESIGN.md reading R13a: north_star's Laplacian bound uses the LARGEST plane spacing while the
+    # fp32 rounding error scales with the smallest one, so the bound is only claimed for spacing
+    # ratios up to 10 (the five configs have <= 1.09).  Redraw the grid until the case is inside.
+    while True:
+        hs = oracle.spacing(lat, grid)
+        if hs.max() / hs.min() <= 10.0:
+            break
+        grid = tuple(int(x) for x in rng.integers(4, 40, size=3))
     path = int(rng.choice([0, 0, 1, 2]))
     mode = int(rng.choice([0, 1, 1]))
     contract = rng.random() < 0.3

@@ -513,3 +513,23 @@ def test_contract_one_hot_selects_an_orbital_and_constant_table_sums_d():
     assert np.abs(out[:, 1:]).max() < 1e-11
     vo = oracle.contract(val, None, None, d1)
     assert np.array_equal(vo[:, 0], oracle.contract(val, grad, lap, d1)[:, 0]) and not vo[:, 1:].any()
+
+
+def test_contract_rows_equals_contract_and_its_pins():
+    """oracle.contract_rows (numpy dot per position, used for full-size comparisons) against the
+    loop form oracle.contract, and against the same one-hot / constant-table facts."""
+    rng = np.random.default_rng(6)
+    A, c, pos = workloads.small_case((6, 5, 7), 37, 40, ((5.0, 0.3, -0.2), (1.1, 4.0, 0.7), (-0.6, 0.9, 6.0)), seed=9)
+    val, grad, lap, _ = oracle.eval_fast(A, (6, 5, 7), c, pos)
+    d = rng.standard_normal((40, 37))
+    a, b = oracle.contract(val, grad, lap, d), oracle.contract_rows(val, grad, lap, d)
+    scale = np.abs(val).max() * np.abs(d).sum(axis=1).max()
+    assert np.abs(a[:, 0] - b[:, 0]).max() <= 1e-14 * scale
+    assert np.abs(a[:, 1:4] - b[:, 1:4]).max() <= 1e-14 * np.abs(grad).max() * np.abs(d).sum(axis=1).max()
+    assert np.abs(a[:, 4] - b[:, 4]).max() <= 1e-14 * np.abs(lap).max() * np.abs(d).sum(axis=1).max()
+    e = np.zeros((40, 37)); e[:, 11] = 1.0
+    out = oracle.contract_rows(val, grad, lap, e)
+    assert np.array_equal(out[:, 0], val[:, 11]) and np.array_equal(out[:, 1:4], grad[:, :, 11])
+    assert np.array_equal(out[:, 4], lap[:, 11])
+    vo = oracle.contract_rows(val, None, None, d)
+    assert np.array_equal(vo[:, 0], b[:, 0]) and not vo[:, 1:].any()
