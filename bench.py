@@ -2,7 +2,7 @@
 """bench.py — orbital evaluations/s (value + gradient + Laplacian, fp32) of the blip hot path.
 
     python bench.py [--gpus N] [--steps K] [--warmup W] [--workload tio2|small|tiny|large]
-                    [--mode vgl|value] [--sweep] [--impl reference]
+                    [--mode vgl|value] [--no-configs] [--impl reference]
 
 One "step" is one blipgpu_eval over one batch of synthetic positions: every row of SURVEY.md
 §8a (cell map, weights, 64-row gather + FMA, grouping, output).  At N = 1 the workload is
@@ -225,6 +225,201 @@ def needs_l2_flush(cfg, args):
 # ---------------------------------------------------------------------------------------------
 # GPU arm
 # ---------------------------------------------------------------------------------------------
+KERNEL_NAMES = {1: "blip::eval_direct_kernel", 2: "blip::eval_staged_kernel", 3: "blip::eval_split_kernel"}
+FMA_PER_EVAL_CONTRACT = {True: 320, False: 64}      # SURVEY.md §8d R_fp32: five weights per site x 64 sites
+
+
+def distinct_rows(torch, cells, grid):
+    """Number of distinct table rows the batch touches (R_compulsory of SURVEY.md §8d), counted on
+    the device from the `cell` output of blipgpu_eval: the 4x4x4 block of sites of every position."""
+    n = torch.tensor(list(grid), device="cuda", dtype=torch.int64)
+    off = torch.arange(-1, 3, device="cuda", dtype=torch.int64)
+    ci = cells.to(torch.int64)
+    ci = ci[(ci >= 0).all(dim=1)]
+    seen = torch.zeros(int(n[0] * n[1] * n[2]), dtype=torch.bool, device="cuda")
+    for lo in range(0, ci.shape[0], 1 << 16):
+        c = ci[lo:lo + (1 << 16)]
+        k0 = (c[:, 0:1] + off) % n[0]
+        k1 = (c[:, 1:2] + off) % n[1]
+        k2 = (c[:, 2:3] + off) % n[2]
+        rows = ((k0[:, :, None, None] * n[1] + k1[:, None, :, None]) * n[2] + k2[:, None, None, :]).reshape(-1)
+        seen[rows] = True
+    return int(seen.sum())
+
+
+def roofline_block(torch, blip, handle, cfg, M, L, mode_vgl, k_ms, g_ms, n_rows, fp32_meas, nsm):
+    """The `roofline` object of the JSON line for the dominant (gather + FMA) kernel.
+
+    SURVEY.md §8d gives three figures per evaluation and says which one binds:
+      R_gather      64 x 4 B gathered + 20 B (4 B) written, at the HBM copy rate — north_star's contract
+                    roofline ("the slower of the gathered coefficient and output bytes at HBM bandwidth
+                    and the FMAs at FP32 peak"), with its >= 60 % target;
+      R_fp32        320 (64) FMAs at the FP32 peak;
+      R_compulsory  distinct rows once + the outputs, at the HBM copy rate.
+    A kernel that shares rows between electrons on chip runs faster than R_gather allows; then
+    max(R_compulsory, R_fp32) is what binds it and `bound`/`achieved`/`peak`/`frac` describe that
+    bound; the contract figure is kept under `contract_frac`."""
+    peak_hbm, peak_src, sm_max = measured_peaks()
+    evals = M * L
+    gather_bytes = algorithmic_bytes(M, L, mode_vgl)
+    comp_bytes = n_rows * L * 4 + evals * (20 if mode_vgl else 4)
+    flops = 2.0 * FMA_PER_EVAL_CONTRACT[mode_vgl] * evals
+    fp32_nominal = nsm * 128 * 2 * sm_max * 1e6                     # FP32 lanes x 2 flop x max SM clock (B200_PROFILING.md)
+    t = k_ms * 1e-3
+    t_gather = gather_bytes / (peak_hbm * 1e9)
+    t_comp = comp_bytes / (peak_hbm * 1e9)
+    t_fp32 = flops / fp32_meas
+    beats_gather = t < t_gather
+    t_hbm = t_comp if beats_gather else t_gather
+    if t_fp32 >= t_hbm:
+        bound, unit, achieved, peak = "alu", "TFLOP/s", flops / t / 1e12, fp32_meas / 1e12
+        peak_source = ("packed-FP32 FMA rate measured in this run (blipgpu_probe_fp32); nominal "
+                       f"{nsm} SMs x 128 lanes x 2 x {sm_max:.0f} MHz = {fp32_nominal / 1e12:.2f} TFLOP/s (DESIGN.md §6)")
+        per_unit = f"{FMA_PER_EVAL_CONTRACT[mode_vgl]} FMA per evaluation (SURVEY.md §8d R_fp32)"
+    else:
+        hb = comp_bytes if beats_gather else gather_bytes
+        bound, unit, achieved, peak = "hbm", "GB/s", hb / t / 1e9, peak_hbm
+        peak_source = peak_src
+        per_unit = ("distinct table rows once + outputs (SURVEY.md §8d R_compulsory)" if beats_gather
+                    else "256 B gathered + 20 B (4 B) written per evaluation (SURVEY.md §8d R_gather)")
+    out = {
+        "bound": bound, "achieved": achieved, "peak": peak, "unit": unit, "frac": achieved / peak, "traffic": None,
+        "kernel": KERNEL_NAMES.get(blip.blipgpu_last_path(handle), "?") + " (gather + FMA, steps a-2, a-3, a-5)",
+        "kernel_ms": k_ms, "grouping_ms": g_ms, "kernel_share_of_step": k_ms / (k_ms + g_ms) if k_ms + g_ms > 0 else None,
+        "algorithmic_per_unit": per_unit, "peak_source": peak_source,
+        "binding": ("max(R_compulsory, R_fp32): the kernel beats R_gather by sharing rows on chip" if beats_gather
+                    else "max(R_gather, R_fp32)"),
+        "bound_ms": {"R_gather": 1e3 * t_gather, "R_fp32": 1e3 * t_fp32, "R_compulsory": 1e3 * t_comp},
+        "contract_frac": gather_bytes / t / 1e9 / peak_hbm, "contract_target": 0.6,
+        "contract_note": "north_star's roofline: R_gather bytes at the measured HBM copy rate; >= 0.6 asked, "
+                         "> 1 means rows are served from shared memory / L2 instead of HBM",
+        "gather_bytes": gather_bytes, "compulsory_bytes": comp_bytes, "distinct_rows": n_rows,
+        "compulsory_hbm_frac": comp_bytes / t / 1e9 / peak_hbm,
+        "fp32_frac_issued": 2 * fma_count(M, L, mode_vgl) / t / fp32_meas,
+        "fp32_peak_tflops_measured": fp32_meas / 1e12, "fp32_peak_tflops_nominal": fp32_nominal / 1e12,
+        "hbm_peak_GBps": peak_hbm,
+    }
+    traffic_file = os.path.join(ROOT, "profiles", "traffic.json")     # written from ncu --set full captures
+    try:
+        with open(traffic_file) as fh:
+            tr = json.load(fh)
+        key = f"{cfg.name}:{'vgl' if mode_vgl else 'value'}"
+        if key in tr:
+            out["traffic"] = tr[key]["dram_bytes_per_launch"]
+            out["traffic_source"] = tr[key].get("source")
+            out["traffic_over_compulsory"] = tr[key]["dram_bytes_per_launch"] / comp_bytes
+    except Exception:
+        pass
+    return out
+
+
+class Workload:
+    """One config resident on the device: table handle, positions, output buffers."""
+
+    def __init__(self, torch, blip, cfg, mode_vgl, rank=0, M=None):
+        self.torch, self.blip, self.cfg, self.mode_vgl = torch, blip, cfg, mode_vgl
+        self.mode = blip.VGL if mode_vgl else blip.VALUE
+        self.L, self.ld = cfg.norb, (cfg.norb + 3) // 4 * 4
+        self.coeffs = workloads.coefficients(cfg.grid, cfg.norb)
+        self.handle = blip.blipgpu_create(workloads.lattice(cfg), cfg.grid, self.L, self.coeffs)
+        self.hpos = workloads.positions(cfg, rank=rank, M=M)
+        self.M = self.hpos.shape[0]
+        blip.blipgpu_reserve(self.handle, self.M)
+        self.stream = torch.cuda.current_stream()
+        self.dpos = torch.from_numpy(self.hpos).cuda()
+        self.val = torch.empty((self.M, self.ld), dtype=torch.float32, device="cuda")
+        self.grad = torch.empty((self.M, 3, self.ld), dtype=torch.float32, device="cuda")
+        self.lap = torch.empty((self.M, self.ld), dtype=torch.float32, device="cuda")
+
+    def step(self, M=None, mode=None, pos=None, stream=None):
+        self.blip.blipgpu_eval(self.handle, self.dpos if pos is None else pos, self.M if M is None else M,
+                               self.mode if mode is None else mode, self.val, self.grad, self.lap, self.ld, None,
+                               self.stream if stream is None else stream)
+
+    def close(self):
+        self.blip.blipgpu_destroy(self.handle)
+        self.handle = None
+
+
+def time_steps(torch, w, steps, warmup, flush, barrier=None):
+    """W warm-ups, then exactly `steps` steps.  Without flush: one event pair around all steps.  With
+    flush (working set would fit in L2): a 512 MB buffer is overwritten before every step and every
+    step has its own event pair.  Returns (total milliseconds, kernels launched in the timed region)."""
+    sync = barrier or torch.cuda.synchronize
+    for _ in range(warmup):
+        w.step()
+    sync()
+    n0 = w.blip.blipgpu_launch_count(w.handle)
+    if not flush:
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(w.stream)
+        for _ in range(steps):
+            w.step()
+        e1.record(w.stream)
+        sync()
+        return e0.elapsed_time(e1), w.blip.blipgpu_launch_count(w.handle) - n0
+    scratch = torch.empty(512 * 1024 * 1024, dtype=torch.uint8, device="cuda")
+    pairs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(steps)]
+    for a, b in pairs:
+        scratch.add_(1)                                        # evicts the table and the outputs from L2
+        a.record(w.stream)
+        w.step()
+        b.record(w.stream)
+    sync()
+    return sum(a.elapsed_time(b) for a, b in pairs), w.blip.blipgpu_launch_count(w.handle) - n0
+
+
+def kernel_times(w, reps, flush_buf=None):
+    """Device time of the grouping kernels and of the gather + FMA kernel of a step, from the
+    library's own events on the launching stream (blipgpu_set_profiling), mean over `reps` steps."""
+    blip = w.blip
+    blip.blipgpu_set_profiling(w.handle, 1)
+    kms, gms = [], []
+    for _ in range(reps):
+        if flush_buf is not None:
+            flush_buf.add_(1)
+        w.step()
+        g_, k_ = blip.blipgpu_last_kernel_ms(w.handle)
+        gms.append(g_)
+        kms.append(k_)
+    blip.blipgpu_set_profiling(w.handle, 0)
+    return float(np.mean(kms)), float(np.mean(gms))
+
+
+def measure_config(torch, blip, name, steps, fp32_meas, nsm, mode_vgl=True):
+    """One of the other BASELINE.json configs for the `configs` block: ms per step, evaluations/s,
+    the kernel that ran, and the same roofline object as the headline."""
+    cfg = workloads.CONFIGS[name]
+
+    class A:                                                   # needs_l2_flush reads .mode
+        mode = "vgl" if mode_vgl else "value"
+    flush = needs_l2_flush(cfg, A)
+    w = Workload(torch, blip, cfg, mode_vgl)
+    try:
+        ms = time_steps(torch, w, steps, 3, flush)[0] / steps
+        fb = torch.empty(512 * 1024 * 1024, dtype=torch.uint8, device="cuda") if flush else None
+        k_ms, g_ms = kernel_times(w, min(steps, 10), fb)
+        del fb
+        cells = torch.empty((w.M, 3), dtype=torch.int32, device="cuda")
+        blip.blipgpu_eval(w.handle, w.dpos, w.M, w.mode, w.val, w.grad, w.lap, w.ld, cells, w.stream)
+        torch.cuda.synchronize()
+        rows = distinct_rows(torch, cells, cfg.grid)
+        roof = roofline_block(torch, blip, w.handle, cfg, w.M, w.L, mode_vgl, k_ms, g_ms, rows, fp32_meas, nsm)
+        keep = ("bound", "achieved", "peak", "unit", "frac", "kernel", "kernel_ms", "grouping_ms", "binding", "bound_ms",
+                "contract_frac", "compulsory_hbm_frac", "distinct_rows", "traffic", "traffic_source")
+        return {"workload": f"{cfg.name}: BASELINE.json configs[{list(workloads.CONFIGS).index(cfg.name)}]",
+                "positions": w.M, "orbitals": w.L, "grid": list(cfg.grid), "table_bytes": cfg.table_bytes,
+                "mode": "value+grad+lap" if mode_vgl else "value", "steps": steps, "ms_per_step": ms,
+                "evals_per_s": w.M * w.L / (ms * 1e-3), "positions_per_s": w.M / (ms * 1e-3),
+                "last_path": blip.blipgpu_last_path(w.handle),
+                "l2": "flushed between steps" if flush else "no flush (working set exceeds L2)",
+                "roofline": {k: roof[k] for k in keep if k in roof}}
+    finally:
+        w.close()
+        del w
+        torch.cuda.empty_cache()
+
+
 def run_gpu(args):
     import torch
     import paper_1204_1121_b200 as blip
@@ -247,129 +442,48 @@ def run_gpu(args):
 
     cfg = workloads.CONFIGS[args.workload]
     mode_vgl = args.mode == "vgl"
-    mode = blip.VGL if mode_vgl else blip.VALUE
-    L, ld = cfg.norb, (cfg.norb + 3) // 4 * 4
-    A = workloads.lattice(cfg)
-    coeffs = workloads.coefficients(cfg.grid, cfg.norb)
-    handle = blip.blipgpu_create(A, cfg.grid, L, coeffs)
-    hpos = workloads.positions(cfg, rank=rank)                       # every rank: its own walkers
-    M = hpos.shape[0]
-    blip.blipgpu_reserve(handle, M)
-    stream = torch.cuda.current_stream()
-    dpos = torch.from_numpy(hpos).cuda()
-    val = torch.empty((M, ld), dtype=torch.float32, device="cuda")
-    grad = torch.empty((M, 3, ld), dtype=torch.float32, device="cuda") if mode_vgl else None
-    lap = torch.empty((M, ld), dtype=torch.float32, device="cuda") if mode_vgl else None
+    nsm = torch.cuda.get_device_properties(local_rank).multi_processor_count
+    w = Workload(torch, blip, cfg, mode_vgl, rank=rank)          # every rank: a replica and its own walkers
+    M, L, ld, handle, stream = w.M, w.L, w.ld, w.handle, w.stream
 
-    def step():
-        blip.blipgpu_eval(handle, dpos, M, mode, val, grad, lap, ld, None, stream)
-
-    # ---- device-resident timing: W warm-ups, then exactly K steps between two events --------
-    for _ in range(max(args.warmup, 3)):
-        step()
-    barrier()
-    n0 = blip.blipgpu_launch_count(handle)
-    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    # ---- device-resident timing: W warm-ups, then exactly K steps between CUDA events ---------
     flush = needs_l2_flush(cfg, args)
+    for _ in range(max(args.warmup, 3)):
+        w.step()
+    barrier()
     with ClockSampler(local_rank) as clocks:
-        if not flush:
-            e0.record(stream)
-            for _ in range(args.steps):
-                step()
-            e1.record(stream)
-            barrier()
-            ms_total = e0.elapsed_time(e1)
-        else:
-            scratch = torch.empty(512 * 1024 * 1024, dtype=torch.uint8, device="cuda")
-            pairs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True))
-                     for _ in range(args.steps)]
-            for a, b in pairs:
-                scratch.add_(1)                                        # evicts the table and the outputs from L2
-                a.record(stream)
-                step()
-                b.record(stream)
-            barrier()
-            ms_total = sum(a.elapsed_time(b) for a, b in pairs)
-            del scratch
-    launches = blip.blipgpu_launch_count(handle) - n0
+        ms_total, launches = time_steps(torch, w, args.steps, 0, flush, barrier)
     ms_total = max_over_ranks(dist, ms_total, "cuda")
     ms_step = ms_total / args.steps
     evals_step = M * L * world
     value = whole_job_value(M, L, world, ms_step)
 
     # ---- dominant kernel (gather + FMA) timed by the library's own events on the same stream
-    blip.blipgpu_set_profiling(handle, 1)
-    kms, gms = [], []
-    for _ in range(min(args.steps, 20)):
-        step()
-        g_, k_ = blip.blipgpu_last_kernel_ms(handle)
-        gms.append(g_)
-        kms.append(k_)
-    blip.blipgpu_set_profiling(handle, 0)
-    k_ms, g_ms = float(np.mean(kms)), float(np.mean(gms))
-    peak, peak_src, sm_max = measured_peaks()
-    abytes = algorithmic_bytes(M, L, mode_vgl)
-    achieved = abytes / (k_ms * 1e-3) / 1e9
-    fp32_peak = 148 * 128 * 2 * sm_max * 1e6                          # FMA lanes x 2 flop x clock
+    fb = torch.empty(512 * 1024 * 1024, dtype=torch.uint8, device="cuda") if flush else None
+    k_ms, g_ms = kernel_times(w, min(args.steps, 20), fb)
+    del fb
     fp32_meas = blip.blipgpu_probe_fp32(handle, stream) * 1e12        # packed-FMA rate measured in this run
-    # R_compulsory: distinct table rows the batch touches, once, plus the outputs
     cellbuf = torch.empty((M, 3), dtype=torch.int32, device="cuda")
-    blip.blipgpu_eval(handle, dpos, M, mode, val, grad, lap, ld, cellbuf, stream)
+    blip.blipgpu_eval(handle, w.dpos, M, w.mode, w.val, w.grad, w.lap, ld, cellbuf, stream)
     torch.cuda.synchronize()
-    n = torch.tensor(list(cfg.grid), device="cuda", dtype=torch.int64)
-    off = torch.arange(-1, 3, device="cuda", dtype=torch.int64)
-    ci = cellbuf.to(torch.int64)
-    k0 = (ci[:, 0:1] + off) % n[0]
-    k1 = (ci[:, 1:2] + off) % n[1]
-    k2 = (ci[:, 2:3] + off) % n[2]
-    rows = ((k0[:, :, None, None] * n[1] + k1[:, None, :, None]) * n[2] + k2[:, None, None, :]).reshape(-1)
-    distinct_rows = int(torch.unique(rows).numel())
-    del rows, k0, k1, k2, ci, cellbuf
-    comp_bytes = distinct_rows * L * 4 + M * L * (20 if mode_vgl else 4)
-    roofline = {
-        "bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-        "traffic": None,
-        "kernel": {1: "blip::eval_direct_kernel", 2: "blip::eval_staged_kernel", 3: "blip::eval_split_kernel"}.get(
-            blip.blipgpu_last_path(handle), "?") + " (gather + FMA, steps a-2, a-3, a-5)",
-        "kernel_ms": k_ms, "grouping_ms": g_ms, "kernel_share_of_step": k_ms / (k_ms + g_ms),
-        "algorithmic_bytes": abytes, "bytes_per_eval": abytes / (M * L), "peak_source": peak_src,
-        "fp32_fma_frac_of_nominal": 2 * fma_count(M, L, mode_vgl) / (k_ms * 1e-3) / fp32_peak,
-        "fp32_peak_tflops_nominal": fp32_peak / 1e12,
-        "fp32_peak_tflops_measured": fp32_meas / 1e12,
-        "fp32_fma_frac_of_measured": 2 * fma_count(M, L, mode_vgl) / (k_ms * 1e-3) / fp32_meas,
-        "distinct_rows": distinct_rows, "compulsory_bytes": comp_bytes,
-        "compulsory_hbm_frac": comp_bytes / (k_ms * 1e-3) / 1e9 / peak,
-        "note": "contract roofline of BASELINE.json north_star: every gathered coefficient (64 x 4 B) and every "
-                "output byte per evaluation at the measured HBM copy rate.  The staged kernel reads each table "
-                "row from HBM about 3 times instead of once per electron (see traffic), so achieved exceeds the "
-                "HBM peak; what binds it is the shared-memory pipe and the FP32 issue ports (DESIGN.md §6)",
-    }
-    traffic_file = os.path.join(ROOT, "profiles", "traffic.json")     # written from an ncu --set full capture
-    if os.path.exists(traffic_file):
-        try:
-            with open(traffic_file) as fh:
-                tr = json.load(fh)
-            key = f"{cfg.name}:{args.mode}"
-            if key in tr:
-                roofline["traffic"] = tr[key]["dram_bytes_per_launch"]
-                roofline["traffic_source"] = tr[key].get("source")
-        except Exception:
-            pass
+    n_rows = distinct_rows(torch, cellbuf, cfg.grid)
+    del cellbuf
+    roofline = roofline_block(torch, blip, handle, cfg, M, L, mode_vgl, k_ms, g_ms, n_rows, fp32_meas, nsm)
 
     # ---- end to end through the C ABI with HOST buffers (pinned): H2D + eval + D2H per step --
     e2e = None
     if not args.no_e2e:
-        ppos = torch.from_numpy(hpos).pin_memory()
+        ppos = torch.from_numpy(w.hpos).pin_memory()
         pval = torch.empty((M, ld), dtype=torch.float32).pin_memory()
         pgrad = torch.empty((M, 3, ld), dtype=torch.float32).pin_memory() if mode_vgl else None
         plap = torch.empty((M, ld), dtype=torch.float32).pin_memory() if mode_vgl else None
         e2e_steps = max(1, min(args.steps, args.e2e_steps))
         for _ in range(2):
-            blip.blipgpu_eval_host(handle, ppos, M, mode, pval, pgrad, plap, ld, None, stream)
+            blip.blipgpu_eval_host(handle, ppos, M, w.mode, pval, pgrad, plap, ld, None, stream)
         barrier()
         t0 = time.perf_counter()
         for _ in range(e2e_steps):
-            blip.blipgpu_eval_host(handle, ppos, M, mode, pval, pgrad, plap, ld, None, stream)
+            blip.blipgpu_eval_host(handle, ppos, M, w.mode, pval, pgrad, plap, ld, None, stream)
         barrier()
         dt = time.perf_counter() - t0
         dt = max_over_ranks(dist, dt, "cuda")
@@ -377,6 +491,7 @@ def run_gpu(args):
                "d2h_bytes_per_step": int(M * ld * 4 * (5 if mode_vgl else 1)), "steps": e2e_steps,
                "ms_per_step": 1e3 * dt / e2e_steps, "api": "blipgpu_eval_host (pinned host buffers)",
                "checksum": float(pval[0, :L].double().sum())}
+        del ppos, pval, pgrad, plap
 
     line = None
     if rank == 0:
@@ -389,19 +504,47 @@ def run_gpu(args):
             "roofline": roofline,
         }
         if world == 1 and not args.no_cpu_baseline:
-            line["cpu_baseline"] = cpu_baseline(cfg, coeffs, mode_vgl)
-        if args.sweep:
-            line["sweep"] = run_sweep(torch, blip, handle, cfg, dpos, stream)
+            line["cpu_baseline"] = cpu_baseline(cfg, w.coeffs, mode_vgl)
         if mode_vgl and not args.no_contract:
-            line["contract"] = run_contract(torch, blip, handle, cfg, hpos, dpos, stream, args)
-            line["f64"] = run_f64(torch, blip, handle, cfg, dpos, stream)
-    blip.blipgpu_destroy(handle)
+            line["contract"] = run_contract(torch, blip, handle, cfg, w.hpos, w.dpos, stream, args)
+            line["f64"] = run_f64(torch, blip, handle, cfg, w.dpos, stream)
+        if world == 1 and not args.no_configs:
+            # the other BASELINE.json configs (north_star item 4): sweep on this table, then small, tiny, large
+            block = {}
+            if cfg.name == "tio2":
+                block["sweep"] = run_sweep(torch, blip, w)
+                block["sweep_c_caller"] = run_c_harness()
+            w.close()
+            w = None
+            torch.cuda.empty_cache()
+            for name in ("small", "tiny", "large"):
+                if name != cfg.name:
+                    block[name] = measure_config(torch, blip, name, 20 if name != "large" else 10, fp32_meas, nsm)
+            line["configs"] = block
+    if w is not None and getattr(w, "handle", None) is not None:
+        w.close()
     if dist is not None:
         dist.barrier()
         dist.destroy_process_group()
     if line is not None:
         print(json.dumps(line), flush=True)
     return 0
+
+
+def run_c_harness():
+    """Per-call latency of blipgpu_eval from a plain-C caller (tests/harness/blip_harness.c): no
+    Python, ctypes or torch between the caller and the C ABI."""
+    import subprocess
+    try:
+        sys.path.insert(0, os.path.join(ROOT, "tests", "harness"))
+        import build as harness_build
+        exe = harness_build.build()
+        r = subprocess.run([exe, "latency", "300"], capture_output=True, text=True, timeout=600)
+        if r.returncode != 0:
+            return {"error": (r.stderr or r.stdout)[-300:]}
+        return json.loads(r.stdout.strip().splitlines()[-1])
+    except Exception as exc:                                          # the benchmark line must still be printed
+        return {"error": repr(exc)}
 
 
 def run_contract(torch, blip, handle, cfg, hpos, dpos, stream, args):
@@ -463,48 +606,57 @@ def run_f64(torch, blip, handle, cfg, dpos, stream):
     return {"api": "blipgpu_eval_f64", "positions": M, "ms_per_call": ms, "evals_per_s": M * L / (ms * 1e-3), "dtype": "f64"}
 
 
-def run_sweep(torch, blip, handle, cfg, dpos, stream):
-    """BASELINE.json configs[3]: throughput vs batch size M on the resident table, both modes."""
-    L, ld = cfg.norb, (cfg.norb + 3) // 4 * 4
+def run_sweep(torch, blip, w):
+    """BASELINE.json configs[3]: throughput against the batch size M on the resident TiO2-sized
+    table, both modes.  Device time per call from CUDA-graph replays (no host cost in the number):
+      cold  every call of the graph evaluates a different slice of the 49,152-position set, enough
+            slices that the table rows they touch exceed twice the L2 (the paper's particle-by-
+            particle regime: new positions every call, rows come from HBM);
+      warm  the same M positions every call (rows stay in L2) — an upper bound, labelled as such.
+    Per call from the host (Python binding, eager) beside them; tests/harness measures it from C."""
+    cfg, L, ld, stream = w.cfg, w.L, w.ld, w.stream
     out = []
+    pool = w.dpos.shape[0]
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     for mode_name, mode in (("value", blip.VALUE), ("vgl", blip.VGL)):
         for M in workloads.CONFIGS["sweep"].sweep:
-            val = torch.empty((M, ld), dtype=torch.float32, device="cuda")
-            grad = torch.empty((M, 3, ld), dtype=torch.float32, device="cuda")
-            lap = torch.empty((M, ld), dtype=torch.float32, device="cuda")
-            reps = 200
-            for _ in range(10):
-                blip.blipgpu_eval(handle, dpos, M, mode, val, grad, lap, ld, None, stream)
-            torch.cuda.synchronize()
-            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-            e0.record(stream)
-            for _ in range(reps):
-                blip.blipgpu_eval(handle, dpos, M, mode, val, grad, lap, ld, None, stream)
-            e1.record(stream)
-            torch.cuda.synchronize()
-            us = 1e3 * e0.elapsed_time(e1) / reps
-            # the same calls captured once in a CUDA graph and replayed: device time per call
-            # without the host's per-call cost (Python + ctypes + launch)
-            gus = None
-            if M <= 2048:                                    # these calls only launch kernels
+            slots = pool // M
+            # touched rows per call ~ 64 M rows of 3 KB (less what positions share); want > 2 x L2 in total
+            ncold = int(min(slots, max(16, -(-2 * L2_BYTES // (64 * M * L * 4)) + 1)))
+            row = {"M": M, "mode": mode_name, "cold_calls_per_graph": ncold}
+            for label, ncalls, slot_of in (("cold", ncold, lambda i: i % slots), ("warm", 20, lambda i: 0)):
                 side = torch.cuda.Stream()
                 side.wait_stream(stream)
                 graph = torch.cuda.CUDAGraph()
                 with torch.cuda.graph(graph, stream=side):
-                    for _ in range(20):
-                        blip.blipgpu_eval(handle, dpos, M, mode, val, grad, lap, ld, None, side)
+                    for i in range(ncalls):
+                        w.step(M=M, mode=mode, pos=w.dpos[slot_of(i) * M:], stream=side)
                 graph.replay()
                 torch.cuda.synchronize()
+                reps = max(2, 200 // ncalls)
                 e0.record(stream)
-                for _ in range(10):
+                for _ in range(reps):
                     graph.replay()
                 e1.record(stream)
                 torch.cuda.synchronize()
-                gus = 1e3 * e0.elapsed_time(e1) / 200
-            out.append({"M": M, "mode": mode_name, "us_per_call": us, "us_per_call_graph": gus,
-                        "evals_per_s": M * L / (us * 1e-6),
-                        "evals_per_s_graph": None if gus is None else M * L / (gus * 1e-6),
-                        "gathered_GBps": algorithmic_bytes(M, L, mode == blip.VGL) / (us * 1e-6) / 1e9})
+                us = 1e3 * e0.elapsed_time(e1) / (reps * ncalls)
+                row[f"us_per_call_{label}"] = us
+                row[f"evals_per_s_{label}"] = M * L / (us * 1e-6)
+                del graph
+            for i in range(10):
+                w.step(M=M, mode=mode, pos=w.dpos[(i % slots) * M:])
+            torch.cuda.synchronize()
+            e0.record(stream)
+            for i in range(200):
+                w.step(M=M, mode=mode, pos=w.dpos[(i % slots) * M:])
+            e1.record(stream)
+            torch.cuda.synchronize()
+            row["us_per_call_python_eager"] = 1e3 * e0.elapsed_time(e1) / 200
+            row["last_path"] = blip.blipgpu_last_path(w.handle)
+            gb = algorithmic_bytes(M, L, mode == blip.VGL)
+            row["gathered_GBps_cold"] = gb / (row["us_per_call_cold"] * 1e-6) / 1e9
+            row["frac_of_R_gather_cold"] = row["gathered_GBps_cold"] / measured_peaks()[0]
+            out.append(row)
     return out
 
 
@@ -516,12 +668,25 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="tio2", choices=["tiny", "small", "tio2", "large"])
     ap.add_argument("--mode", default="vgl", choices=["vgl", "value"])
-    ap.add_argument("--sweep", action="store_true", help="also time BASELINE configs[3] (M sweep)")
+    ap.add_argument("--no-configs", action="store_true",
+                    help="skip the `configs` block (batch sweep, small, tiny, large)")
     ap.add_argument("--e2e-steps", type=int, default=10)
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-contract", action="store_true", help="skip the blipgpu_eval_contract timing")
     args = ap.parse_args()
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    if args.gpus != world:
+        if "RANK" in os.environ or args.gpus < 1:
+            raise SystemExit(f"bench.py: --gpus {args.gpus} but WORLD_SIZE is {world}")
+        # run bare with --gpus N > 1: become the torchrun launch the contract describes
+        import socket
+        with socket.socket() as sk:
+            sk.bind(("127.0.0.1", 0))
+            port = sk.getsockname()[1]
+        os.execv(sys.executable, [sys.executable, "-m", "torch.distributed.run", "--nnodes=1",
+                                  f"--nproc-per-node={args.gpus}", "--master-addr", "127.0.0.1",
+                                  "--master-port", str(port), os.path.abspath(__file__), *sys.argv[1:]])
     if args.impl == "reference":
         return run_reference(args)
     return run_gpu(args)
