@@ -202,7 +202,7 @@ def workload_config(cfg, args, n_positions=None):
     return {
         "workload": f"{cfg.name}: BASELINE.json configs[{list(workloads.CONFIGS).index(cfg.name)}]",
         "lattice_bohr": [list(r) for r in cfg.lattice], "grid": list(cfg.grid), "orbitals": cfg.norb,
-        "positions_per_step": int(cfg.M if n_positions is None else n_positions),
+        "positions_per_step": int((getattr(args, "positions", 0) or cfg.M) if n_positions is None else n_positions),
         "electrons": cfg.electrons, "walkers": cfg.walkers, "clustered_20pct": bool(cfg.clustered),
         "mode": "value+grad+lap" if args.mode == "vgl" else "value",
         "table_bytes": cfg.table_bytes, "parallelism": f"walkers x{args.gpus} (table replicated, no collective)",
@@ -216,10 +216,12 @@ L2_BYTES = 126 * 1024 * 1024
 
 
 def needs_l2_flush(cfg, args):
-    """Working set of one step: the table plus the outputs.  Below ~2x L2 a repeat of the step would
-    find its data cached, so the timed loop flushes L2 between steps (timing rules of the task)."""
-    out_bytes = cfg.M * cfg.norb * 4 * (5 if args.mode == "vgl" else 1)
-    return cfg.table_bytes + out_bytes < 2 * L2_BYTES
+    """Working set of one step: the table rows the batch can touch plus the outputs.  Below ~2x L2 a
+    repeat of the step would find its data cached, so the timed loop flushes L2 between steps
+    (timing rules of the task)."""
+    M = getattr(args, "positions", 0) or cfg.M
+    out_bytes = M * cfg.norb * 4 * (5 if args.mode == "vgl" else 1)
+    return min(cfg.table_bytes, 64 * M * cfg.norb * 4) + out_bytes < 2 * L2_BYTES
 
 
 # ---------------------------------------------------------------------------------------------
@@ -443,7 +445,7 @@ def run_gpu(args):
     cfg = workloads.CONFIGS[args.workload]
     mode_vgl = args.mode == "vgl"
     nsm = torch.cuda.get_device_properties(local_rank).multi_processor_count
-    w = Workload(torch, blip, cfg, mode_vgl, rank=rank)          # every rank: a replica and its own walkers
+    w = Workload(torch, blip, cfg, mode_vgl, rank=rank, M=args.positions or None)   # every rank: a replica and its own walkers
     M, L, ld, handle, stream = w.M, w.L, w.ld, w.handle, w.stream
 
     # ---- device-resident timing: W warm-ups, then exactly K steps between CUDA events ---------
@@ -670,6 +672,8 @@ def main():
     ap.add_argument("--mode", default="vgl", choices=["vgl", "value"])
     ap.add_argument("--no-configs", action="store_true",
                     help="skip the `configs` block (batch sweep, small, tiny, large)")
+    ap.add_argument("--positions", type=int, default=0,
+                    help="evaluate only the first M positions of the workload (a row of the batch sweep, configs[3])")
     ap.add_argument("--e2e-steps", type=int, default=10)
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")

@@ -29,6 +29,8 @@ def lib():
         L.blip_oracle_eval.argtypes = [dp, ip, ctypes.c_int, fp, dp, ctypes.c_longlong,
                                        ctypes.c_int, dp, dp, dp, ip]
         L.blip_oracle_eval.restype = ctypes.c_int
+        L.blip_oracle_eval_hess.argtypes = [dp, ip, ctypes.c_int, fp, dp, ctypes.c_longlong, dp, dp, dp, ip]
+        L.blip_oracle_eval_hess.restype = ctypes.c_int
         L.blip_oracle_spacing.argtypes = [dp, ip, dp]
         L.blip_oracle_spacing.restype = ctypes.c_int
         L.blip_oracle_num_threads.restype = ctypes.c_int
@@ -93,6 +95,69 @@ def eval_fast(lattice, grid, coeffs, positions, mode=VGL):
     if rc:
         raise ValueError(f"blip_oracle_eval failed with code {rc}")
     return val, grad, lap, cell
+
+
+HESS_COMPONENTS = ((0, 0), (1, 1), (2, 2), (0, 1), (0, 2), (1, 2))     # xx yy zz xy xz yz
+
+
+def eval_hess(lattice, grid, coeffs, positions):
+    """Value, Cartesian gradient and full Cartesian Hessian (blip_oracle_eval_hess): returns
+    (val [M][L], grad [M][3][L], hess [M][6][L] in the order xx yy zz xy xz yz, cell [M][3]), fp64."""
+    A, n = _prep(lattice, grid)
+    c = np.ascontiguousarray(coeffs, dtype=np.float32)
+    assert c.ndim == 4 and tuple(c.shape[:3]) == tuple(int(x) for x in n), c.shape
+    L = c.shape[3]
+    pos = np.ascontiguousarray(np.asarray(positions, dtype=np.float64).reshape(-1, 3))
+    M = pos.shape[0]
+    val = np.empty((M, L), dtype=np.float64)
+    grad = np.empty((M, 3, L), dtype=np.float64)
+    hess = np.empty((M, 6, L), dtype=np.float64)
+    cell = np.empty((M, 3), dtype=np.int32)
+    rc = lib().blip_oracle_eval_hess(_d(A), _i(n), L, c.ctypes.data_as(ctypes.POINTER(ctypes.c_float)),
+                                     _d(pos), M, _d(val), _d(grad), _d(hess), _i(cell))
+    if rc:
+        raise ValueError(f"blip_oracle_eval_hess failed with code {rc}")
+    return val, grad, hess, cell
+
+
+def bloch(val, grad, lap, kpoints, positions):
+    """Complex orbitals with a per-orbital Bloch phase (the paper's orbitals
+    are complex, "2 components in complex numbers").  Complex orbital m is made of the
+    real channels (2m, 2m+1) of the table — u_m = S_{2m} + i S_{2m+1}, periodic in the cell — times
+    the phase of its k-point [DESIGN.md reading R8a; the paper does not write the phase out]:
+
+        psi_m(r)       = exp(i k_m . r) u_m(r)
+        grad psi_m     = exp(i k_m . r) (grad u_m + i k_m u_m)                          (product rule)
+        laplace psi_m  = exp(i k_m . r) (laplace u_m + 2 i k_m . grad u_m - |k_m|^2 u_m)
+
+    val [M][L], grad [M][3][L], lap [M][L]: oracle results (fp64) for the real channels, L even;
+    kpoints [L/2][3] Cartesian (rad / bohr); positions [M][3] Cartesian.  grad / lap may be None.
+    Returns complex128 (psi [M][L/2], gpsi [M][3][L/2] or None, lpsi [M][L/2] or None).
+    Pins (tests/test_oracle_pins.py): k = 0 returns the real channels; |psi|^2 does not depend on k;
+    a constant table gives a plane wave (grad = i k psi, laplace = -|k|^2 psi); central differences
+    of psi VALUES; psi(r + a_j) = exp(i k . a_j) psi(r)."""
+    val = np.asarray(val, dtype=np.float64)
+    k = np.asarray(kpoints, dtype=np.float64).reshape(-1, 3)
+    r = np.asarray(positions, dtype=np.float64).reshape(-1, 3)
+    M, L = val.shape
+    assert L % 2 == 0 and k.shape[0] == L // 2 and r.shape[0] == M
+    Lc = L // 2
+    psi = np.empty((M, Lc), dtype=np.complex128)
+    gpsi = None if grad is None else np.empty((M, 3, Lc), dtype=np.complex128)
+    lpsi = None if lap is None else np.empty((M, Lc), dtype=np.complex128)
+    for m in range(Lc):
+        theta = r[:, 0] * k[m, 0] + r[:, 1] * k[m, 1] + r[:, 2] * k[m, 2]
+        phase = np.cos(theta) + 1j * np.sin(theta)
+        u = val[:, 2 * m] + 1j * val[:, 2 * m + 1]
+        psi[:, m] = phase * u
+        if grad is not None:
+            gu = grad[:, :, 2 * m] + 1j * grad[:, :, 2 * m + 1]                 # [M][3]
+            gpsi[:, :, m] = phase[:, None] * (gu + 1j * k[m][None, :] * u[:, None])
+            if lap is not None:
+                lu = lap[:, 2 * m] + 1j * lap[:, 2 * m + 1]
+                kg = gu[:, 0] * k[m, 0] + gu[:, 1] * k[m, 1] + gu[:, 2] * k[m, 2]
+                lpsi[:, m] = phase * (lu + 2j * kg - (k[m] @ k[m]) * u)
+    return psi, gpsi, lpsi
 
 
 def spacing(lattice, grid):

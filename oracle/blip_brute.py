@@ -51,8 +51,9 @@ def _periodic(fn, t, n, images):
     return out
 
 
-def eval_brute(lattice, grid, coeffs, positions, images=2):
-    """Returns (val [M][L], grad [M][3][L], lap [M][L]) in fp64 — sum over all n1*n2*n3 sites."""
+def eval_brute(lattice, grid, coeffs, positions, images=2, want_hessian=False):
+    """Returns (val [M][L], grad [M][3][L], lap [M][L]) in fp64 — sum over all n1*n2*n3 sites;
+    with want_hessian also the Cartesian Hessian [M][3][3][L] as a fourth entry."""
     A = np.asarray(lattice, dtype=np.float64).reshape(3, 3)
     n = [int(x) for x in grid]
     c = np.asarray(coeffs, dtype=np.float64)
@@ -66,6 +67,7 @@ def eval_brute(lattice, grid, coeffs, positions, images=2):
     val = np.zeros((M, L))
     grad = np.zeros((M, 3, L))
     lap = np.zeros((M, L))
+    hess = np.zeros((M, 3, 3, L))
     for e in range(M):
         t = (pos[e] @ Ainv) * np.array(n, dtype=np.float64)
         b = [_periodic(B, t[a], n[a], images) for a in range(3)]
@@ -89,4 +91,7 @@ def eval_brute(lattice, grid, coeffs, positions, images=2):
         grad[e] = Jm.T @ dt                                   # grad_i = sum_a J[a][i] dS/dt_a
         Hc = np.einsum("ai,abl,bj->ijl", Jm, Ht, Jm)          # Cartesian Hessian
         lap[e] = Hc[0, 0] + Hc[1, 1] + Hc[2, 2]
+        hess[e] = Hc
+    if want_hessian:
+        return val, grad, lap, hess
     return val, grad, lap

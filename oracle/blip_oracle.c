@@ -34,7 +34,8 @@
  * discrete cosine eigenfunction, lattice periodicity, central finite differences of oracle
  * VALUES for gradient and Laplacian (orthorhombic and triclinic), continuity across cell
  * faces, separable case against scipy.interpolate.BSpline, adversarial cell-index inputs.
- * No function here is "parity unpinned".
+ * blip_oracle_eval_hess (full Cartesian Hessian, added in round 2) has its own pins, listed at
+ * the function.  No function here is "parity unpinned".
  *
  * Build: gcc -O2 -ffp-contract=off -fopenmp -fPIC -shared (oracle/build.py).  The
  * -ffp-contract=off matters only for the index map (step 1), whose IEEE sequence is pinned
@@ -248,6 +249,106 @@ int blip_oracle_eval(const double A[9], const int n[3], int L, const float *c,
                             J[0][x] * T0[l] + J[1][x] * T1[l] + J[2][x] * T2[l];
                     lap[e * L + l] = Q[0][0] * H00[l] + Q[1][1] * H11[l] + Q[2][2] * H22[l]
                                    + 2.0 * (Q[0][1] * H01[l] + Q[0][2] * H02[l] + Q[1][2] * H12[l]);
+                }
+            }
+        }
+        free(acc);
+    }
+    return failed ? -3 : 0;
+}
+
+/* ---------------------------------------------------------------------------------------
+ * Value, Cartesian gradient and the full Cartesian HESSIAN (the paper's
+ * local-energy call needs second derivatives).  Same steps 1-3 as
+ * blip_oracle_eval — the 64-term sum of Eq. 6 for S, dS/dt_a and d2S/dt_a dt_b in grid
+ * coordinates — and in step 4 the chain rule for second derivatives of a function of
+ * t(r) = J r (J constant, so no first-derivative term appears):
+ *      Hc[i][j] = d2S/dr_i dr_j = sum_ab J[a][i] Ht[a][b] J[b][j]
+ *   hess   [M][6][L]  fp64 out, components in the order xx, yy, zz, xy, xz, yz
+ * Returns as blip_oracle_eval.  Pins (tests/test_oracle_pins.py): trace = the Laplacian of
+ * blip_oracle_eval; bilinear / quadratic tables (Hc = J_a^T J_b + J_b^T J_a); central
+ * differences of oracle GRADIENTS; the brute-force definition (oracle/blip_brute.py).
+ * ------------------------------------------------------------------------------------- */
+int blip_oracle_eval_hess(const double A[9], const int n[3], int L, const float *c,
+                          const double *pos, long long M,
+                          double *val, double *grad, double *hess, int *cell)
+{
+    if (L < 1 || M < 0 || n[0] < 4 || n[1] < 4 || n[2] < 4 || !c || !val || !grad || !hess) return -2;
+    double G[9];
+    if (blip_oracle_inverse_lattice(A, G)) return -1;
+    double J[3][3];
+    for (int a = 0; a < 3; ++a)
+        for (int i = 0; i < 3; ++i)
+            J[a][i] = (double)n[a] * G[3 * i + a];
+    static const int ci[6] = {0, 1, 2, 0, 0, 1}, cj[6] = {0, 1, 2, 1, 2, 2};   /* xx yy zz xy xz yz */
+
+    int failed = 0;
+#pragma omp parallel
+    {
+        double *acc = (double *)malloc(sizeof(double) * 10 * (size_t)L);
+        if (!acc) {
+#pragma omp atomic write
+            failed = 1;
+        }
+#pragma omp for schedule(dynamic, 16)
+        for (long long e = 0; e < M; ++e) {
+            if (!acc) continue;
+            int i[3]; double f[3];
+            int bad = cell_of(G, n, pos + 3 * e, i, f);
+            if (cell) { cell[3 * e] = i[0]; cell[3 * e + 1] = i[1]; cell[3 * e + 2] = i[2]; }
+            if (bad) {
+                for (int l = 0; l < L; ++l) {
+                    val[e * L + l] = NAN;
+                    for (int x = 0; x < 3; ++x) grad[(e * 3 + x) * L + l] = NAN;
+                    for (int q = 0; q < 6; ++q) hess[(e * 6 + q) * L + l] = NAN;
+                }
+                continue;
+            }
+            double w[3][4], d1[3][4], d2[3][4];
+            for (int a = 0; a < 3; ++a) phi_weights(f[a], w[a], d1[a], d2[a]);
+            double *S = acc;
+            double *T[3] = {acc + L, acc + 2 * L, acc + 3 * L};
+            double *H[3][3];
+            H[0][0] = acc + 4 * L; H[1][1] = acc + 5 * L; H[2][2] = acc + 6 * L;
+            H[0][1] = H[1][0] = acc + 7 * L; H[0][2] = H[2][0] = acc + 8 * L; H[1][2] = H[2][1] = acc + 9 * L;
+            memset(acc, 0, sizeof(double) * 10 * (size_t)L);
+            for (int m0 = 0; m0 < 4; ++m0) {
+                int k0 = ((i[0] - 1 + m0) % n[0] + n[0]) % n[0];
+                for (int m1 = 0; m1 < 4; ++m1) {
+                    int k1 = ((i[1] - 1 + m1) % n[1] + n[1]) % n[1];
+                    for (int m2 = 0; m2 < 4; ++m2) {
+                        int k2 = ((i[2] - 1 + m2) % n[2] + n[2]) % n[2];
+                        const float *row = c + (((size_t)k0 * n[1] + k1) * n[2] + k2) * (size_t)L;
+                        double th = w[0][m0] * w[1][m1] * w[2][m2];
+                        double t0 = d1[0][m0] * w[1][m1] * w[2][m2];
+                        double t1 = w[0][m0] * d1[1][m1] * w[2][m2];
+                        double t2 = w[0][m0] * w[1][m1] * d1[2][m2];
+                        double h00 = d2[0][m0] * w[1][m1] * w[2][m2];
+                        double h11 = w[0][m0] * d2[1][m1] * w[2][m2];
+                        double h22 = w[0][m0] * w[1][m1] * d2[2][m2];
+                        double h01 = d1[0][m0] * d1[1][m1] * w[2][m2];
+                        double h02 = d1[0][m0] * w[1][m1] * d1[2][m2];
+                        double h12 = w[0][m0] * d1[1][m1] * d1[2][m2];
+                        for (int l = 0; l < L; ++l) {
+                            double a = (double)row[l];
+                            S[l] += th * a;
+                            T[0][l] += t0 * a; T[1][l] += t1 * a; T[2][l] += t2 * a;
+                            H[0][0][l] += h00 * a; H[1][1][l] += h11 * a; H[2][2][l] += h22 * a;
+                            H[0][1][l] += h01 * a; H[0][2][l] += h02 * a; H[1][2][l] += h12 * a;
+                        }
+                    }
+                }
+            }
+            for (int l = 0; l < L; ++l) {
+                val[e * L + l] = S[l];
+                for (int x = 0; x < 3; ++x)
+                    grad[(e * 3 + x) * L + l] = J[0][x] * T[0][l] + J[1][x] * T[1][l] + J[2][x] * T[2][l];
+                for (int q = 0; q < 6; ++q) {
+                    double s = 0.0;
+                    for (int a = 0; a < 3; ++a)
+                        for (int b = 0; b < 3; ++b)
+                            s += J[a][ci[q]] * H[a][b][l] * J[b][cj[q]];
+                    hess[(e * 6 + q) * L + l] = s;
                 }
             }
         }

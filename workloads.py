@@ -128,3 +128,13 @@ def contraction_vectors(M, norb, seed=4):
     (the paper's matrices are not available)."""
     rng = np.random.default_rng(seed)
     return (rng.standard_normal((int(M), int(norb)), dtype=np.float32) / np.float32(np.sqrt(norb)))
+
+
+def kpoints(lattice_rows, n_complex, seed=5):
+    """Cartesian k-points [n_complex][3] (rad / bohr) for the complex-orbital API: a twist
+    q ~ U[-1/2, 1/2)^3 per orbital in units of the reciprocal lattice, k = 2 pi q . (A^-1)^T, i.e.
+    anywhere in the first Brillouin zone of the simulation cell (the paper's orbitals are complex,
+    PAPER.md:355; its k-points are not given)."""
+    A = np.array(lattice_rows, dtype=np.float64).reshape(3, 3)
+    q = np.random.default_rng(seed).random((int(n_complex), 3)) - 0.5
+    return np.ascontiguousarray(2.0 * np.pi * q @ np.linalg.inv(A).T)
