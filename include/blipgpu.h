@@ -40,6 +40,7 @@ typedef struct blipgpu_table blipgpu_table;       /* opaque handle: table + work
 /* mode */
 #define BLIPGPU_VALUE 0                           /* psi only                              */
 #define BLIPGPU_VGL   1                           /* psi, Cartesian gradient, Laplacian    */
+#define BLIPGPU_VGH   2                           /* psi, Cartesian gradient, Cartesian Hessian (6 components) */
 
 /* return codes */
 #define BLIPGPU_OK       0
@@ -78,10 +79,13 @@ int blipgpu_create(const double* lattice, const int* grid, int norb, const float
  *
  *   positions DEVICE [M][3] fp64 Cartesian (bohr); any finite value (wrapped into the cell)
  *   M               >= 0; M == 0 returns OK without launching anything
- *   mode            BLIPGPU_VALUE or BLIPGPU_VGL
- *   val       DEVICE [M][ld]      fp32 out, required            val[j][l]     = psi_l(r_j)
- *   grad      DEVICE [M][3][ld]   fp32 out, required iff VGL    grad[j][i][l] = d psi_l / d r_i
- *   lap       DEVICE [M][ld]      fp32 out, required iff VGL    lap[j][l]     = nabla^2 psi_l
+ *   mode            BLIPGPU_VALUE, BLIPGPU_VGL or BLIPGPU_VGH
+ *   val       DEVICE [M][ld]      fp32 out, required               val[j][l]     = psi_l(r_j)
+ *   grad      DEVICE [M][3][ld]   fp32 out, required iff VGL / VGH grad[j][i][l] = d psi_l / d r_i
+ *   lap       DEVICE [M][ld]      fp32 out, required iff VGL       lap[j][l]     = nabla^2 psi_l
+ *             DEVICE [M][6][ld]   fp32 out, required iff VGH       lap[j][q][l]  = d2 psi_l / d r_a d r_b,
+ *                                 q = 0..5 <-> (a,b) = xx, yy, zz, xy, xz, yz (the local-energy call's
+ *                                 second derivatives; its trace is the Laplacian)
  *   ld              row pitch in floats: ld >= L and ld % 4 == 0.  Columns L..ld-1 are
  *                   padding; up to the next multiple of 4 they may be overwritten
  *   cell      DEVICE [M][3] int32 out, optional (NULL ok): floor(t_a) in [0,n_a) of step a-1
@@ -95,6 +99,8 @@ int blipgpu_create(const double* lattice, const int* grid, int norb, const float
  * The call keeps no state on the host between calls and leaves its device workspace as it
  * found it, so once the workspace is reserved it may be captured in a CUDA graph and
  * replayed.
+ * VGH runs the per-position kernel of blipgpu_eval_f64 in fp32 (no grouping): it is meant for
+ * the occasional local-energy call, not for the per-move batch.
  * Errors: EINVAL (NULL required pointer, M < 0, unknown mode, bad ld, misaligned output),
  * ENOMEM, ECUDA.
  */
@@ -150,8 +156,9 @@ int blipgpu_eval_contract(blipgpu_table* t, const double* positions, long long M
  * to rounding (~1e-14 relative to max|c| x weights).  It is the accuracy path, not the fast
  * one: one CTA per (position, 128 orbitals), no grouping, about 1/2 the FMA rate.
  *
- *   positions DEVICE [M][3] fp64;  mode BLIPGPU_VALUE or BLIPGPU_VGL
- *   val  DEVICE [M][ld] fp64;  grad DEVICE [M][3][ld] fp64;  lap DEVICE [M][ld] fp64 (VGL only)
+ *   positions DEVICE [M][3] fp64;  mode BLIPGPU_VALUE, BLIPGPU_VGL or BLIPGPU_VGH
+ *   val  DEVICE [M][ld] fp64;  grad DEVICE [M][3][ld] fp64 (VGL, VGH);
+ *   lap  DEVICE [M][ld] fp64 (VGL) or [M][6][ld] fp64 (VGH: Hessian xx, yy, zz, xy, xz, yz)
  *   ld   row pitch in doubles, >= L, multiple of 4; outputs 16-byte aligned
  *   cell DEVICE [M][3] int32, optional
  *
@@ -160,6 +167,32 @@ int blipgpu_eval_contract(blipgpu_table* t, const double* positions, long long M
  */
 int blipgpu_eval_f64(blipgpu_table* t, const double* positions, long long M, int mode,
                      double* val, double* grad, double* lap, long long ld, int* cell, void* stream);
+
+/*
+ * blipgpu_set_kpoints / blipgpu_eval_complex — complex orbitals with a per-orbital Bloch phase.
+ * The paper's coefficients are complex ("2 components in complex numbers"); the
+ * table holds complex orbital m as the two adjacent real channels (2m, 2m+1), so that
+ * u_m(r) = S_2m(r) + i S_2m+1(r) is periodic in the cell, and the orbital itself is
+ *
+ *     psi_m(r) = exp(i k_m . r) u_m(r),      m = 0 .. L/2 - 1
+ *
+ * with k_m the k-point (twist) of orbital m [the paper does not write the phase out; DESIGN.md
+ * reading R8a].  blipgpu_eval_complex returns psi_m, its Cartesian gradient and Laplacian
+ *     grad psi_m = e^{i k.r} (grad u_m + i k_m u_m),
+ *     lap  psi_m = e^{i k.r} (lap u_m + 2 i k_m . grad u_m - |k_m|^2 u_m)
+ * as interleaved (re, im) fp32 in the places of the two real channels: val[j][2m] = Re psi_m(r_j),
+ * val[j][2m+1] = Im psi_m(r_j), likewise grad and lap — i.e. `val` viewed as complex64 is
+ * [M][ld/2].  It is the same pass as blipgpu_eval (same kernels, same grouping); the phase is an
+ * epilogue on the accumulators, k.r taken in fp64 and reduced mod 2 pi before it is rounded.
+ *
+ *   blipgpu_set_kpoints   kpoints HOST [L/2][3] fp64, Cartesian, rad / bohr; copied (synchronous);
+ *                         NULL drops them.  EINVAL if L is odd or a component is not finite.
+ *   blipgpu_eval_complex  arguments as blipgpu_eval; mode BLIPGPU_VALUE or BLIPGPU_VGL;
+ *                         EINVAL also if no k-points are set.
+ */
+int blipgpu_set_kpoints(blipgpu_table* t, const double* kpoints);
+int blipgpu_eval_complex(blipgpu_table* t, const double* positions, long long M, int mode,
+                         float* val, float* grad, float* lap, long long ld, int* cell, void* stream);
 
 /* blipgpu_reserve — pre-size the grouping workspace (bins, permutation, per-electron records)
  * for batches of up to M_max positions, so that blipgpu_eval never has to grow it (growing

@@ -1,4 +1,5 @@
-"""paper_1204_1121_b200 — thin Python binding of the blipgpu C ABI (include/blipgpu.h).
+"""paper_1204_1121_b200 — thin Python binding of the blipgpu C ABI (include/blipgpu.h, plus the
+test / benchmark instrumentation of include/blipgpu_dev.h).
 
 Argument marshalling only: every step of the hot path (cell map, B-spline weights, 64-row
 gather + FMA, grouping, output; Eq. 6-8) runs in the sm_100a kernels of
@@ -12,7 +13,7 @@ import numpy as np
 
 from . import _build
 
-VALUE, VGL = 0, 1
+VALUE, VGL, VGH = 0, 1, 2
 OK, EINVAL, ENOMEM, ECUDA, EARCH = 0, -1, -2, -3, -4
 
 _lib = None
@@ -37,6 +38,10 @@ SIGNATURES = {
     "blipgpu_eval_f64": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_void_p, ctypes.c_longlong, ctypes.c_int,
                                         ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p,
                                         ctypes.c_longlong, ctypes.c_void_p, ctypes.c_void_p]),
+    "blipgpu_set_kpoints": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_void_p]),
+    "blipgpu_eval_complex": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_void_p, ctypes.c_longlong, ctypes.c_int,
+                                            ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p,
+                                            ctypes.c_longlong, ctypes.c_void_p, ctypes.c_void_p]),
     "blipgpu_reserve": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_longlong]),
     "blipgpu_destroy": (ctypes.c_int, [ctypes.c_void_p]),
     "blipgpu_info": (ctypes.c_int, [ctypes.c_void_p, _c_ip, _c_ip, _c_llp, _c_llp]),
@@ -139,6 +144,23 @@ def blipgpu_eval_f64(handle, positions, M, mode, val, grad, lap, ld, cell=None, 
     _check(rc, "blipgpu_eval_f64", handle)
 
 
+def blipgpu_set_kpoints(handle, kpoints):
+    """kpoints: [L/2][3] Cartesian k-points (rad / bohr) of the complex orbitals, or None to drop them."""
+    if kpoints is None:
+        _check(lib().blipgpu_set_kpoints(handle, ctypes.c_void_p(0)), "blipgpu_set_kpoints", handle)
+        return
+    k = np.ascontiguousarray(np.asarray(kpoints, dtype=np.float64).reshape(-1, 3))
+    info = blipgpu_info(handle)
+    assert k.shape[0] * 2 == info["norb"], "one k-point per complex orbital (pair of real channels)"
+    _check(lib().blipgpu_set_kpoints(handle, _ptr(k)), "blipgpu_set_kpoints", handle)
+
+
+def blipgpu_eval_complex(handle, positions, M, mode, val, grad, lap, ld, cell=None, stream=None):
+    rc = lib().blipgpu_eval_complex(handle, _ptr(positions), int(M), int(mode), _ptr(val), _ptr(grad), _ptr(lap),
+                                    int(ld), _ptr(cell), _stream_ptr(stream))
+    _check(rc, "blipgpu_eval_complex", handle)
+
+
 def blipgpu_reserve(handle, M_max):
     _check(lib().blipgpu_reserve(handle, int(M_max)), "blipgpu_reserve", handle)
 
@@ -203,13 +225,17 @@ class BlipTable:
         M = positions.shape[0]
         dev = positions.device
         val = torch.empty((M, self.ld), dtype=torch.float32, device=dev)
-        grad = torch.empty((M, 3, self.ld), dtype=torch.float32, device=dev) if mode == VGL else None
-        lap = torch.empty((M, self.ld), dtype=torch.float32, device=dev) if mode == VGL else None
+        grad = torch.empty((M, 3, self.ld), dtype=torch.float32, device=dev) if mode != VALUE else None
+        lap = None
+        if mode == VGL:
+            lap = torch.empty((M, self.ld), dtype=torch.float32, device=dev)
+        elif mode == VGH:
+            lap = torch.empty((M, 6, self.ld), dtype=torch.float32, device=dev)      # Hessian xx yy zz xy xz yz
         cell = torch.empty((M, 3), dtype=torch.int32, device=dev) if want_cell else None
         blipgpu_eval(self.handle, positions, M, mode, val, grad, lap, self.ld, cell, stream)
         L = self.norb
         return (val[:, :L], grad[:, :, :L] if grad is not None else None,
-                lap[:, :L] if lap is not None else None, cell)
+                lap[..., :L] if lap is not None else None, cell)
 
     def launch_count(self):
         return blipgpu_launch_count(self.handle)

@@ -539,6 +539,80 @@ __device__ __forceinline__ void store_pairs(const Geom& g, const PairAcc (&acc)[
     }
 }
 
+// a-5 for complex orbitals with a Bloch phase (the paper's orbitals are
+// complex): real channels (2m, 2m+1) form u_m = S_2m + i S_2m+1 and the output is
+//     psi_m = e^{i k_m.r} u_m,   grad psi_m = e^{i k_m.r} (grad u_m + i k_m u_m),
+//     laplace psi_m = e^{i k_m.r} (laplace u_m + 2 i k_m.grad u_m - |k_m|^2 u_m)
+// stored as interleaved (re, im) fp32 in the places of the two real channels.  A lane's 4
+// orbitals are 2 complex ones (acc[0], acc[1]); the phase k.r is taken in fp64, brought to
+// (-1, 1] half-turns exactly, and only then rounded to fp32 for sincospi, so its error does not
+// grow with |k.r| (reading R8a).  Once per electron x complex orbital.
+__device__ __forceinline__ void bloch_phase(const double* __restrict__ pos, const double* __restrict__ kvec, int e, int m,
+                                            int ncomplex, float& c, float& s, float (&kf)[3], float& k2)
+{
+    double k0 = 0.0, k1 = 0.0, k2d = 0.0;
+    if (m < ncomplex) { k0 = __ldg(kvec + 3 * (size_t)m); k1 = __ldg(kvec + 3 * (size_t)m + 1); k2d = __ldg(kvec + 3 * (size_t)m + 2); }
+    const double x = __ldg(pos + 3 * (size_t)e), y = __ldg(pos + 3 * (size_t)e + 1), z = __ldg(pos + 3 * (size_t)e + 2);
+    const double theta = fma(k2d, z, fma(k1, y, k0 * x));
+    double t = theta * 0.31830988618379067154;              // half-turns: theta / pi
+    t = fma(-2.0, rint(0.5 * t), t);                         // exact: t in [-1, 1]
+    sincospif((float)t, &s, &c);
+    kf[0] = (float)k0; kf[1] = (float)k1; kf[2] = (float)k2d;
+    k2 = (float)fma(k2d, k2d, fma(k1, k1, k0 * k0));
+}
+
+template <int MODE>
+__device__ __forceinline__ void store_pairs_complex(const Geom& g, const PairAcc (&acc)[2], int e, int col0,
+                                                    const double* __restrict__ pos, const double* __restrict__ kvec,
+                                                    float* __restrict__ val, float* __restrict__ grad,
+                                                    float* __restrict__ lap, long long ld)
+{
+    float v[4], gx[4], gy[4], gz[4], lp[4];
+#pragma unroll
+    for (int p = 0; p < 2; ++p) {
+        float c, s, k[3], k2;
+        bloch_phase(pos, kvec, e, (col0 >> 1) + p, g.L >> 1, c, s, k, k2);
+        const float2 u = unpack2(acc[p].val);                // u = u.x + i u.y
+        v[2 * p] = __fmaf_rn(c, u.x, -__fmul_rn(s, u.y));
+        v[2 * p + 1] = __fmaf_rn(s, u.x, __fmul_rn(c, u.y));
+        if (MODE != 0) {
+            const float2 a = unpack2(acc[p].t1), b = unpack2(acc[p].t2), d = unpack2(acc[p].t3), l = unpack2(acc[p].lp);
+            float gr[3], gi[3];                              // Cartesian gradient of u: real and imaginary channel
+            if (MODE == 2) {
+                gr[0] = a.x; gr[1] = b.x; gr[2] = d.x; gi[0] = a.y; gi[1] = b.y; gi[2] = d.y;
+            } else {
+#pragma unroll
+                for (int i = 0; i < 3; ++i) {
+                    gr[i] = __fmaf_rn(g.J[i], a.x, __fmaf_rn(g.J[3 + i], b.x, __fmul_rn(g.J[6 + i], d.x)));
+                    gi[i] = __fmaf_rn(g.J[i], a.y, __fmaf_rn(g.J[3 + i], b.y, __fmul_rn(g.J[6 + i], d.y)));
+                }
+            }
+            float* const out[3] = {gx, gy, gz};
+#pragma unroll
+            for (int i = 0; i < 3; ++i) {                    // grad u + i k u
+                const float re = __fmaf_rn(-k[i], u.y, gr[i]), im = __fmaf_rn(k[i], u.x, gi[i]);
+                out[i][2 * p] = __fmaf_rn(c, re, -__fmul_rn(s, im));
+                out[i][2 * p + 1] = __fmaf_rn(s, re, __fmul_rn(c, im));
+            }
+            const float kgr = __fmaf_rn(k[0], gr[0], __fmaf_rn(k[1], gr[1], __fmul_rn(k[2], gr[2])));
+            const float kgi = __fmaf_rn(k[0], gi[0], __fmaf_rn(k[1], gi[1], __fmul_rn(k[2], gi[2])));
+            const float re = __fmaf_rn(-k2, u.x, __fmaf_rn(-2.0f, kgi, l.x));      // laplace u + 2 i k.grad u - k^2 u
+            const float im = __fmaf_rn(-k2, u.y, __fmaf_rn(2.0f, kgr, l.y));
+            lp[2 * p] = __fmaf_rn(c, re, -__fmul_rn(s, im));
+            lp[2 * p + 1] = __fmaf_rn(s, re, __fmul_rn(c, im));
+        }
+    }
+    const size_t o = (size_t)e * (size_t)ld + (size_t)col0;
+    const size_t og = (size_t)e * 3 * (size_t)ld + (size_t)col0;
+    st_stream4(val + o, v[0], v[1], v[2], v[3]);
+    if (MODE != 0) {
+        st_stream4(grad + og, gx[0], gx[1], gx[2], gx[3]);
+        st_stream4(grad + og + ld, gy[0], gy[1], gy[2], gy[3]);
+        st_stream4(grad + og + 2 * ld, gz[0], gz[1], gz[2], gz[3]);
+        st_stream4(lap + o, lp[0], lp[1], lp[2], lp[3]);
+    }
+}
+
 // Contraction epilogue (§VI.D, Eq. 11): instead of
 // storing the orbitals of electron e, contract them with the caller's vector d_e (column of
 // the inverse Slater matrix in the paper's use):
@@ -664,7 +738,7 @@ eval_direct_kernel(Geom g, const float4* __restrict__ table4, const double* __re
                    const int* __restrict__ perm, long long M,
                    float* __restrict__ val, float* __restrict__ grad, float* __restrict__ lap,
                    long long ld, const float* __restrict__ dvec, long long ldd, float* __restrict__ cout,
-                   int* __restrict__ cell_out)
+                   int* __restrict__ cell_out, const double* __restrict__ kvec)
 {
     __shared__ DirectScratch scratch[kWarpsPerBlock];
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
@@ -727,6 +801,12 @@ eval_direct_kernel(Geom g, const float4* __restrict__ table4, const double* __re
         contract_flush<MODE>(g, sum, e, cout, lane);
         return;
     }
+    if (kvec) {                                              // complex orbitals (blipgpu_eval_complex)
+#pragma unroll
+        for (int j = 0; j < NQ; ++j)
+            if (quad[j] < g.pitch4) store_pairs_complex<MODE>(g, acc[j], e, 4 * quad[j], pos, kvec, val, grad, lap, ld);
+        return;
+    }
 #pragma unroll
     for (int j = 0; j < NQ; ++j)
         if (quad[j] < g.pitch4) store_pairs<MODE, 2>(g, acc[j], e, 4 * quad[j], val, grad, lap, ld);
@@ -744,7 +824,7 @@ __global__ void __launch_bounds__(128)
 eval_split_kernel(Geom g, const float4* __restrict__ table4, const double* __restrict__ pos,
                   const int* __restrict__ perm, long long M, float* __restrict__ val, float* __restrict__ grad, float* __restrict__ lap,
                   long long ld, const float* __restrict__ dvec, long long ldd, float* __restrict__ cout,
-                  int* __restrict__ cell_out)
+                  int* __restrict__ cell_out, const double* __restrict__ kvec)
 {
     __shared__ DirectScratch ws;
     __shared__ u64 part[3][5 * 2][32];                       // partial sums of warps 1..3
@@ -815,7 +895,9 @@ eval_split_kernel(Geom g, const float4* __restrict__ table4, const double* __res
         contract_flush<MODE>(g, sum, e, cout, lane);
         return;
     }
-    if (quad < g.pitch4) store_pairs<MODE, 2>(g, acc[0], e, 4 * quad, val, grad, lap, ld);
+    if (quad >= g.pitch4) return;
+    if (kvec) store_pairs_complex<MODE>(g, acc[0], e, 4 * quad, pos, kvec, val, grad, lap, ld);
+    else store_pairs<MODE, 2>(g, acc[0], e, 4 * quad, val, grad, lap, ld);
 }
 
 // ---------------------------------------------------------------------------------------
@@ -959,13 +1041,18 @@ struct StagedCfg {
 // left item k and released all of its planes; while it still works on a unit of item k it
 // only looks whether the descriptor is there yet (to prefetch its first record of item k+1).
 // So whatever a consumer waits for never depends on something that consumer still holds.
-template <int MODE, bool CONTRACT, int VEC, int BY, int BZ, int R, int NW>
+// EPI: what happens to a unit's results (a-5): 0 stored, 1 contracted with d (blipgpu_eval_contract),
+// 2 stored as complex orbitals with a Bloch phase (blipgpu_eval_complex).
+constexpr int kEpiStore = 0, kEpiContract = 1, kEpiComplex = 2;
+template <int MODE, int EPI, int VEC, int BY, int BZ, int R, int NW>
 __global__ void __launch_bounds__((NW + 1) * 32, 1)
 eval_staged_kernel(const __grid_constant__ CUtensorMap tmap, Geom g, StagedGeom sg,
                    const float4* __restrict__ recs, const int4* __restrict__ order, int* __restrict__ meta,
                    int nchunk, float* __restrict__ val, float* __restrict__ grad, float* __restrict__ lap,
-                   long long ld, const float* __restrict__ dvec, long long ldd, float* __restrict__ cout)
+                   long long ld, const float* __restrict__ dvec, long long ldd, float* __restrict__ cout,
+                   const double* __restrict__ pos, const double* __restrict__ kvec)
 {
+    constexpr bool CONTRACT = EPI == kEpiContract;
     using Cfg = StagedCfg<VEC, BY, BZ, R, NW>;
     extern __shared__ __align__(128) unsigned char smem_raw[];
     typename Cfg::Smem& sm = *reinterpret_cast<typename Cfg::Smem*>(smem_raw);
@@ -1152,7 +1239,10 @@ eval_staged_kernel(const __grid_constant__ CUtensorMap tmap, Geom g, StagedGeom 
                     contract_pairs<MODE, NP>(g, a, dq, sum);
                 }
                 contract_flush<MODE>(g, sum, loc.w, cout, lane);
-            } else if (it_col0 < 4 * g.pitch4) store_pairs<MODE, NP>(g, a, loc.w, it_col0, val, grad, lap, ld);
+            } else if (it_col0 < 4 * g.pitch4) {
+                if (EPI == kEpiComplex) store_pairs_complex<MODE>(g, a, loc.w, it_col0, pos, kvec, val, grad, lap, ld);
+                else store_pairs<MODE, NP>(g, a, loc.w, it_col0, val, grad, lap, ld);
+            }
         };
         if (!ok) {                                           // non-finite position (rare): NaN out, no plane touched
             PairAcc nanacc[NP];

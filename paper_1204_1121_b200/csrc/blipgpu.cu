@@ -42,41 +42,49 @@ struct StagedArgs {
     const int4* order; int* meta; int nchunk;
     float* val; float* grad; float* lap; long long ld;
     const float* dvec; long long ldd; float* cout;
+    const double* pos; const double* kvec;
 };
 
-template <int MODE, bool CONTRACT>
+template <int MODE, int EPI>
 cudaError_t staged_prepare1()
 {
-    return cudaFuncSetAttribute(blip::eval_staged_kernel<MODE, CONTRACT, kSVec, kSBY, kSBZ, kSRing, kSWarps>,
+    return cudaFuncSetAttribute(blip::eval_staged_kernel<MODE, EPI, kSVec, kSBY, kSBZ, kSRing, kSWarps>,
                                 cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(StagedShape::Smem));
+}
+template <int EPI>
+cudaError_t staged_prepare_epi()
+{
+    cudaError_t e = staged_prepare1<0, EPI>();
+    if (e == cudaSuccess) e = staged_prepare1<1, EPI>();
+    if (e == cudaSuccess) e = staged_prepare1<2, EPI>();
+    return e;
 }
 cudaError_t staged_prepare()
 {
-    cudaError_t e = staged_prepare1<0, false>();
-    if (e == cudaSuccess) e = staged_prepare1<1, false>();
-    if (e == cudaSuccess) e = staged_prepare1<2, false>();
-    if (e == cudaSuccess) e = staged_prepare1<0, true>();
-    if (e == cudaSuccess) e = staged_prepare1<1, true>();
-    if (e == cudaSuccess) e = staged_prepare1<2, true>();
+    cudaError_t e = staged_prepare_epi<blip::kEpiStore>();
+    if (e == cudaSuccess) e = staged_prepare_epi<blip::kEpiContract>();
+    if (e == cudaSuccess) e = staged_prepare_epi<blip::kEpiComplex>();
     return e;
 }
-template <int MODE, bool CONTRACT>
+template <int MODE, int EPI>
 cudaError_t staged_launch1(unsigned nctas, cudaStream_t s, const StagedArgs& a)
 {
-    return launch_pdl(blip::eval_staged_kernel<MODE, CONTRACT, kSVec, kSBY, kSBZ, kSRing, kSWarps>, nctas,
+    return launch_pdl(blip::eval_staged_kernel<MODE, EPI, kSVec, kSBY, kSBZ, kSRing, kSWarps>, nctas,
                       StagedShape::THREADS, sizeof(StagedShape::Smem), s, *a.tmap, *a.g, *a.sg, a.recs, a.order, a.meta,
-                      a.nchunk, a.val, a.grad, a.lap, a.ld, a.dvec, a.ldd, a.cout);
+                      a.nchunk, a.val, a.grad, a.lap, a.ld, a.dvec, a.ldd, a.cout, a.pos, a.kvec);
+}
+template <int EPI>
+cudaError_t staged_launch_epi(int mode, unsigned nctas, cudaStream_t s, const StagedArgs& a)
+{
+    if (mode == 0) return staged_launch1<0, EPI>(nctas, s, a);
+    if (mode == 2) return staged_launch1<2, EPI>(nctas, s, a);
+    return staged_launch1<1, EPI>(nctas, s, a);
 }
 cudaError_t staged_launch(int mode, unsigned nctas, cudaStream_t s, const StagedArgs& a)
 {
-    if (a.dvec) {
-        if (mode == 0) return staged_launch1<0, true>(nctas, s, a);
-        if (mode == 2) return staged_launch1<2, true>(nctas, s, a);
-        return staged_launch1<1, true>(nctas, s, a);
-    }
-    if (mode == 0) return staged_launch1<0, false>(nctas, s, a);
-    if (mode == 2) return staged_launch1<2, false>(nctas, s, a);
-    return staged_launch1<1, false>(nctas, s, a);
+    if (a.dvec) return staged_launch_epi<blip::kEpiContract>(mode, nctas, s, a);
+    if (a.kvec) return staged_launch_epi<blip::kEpiComplex>(mode, nctas, s, a);
+    return staged_launch_epi<blip::kEpiStore>(mode, nctas, s, a);
 }
 }
 
@@ -295,11 +303,29 @@ static int check_eval_args(const blipgpu_table* t, const double* positions, long
                            const float* val, const float* grad, const float* lap, long long ld)
 {
     if (!t || M < 0) return BLIPGPU_EINVAL;
-    if (mode != BLIPGPU_VALUE && mode != BLIPGPU_VGL) return BLIPGPU_EINVAL;
+    if (mode != BLIPGPU_VALUE && mode != BLIPGPU_VGL && mode != BLIPGPU_VGH) return BLIPGPU_EINVAL;
     if (ld < t->L || (ld % 4) != 0) return BLIPGPU_EINVAL;
     if (M == 0) return BLIPGPU_OK;
     if (!positions || !val) return BLIPGPU_EINVAL;
-    if (mode == BLIPGPU_VGL && (!grad || !lap)) return BLIPGPU_EINVAL;
+    if (mode != BLIPGPU_VALUE && (!grad || !lap)) return BLIPGPU_EINVAL;
+    return BLIPGPU_OK;
+}
+
+// The accuracy / Hessian kernel (blip_f64.cuh): T = float or double, mode VALUE / VGL / VGH.
+template <typename T>
+static int launch_full(blipgpu_table* t, const double* positions, long long M, int mode,
+                       T* val, T* grad, T* third, long long ld, int* cell, cudaStream_t s)
+{
+    const dim3 grid((unsigned)M, (unsigned)((t->g.pitch4 + 31) / 32));
+    if (mode == BLIPGPU_VALUE)
+        blip::eval_full_kernel<T, 0><<<grid, 128, 0, s>>>(t->g, t->g64, t->table, positions, M, val, grad, third, ld, cell);
+    else if (mode == BLIPGPU_VGL)
+        blip::eval_full_kernel<T, 1><<<grid, 128, 0, s>>>(t->g, t->g64, t->table, positions, M, val, grad, third, ld, cell);
+    else
+        blip::eval_full_kernel<T, 2><<<grid, 128, 0, s>>>(t->g, t->g64, t->table, positions, M, val, grad, third, ld, cell);
+    t->launches += 1;
+    t->last_path = 4;
+    CK(t, cudaGetLastError());
     return BLIPGPU_OK;
 }
 
@@ -331,8 +357,11 @@ static bool use_staged(const blipgpu_table* t, long long M)
 // contracted with dvec[e][.] into cout[e][0..4] (cleared by the caller of this function).
 static int launch_eval(blipgpu_table* t, const double* positions, long long M, int mode,
                        float* val, float* grad, float* lap, long long ld, int* cell,
-                       cudaStream_t s, const float* dvec = nullptr, long long ldd = 0, float* cout = nullptr)
+                       cudaStream_t s, const float* dvec = nullptr, long long ldd = 0, float* cout = nullptr,
+                       const double* kvec = nullptr)
 {
+    if (mode == BLIPGPU_VGH)                                  // full Hessian: the per-position kernel, fp32
+        return launch_full<float>(t, positions, M, mode, val, grad, lap, ld, cell, s);
     const int* perm = nullptr;
     const bool staged = use_staged(t, M);
     const int kmode = mode == BLIPGPU_VALUE ? 0 : (t->diag ? 2 : 1);      // kernel template MODE
@@ -368,16 +397,16 @@ static int launch_eval(blipgpu_table* t, const double* positions, long long M, i
     if (staged) {
         if (t->profiling) CK(t, cudaEventRecord(t->pe[1], s));
         const StagedArgs a = {&t->tmap, &t->g, &t->sg, t->recs, t->order, t->meta, t->nchunk,
-                              val, grad, lap, ld, dvec, ldd, cout};
+                              val, grad, lap, ld, dvec, ldd, cout, positions, kvec};
         CK(t, staged_launch(kmode, (unsigned)t->nsm, s, a));
         t->last_path = 2;
     } else if (t->path == 0 && !perm && M <= kSplitMax) {
         t->last_path = 3;
         if (t->profiling) CK(t, cudaEventRecord(t->pe[1], s));
         const dim3 grid((unsigned)M, (unsigned)((t->g.pitch4 + 31) / 32));
-        if (kmode == 0) blip::eval_split_kernel<0><<<grid, 128, 0, s>>>(t->g, t->table, positions, perm, M, val, grad, lap, ld, dvec, ldd, cout, cell);
-        else if (kmode == 2) blip::eval_split_kernel<2><<<grid, 128, 0, s>>>(t->g, t->table, positions, perm, M, val, grad, lap, ld, dvec, ldd, cout, cell);
-        else blip::eval_split_kernel<1><<<grid, 128, 0, s>>>(t->g, t->table, positions, perm, M, val, grad, lap, ld, dvec, ldd, cout, cell);
+        if (kmode == 0) blip::eval_split_kernel<0><<<grid, 128, 0, s>>>(t->g, t->table, positions, perm, M, val, grad, lap, ld, dvec, ldd, cout, cell, kvec);
+        else if (kmode == 2) blip::eval_split_kernel<2><<<grid, 128, 0, s>>>(t->g, t->table, positions, perm, M, val, grad, lap, ld, dvec, ldd, cout, cell, kvec);
+        else blip::eval_split_kernel<1><<<grid, 128, 0, s>>>(t->g, t->table, positions, perm, M, val, grad, lap, ld, dvec, ldd, cout, cell, kvec);
     } else {
         t->last_path = 1;
         const int nq = t->nq;
@@ -387,7 +416,7 @@ static int launch_eval(blipgpu_table* t, const double* positions, long long M, i
         if (t->profiling) CK(t, cudaEventRecord(t->pe[1], s));
 #define BLIP_LAUNCH(MODE, NQ)                                                                         \
         blip::eval_direct_kernel<MODE, NQ><<<grid, block, 0, s>>>(t->g, t->table, positions, perm, M, \
-                                                                  val, grad, lap, ld, dvec, ldd, cout, cell)
+                                                                  val, grad, lap, ld, dvec, ldd, cout, cell, kvec)
         if (kmode == 0) {
             if (nq == 1) BLIP_LAUNCH(0, 1); else if (nq == 2) BLIP_LAUNCH(0, 2); else BLIP_LAUNCH(0, 3);
         } else if (kmode == 2) {
@@ -409,10 +438,40 @@ extern "C" int blipgpu_eval(blipgpu_table* t, const double* positions, long long
 {
     int rc = check_eval_args(t, positions, M, mode, val, grad, lap, ld);
     if (rc != BLIPGPU_OK || M == 0) return rc;
-    if (((uintptr_t)val & 15) || (mode == BLIPGPU_VGL && (((uintptr_t)grad & 15) || ((uintptr_t)lap & 15))))
+    if (((uintptr_t)val & 15) || (mode != BLIPGPU_VALUE && (((uintptr_t)grad & 15) || ((uintptr_t)lap & 15))))
         return BLIPGPU_EINVAL;
     if (M >= (1LL << 31)) return BLIPGPU_EINVAL;
     return launch_eval(t, positions, M, mode, val, grad, lap, ld, cell, (cudaStream_t)stream);
+}
+
+extern "C" int blipgpu_set_kpoints(blipgpu_table* t, const double* kpoints)
+{
+    if (!t) return BLIPGPU_EINVAL;
+    if (!kpoints) {                                           // back to real orbitals only
+        cudaFree(t->kvec);
+        t->kvec = nullptr;
+        return BLIPGPU_OK;
+    }
+    if (t->L % 2) return BLIPGPU_EINVAL;                      // a complex orbital is two adjacent real channels
+    const size_t n = 3 * (size_t)(t->L / 2);
+    for (size_t i = 0; i < n; ++i)
+        if (!std::isfinite(kpoints[i])) return BLIPGPU_EINVAL;
+    if (!t->kvec) CK(t, cudaMalloc(&t->kvec, sizeof(double) * n));
+    CK(t, cudaMemcpy(t->kvec, kpoints, sizeof(double) * n, cudaMemcpyHostToDevice));
+    return BLIPGPU_OK;
+}
+
+extern "C" int blipgpu_eval_complex(blipgpu_table* t, const double* positions, long long M, int mode,
+                                    float* val, float* grad, float* lap, long long ld, int* cell, void* stream)
+{
+    if (!t || !t->kvec) return BLIPGPU_EINVAL;
+    if (mode != BLIPGPU_VALUE && mode != BLIPGPU_VGL) return BLIPGPU_EINVAL;
+    int rc = check_eval_args(t, positions, M, mode, val, grad, lap, ld);
+    if (rc != BLIPGPU_OK || M == 0) return rc;
+    if (((uintptr_t)val & 15) || (mode == BLIPGPU_VGL && (((uintptr_t)grad & 15) || ((uintptr_t)lap & 15))))
+        return BLIPGPU_EINVAL;
+    if (M >= (1LL << 31)) return BLIPGPU_EINVAL;
+    return launch_eval(t, positions, M, mode, val, grad, lap, ld, cell, (cudaStream_t)stream, nullptr, 0, nullptr, t->kvec);
 }
 
 extern "C" int blipgpu_eval_contract(blipgpu_table* t, const double* positions, long long M, int mode,
@@ -433,23 +492,14 @@ extern "C" int blipgpu_eval_f64(blipgpu_table* t, const double* positions, long 
                                 double* val, double* grad, double* lap, long long ld, int* cell, void* stream)
 {
     if (!t || M < 0) return BLIPGPU_EINVAL;
-    if (mode != BLIPGPU_VALUE && mode != BLIPGPU_VGL) return BLIPGPU_EINVAL;
+    if (mode != BLIPGPU_VALUE && mode != BLIPGPU_VGL && mode != BLIPGPU_VGH) return BLIPGPU_EINVAL;
     if (ld < t->L || (ld % 4) != 0) return BLIPGPU_EINVAL;
     if (M == 0) return BLIPGPU_OK;
-    if (!positions || !val || (mode == BLIPGPU_VGL && (!grad || !lap))) return BLIPGPU_EINVAL;
-    if (((uintptr_t)val & 15) || (mode == BLIPGPU_VGL && (((uintptr_t)grad & 15) || ((uintptr_t)lap & 15))))
+    if (!positions || !val || (mode != BLIPGPU_VALUE && (!grad || !lap))) return BLIPGPU_EINVAL;
+    if (((uintptr_t)val & 15) || (mode != BLIPGPU_VALUE && (((uintptr_t)grad & 15) || ((uintptr_t)lap & 15))))
         return BLIPGPU_EINVAL;
     if (M >= (1LL << 31)) return BLIPGPU_EINVAL;
-    cudaStream_t s = (cudaStream_t)stream;
-    const dim3 grid((unsigned)M, (unsigned)((t->g.pitch4 + 31) / 32));
-    if (mode == BLIPGPU_VALUE)
-        blip::eval_f64_kernel<0><<<grid, 128, 0, s>>>(t->g, t->g64, t->table, positions, M, val, grad, lap, ld, cell);
-    else
-        blip::eval_f64_kernel<1><<<grid, 128, 0, s>>>(t->g, t->g64, t->table, positions, M, val, grad, lap, ld, cell);
-    t->launches += 1;
-    t->last_path = 4;
-    CK(t, cudaGetLastError());
-    return BLIPGPU_OK;
+    return launch_full<double>(t, positions, M, mode, val, grad, lap, ld, cell, (cudaStream_t)stream);
 }
 
 extern "C" int blipgpu_reserve(blipgpu_table* t, long long M_max)
@@ -472,9 +522,9 @@ static int ensure_host_staging(blipgpu_table* t, long long M, int mode, long lon
     const long long cap = M;
     CK(t, cudaMalloc(&t->d_pos, sizeof(double) * 3 * (size_t)cap));
     CK(t, cudaMalloc(&t->d_val, sizeof(float) * (size_t)cap * (size_t)ld));
-    if (mode == BLIPGPU_VGL) {
+    if (mode != BLIPGPU_VALUE) {
         CK(t, cudaMalloc(&t->d_grad, sizeof(float) * 3 * (size_t)cap * (size_t)ld));
-        CK(t, cudaMalloc(&t->d_lap, sizeof(float) * (size_t)cap * (size_t)ld));
+        CK(t, cudaMalloc(&t->d_lap, sizeof(float) * (mode == BLIPGPU_VGH ? 6 : 1) * (size_t)cap * (size_t)ld));
     }
     CK(t, cudaMalloc(&t->d_cell, sizeof(int) * 3 * (size_t)cap));
     t->hcap = cap; t->hld = ld; t->hmode = mode;
@@ -497,14 +547,14 @@ extern "C" int blipgpu_eval_host(blipgpu_table* t, const double* positions, long
     // PAPER.md:343): 20 B per evaluation over PCIe against < 1 ms of kernel time, so there is
     // nothing to gain from cutting the batch into pieces to overlap the two.
     CK(t, cudaMemcpyAsync(t->d_pos, positions, sizeof(double) * 3 * (size_t)M, cudaMemcpyHostToDevice, s));
-    rc = launch_eval(t, t->d_pos, M, mode, t->d_val, mode == BLIPGPU_VGL ? t->d_grad : nullptr,
-                     mode == BLIPGPU_VGL ? t->d_lap : nullptr, ld, cell ? t->d_cell : nullptr, s);
+    rc = launch_eval(t, t->d_pos, M, mode, t->d_val, mode != BLIPGPU_VALUE ? t->d_grad : nullptr,
+                     mode != BLIPGPU_VALUE ? t->d_lap : nullptr, ld, cell ? t->d_cell : nullptr, s);
     if (rc != BLIPGPU_OK) return rc;
     const size_t rowb = sizeof(float) * (size_t)ld;
     CK(t, cudaMemcpyAsync(val, t->d_val, rowb * (size_t)M, cudaMemcpyDeviceToHost, s));
-    if (mode == BLIPGPU_VGL) {
+    if (mode != BLIPGPU_VALUE) {
         CK(t, cudaMemcpyAsync(grad, t->d_grad, 3 * rowb * (size_t)M, cudaMemcpyDeviceToHost, s));
-        CK(t, cudaMemcpyAsync(lap, t->d_lap, rowb * (size_t)M, cudaMemcpyDeviceToHost, s));
+        CK(t, cudaMemcpyAsync(lap, t->d_lap, (mode == BLIPGPU_VGH ? 6 : 1) * rowb * (size_t)M, cudaMemcpyDeviceToHost, s));
     }
     if (cell) CK(t, cudaMemcpyAsync(cell, t->d_cell, sizeof(int) * 3 * (size_t)M, cudaMemcpyDeviceToHost, s));
     CK(t, cudaStreamSynchronize(s));
