@@ -510,6 +510,16 @@ def run_gpu(args):
         if mode_vgl and not args.no_contract:
             line["contract"] = run_contract(torch, blip, handle, cfg, w.hpos, w.dpos, stream, args)
             line["f64"] = run_f64(torch, blip, handle, cfg, w.dpos, stream)
+            line["hessian"] = run_hessian(torch, blip, handle, cfg, w.dpos, stream)
+            ups = -(-M * ((L + 127) // 128) // nsm)                       # units (electron x 128 orbitals) per SM of this step
+            tc = blip.blipgpu_probe_tensor(handle, ups, stream)
+            line["tensor_core_recast"] = {
+                "units_per_sm": ups, "ms_fp32_ffma2_form": tc[0], "ms_tf32x3_mma_sync_form": tc[1], "ms_tf32x1_mma_sync_form": tc[2],
+                "note": "arithmetic of one step from a shared-memory tile, no TMA / plane hand-offs (csrc/blip_tcprobe.cuh): "
+                        "the K = 64 per-electron recast D[128][5] = C^T[128][64] W[64][5] on mma.sync.m16n8k8 tf32 with the "
+                        "3-term split the tolerances need, against the packed-FP32 form the kernels use (SURVEY.md §8f NEXT-2)"}
+            if L % 2 == 0:
+                line["complex"] = run_complex(torch, blip, w, args)
         if world == 1 and not args.no_configs:
             # the other BASELINE.json configs (north_star item 4): sweep on this table, then small, tiny, large
             block = {}
@@ -606,6 +616,55 @@ def run_f64(torch, blip, handle, cfg, dpos, stream):
     torch.cuda.synchronize()
     ms = e0.elapsed_time(e1) / 20
     return {"api": "blipgpu_eval_f64", "positions": M, "ms_per_call": ms, "evals_per_s": M * L / (ms * 1e-3), "dtype": "f64"}
+
+
+def run_hessian(torch, blip, handle, cfg, dpos, stream):
+    """mode BLIPGPU_VGH (value, gradient, full Cartesian Hessian) on one walker's
+    worth of positions — the paper's local-energy call — in fp32 and fp64."""
+    M, L = min(int(dpos.shape[0]), max(1, cfg.electrons)), cfg.norb
+    ld = (L + 3) // 4 * 4
+    out = {"positions": M, "outputs_per_eval": 10}
+    for name, tt, fn in (("f32", torch.float32, blip.blipgpu_eval), ("f64", torch.float64, blip.blipgpu_eval_f64)):
+        val = torch.empty((M, ld), dtype=tt, device="cuda")
+        grad = torch.empty((M, 3, ld), dtype=tt, device="cuda")
+        hess = torch.empty((M, 6, ld), dtype=tt, device="cuda")
+        for _ in range(3):
+            fn(handle, dpos, M, blip.VGH, val, grad, hess, ld, None, stream)
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(stream)
+        for _ in range(20):
+            fn(handle, dpos, M, blip.VGH, val, grad, hess, ld, None, stream)
+        e1.record(stream)
+        torch.cuda.synchronize()
+        ms = e0.elapsed_time(e1) / 20
+        out[name] = {"ms_per_call": ms, "evals_per_s": M * L / (ms * 1e-3)}
+    return out
+
+
+def run_complex(torch, blip, w, args):
+    """the same step through blipgpu_eval_complex — L/2 complex orbitals with a
+    Bloch phase per orbital (the paper's workload is complex); k-points from
+    workloads.kpoints (one random twist per orbital: the worst case, no two orbitals share a phase)."""
+    blip.blipgpu_set_kpoints(w.handle, workloads.kpoints(workloads.lattice(w.cfg), w.L // 2))
+    steps = max(1, min(args.steps, 50))
+
+    def step():
+        blip.blipgpu_eval_complex(w.handle, w.dpos, w.M, blip.VGL, w.val, w.grad, w.lap, w.ld, None, w.stream)
+
+    for _ in range(3):
+        step()
+    torch.cuda.synchronize()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record(w.stream)
+    for _ in range(steps):
+        step()
+    e1.record(w.stream)
+    torch.cuda.synchronize()
+    ms = e0.elapsed_time(e1) / steps
+    blip.blipgpu_set_kpoints(w.handle, None)
+    return {"api": "blipgpu_eval_complex", "complex_orbitals": w.L // 2, "ms_per_step": ms, "steps": steps,
+            "real_channel_evals_per_s": w.M * w.L / (ms * 1e-3), "complex_evals_per_s": w.M * (w.L // 2) / (ms * 1e-3)}
 
 
 def run_sweep(torch, blip, w):

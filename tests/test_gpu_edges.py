@@ -315,7 +315,7 @@ def test_argument_errors(torch_cuda, blip):
 
     assert ev() == blip.OK
     assert ev(M=-1) == blip.EINVAL
-    assert ev(mode=2) == blip.EINVAL
+    assert ev(mode=3) == blip.EINVAL
     assert ev(ld=4) == blip.EINVAL            # ld < L
     assert ev(ld=10) == blip.EINVAL           # ld % 4 != 0
     assert ev(val=None) == blip.EINVAL
