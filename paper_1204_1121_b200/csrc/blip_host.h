@@ -32,6 +32,11 @@ struct blipgpu_table {
     unsigned* hist = nullptr;        // [nbins] electrons per bin; zero between calls (scan_kernel clears what it reads)
     unsigned* offs = nullptr;        // [nbins] exclusive scan of hist: where each bin starts in the sorted order
     int hist_dirty = 0;              // a grouping launch failed half-way: clear hist before the next call
+    // one-launch grouping (blip::group_kernel, cooperative): two groups of {count, cursor} arrays that
+    // alternate by the parity of the grid barrier's generation word, all device-side state
+    unsigned* counters = nullptr;    // [4][nbins], zero at creation
+    unsigned* gstate = nullptr;      // [2] {barrier arrivals, barrier generation}
+    int fused_ok = 0;                // cooperative launch available and the histogram fits in shared memory
     // complex orbitals (blipgpu_set_kpoints): Cartesian k of complex orbital m, device [L/2][3] fp64
     double* kvec = nullptr;
     // staging for blipgpu_eval_host (device)

@@ -89,6 +89,86 @@ bin_kernel(Geom g, StagedGeom sg, int staged, const double* __restrict__ pos, lo
     atomicAdd(&hist[b], 1u);
 }
 
+// Work items of the staged kernel (pencil segments), ordered by decreasing electron count — the
+// persistent staged kernel takes items from a shared counter, so heavy items first keeps the
+// tail short (longest-processing-time-first) — and the reset of that counter.  One CTA of
+// kScanThreads threads; `start[b]` = first sorted unit of bin b (global or shared memory),
+// `keybuf` = kScanChunk words of shared memory, *nonempty = 0 on entry (shared memory).
+__device__ __forceinline__ void order_items(const unsigned* start, int nbins, long long M, const Geom& g, const StagedGeom& sg,
+                                            int4* __restrict__ order, int* __restrict__ meta, unsigned* keybuf, int* nonempty)
+{
+    const int tid = threadIdx.x;
+    const unsigned* offs = start;
+    if (tid == 0) meta[1] = 0;
+    const int nps = sg.nps;
+    auto units_of = [&](int i, unsigned& u0, unsigned& u1) {
+        const int pencil = i / sg.nseg, segi = i - pencil * sg.nseg;
+        const int p0 = segi * sg.seg, p1 = min(p0 + sg.seg, g.n[0]);
+        const int bin0 = pencil * g.n[0] + p0, bin1 = pencil * g.n[0] + p1;         // [bin0, bin1)
+        u0 = offs[bin0];
+        u1 = (bin1 < nbins) ? offs[bin1] : (unsigned)M;
+    };
+    if (nps > kMaxSortedItems) {
+        for (int i = tid; i < nps; i += kScanThreads) {
+            unsigned u0, u1;
+            units_of(i, u0, u1);
+            order[i] = make_int4(i, (int)u0, (int)(u1 - u0), 0);
+        }
+        if (tid == 0) meta[0] = nps;
+        return;
+    }
+    unsigned* keys = keybuf;
+    int n2 = 1;
+    while (n2 < nps) n2 <<= 1;
+    int mine = 0;
+    for (int i = tid; i < n2; i += kScanThreads) {
+        unsigned key = 0;
+        if (i < nps) {
+            unsigned u0, u1;
+            units_of(i, u0, u1);
+            const unsigned cnt = min(u1 - u0, (1u << 19) - 1u);
+            key = (cnt << 13) | (unsigned)i;
+            mine += (cnt != 0);
+        }
+        keys[i] = key;
+    }
+    if (mine) atomicAdd(nonempty, mine);
+    __syncthreads();
+    if (nps <= kScanThreads) {
+        // rank sort: keys are distinct (they end in the item id), so the number of larger keys
+        // is the item's place; every thread reads the same key at the same time (a broadcast)
+        if (tid < nps) {
+            const unsigned key = keys[tid];
+            int rank = 0;
+            for (int j = 0; j < nps; ++j) rank += (keys[j] > key);
+            const int id = (int)(key & 8191u);
+            unsigned u0, u1;
+            units_of(id, u0, u1);
+            order[rank] = make_int4(id, (int)u0, (int)(u1 - u0), 0);
+        }
+    } else {
+        for (int k = 2; k <= n2; k <<= 1)                     // bitonic sort, descending
+            for (int j = k >> 1; j > 0; j >>= 1) {
+                for (int i = tid; i < n2; i += kScanThreads) {
+                    const int x = i ^ j;
+                    if (x > i) {
+                        const unsigned a = keys[i], b = keys[x];
+                        const bool desc = (i & k) == 0;
+                        if ((a < b) == desc) { keys[i] = b; keys[x] = a; }
+                    }
+                }
+                __syncthreads();
+            }
+        for (int i = tid; i < nps; i += kScanThreads) {
+            const int id = (int)(keys[i] & 8191u);
+            unsigned u0, u1;
+            units_of(id, u0, u1);
+            order[i] = make_int4(id, (int)u0, (int)(u1 - u0), 0);
+        }
+    }
+    if (tid == 0) meta[0] = *nonempty;
+}
+
 // a-4 (2/3): exclusive scan of the histogram into `offs`, one CTA.  `hist` is all zero on entry
 // to every call (blipgpu_create clears it once) and this kernel, its only reader, puts it back
 // to zero as it reads it: a call leaves no state behind for the next one, so a call captured
@@ -159,74 +239,7 @@ scan_kernel(unsigned* __restrict__ hist, unsigned* __restrict__ offs, int nbins,
     }
     if (!staged) return;
     // offs[b] = start of bin b (written above by this block, visible after the barrier)
-    if (tid == 0) meta[1] = 0;
-    const int nps = sg.nps;
-    auto units_of = [&](int i, unsigned& u0, unsigned& u1) {
-        const int pencil = i / sg.nseg, segi = i - pencil * sg.nseg;
-        const int p0 = segi * sg.seg, p1 = min(p0 + sg.seg, g.n[0]);
-        const int bin0 = pencil * g.n[0] + p0, bin1 = pencil * g.n[0] + p1;         // [bin0, bin1)
-        u0 = offs[bin0];
-        u1 = (bin1 < nbins) ? offs[bin1] : (unsigned)M;
-    };
-    if (nps > kMaxSortedItems) {
-        for (int i = tid; i < nps; i += kScanThreads) {
-            unsigned u0, u1;
-            units_of(i, u0, u1);
-            order[i] = make_int4(i, (int)u0, (int)(u1 - u0), 0);
-        }
-        if (tid == 0) meta[0] = nps;
-        return;
-    }
-    unsigned* keys = buf;
-    int n2 = 1;
-    while (n2 < nps) n2 <<= 1;
-    int mine = 0;
-    for (int i = tid; i < n2; i += kScanThreads) {
-        unsigned key = 0;
-        if (i < nps) {
-            unsigned u0, u1;
-            units_of(i, u0, u1);
-            const unsigned cnt = min(u1 - u0, (1u << 19) - 1u);
-            key = (cnt << 13) | (unsigned)i;
-            mine += (cnt != 0);
-        }
-        keys[i] = key;
-    }
-    if (mine) atomicAdd(&nonempty, mine);
-    __syncthreads();
-    if (nps <= kScanThreads) {
-        // rank sort: keys are distinct (they end in the item id), so the number of larger keys
-        // is the item's place; every thread reads the same key at the same time (a broadcast)
-        if (tid < nps) {
-            const unsigned key = keys[tid];
-            int rank = 0;
-            for (int j = 0; j < nps; ++j) rank += (keys[j] > key);
-            const int id = (int)(key & 8191u);
-            unsigned u0, u1;
-            units_of(id, u0, u1);
-            order[rank] = make_int4(id, (int)u0, (int)(u1 - u0), 0);
-        }
-    } else {
-        for (int k = 2; k <= n2; k <<= 1)                     // bitonic sort, descending
-            for (int j = k >> 1; j > 0; j >>= 1) {
-                for (int i = tid; i < n2; i += kScanThreads) {
-                    const int x = i ^ j;
-                    if (x > i) {
-                        const unsigned a = keys[i], b = keys[x];
-                        const bool desc = (i & k) == 0;
-                        if ((a < b) == desc) { keys[i] = b; keys[x] = a; }
-                    }
-                }
-                __syncthreads();
-            }
-        for (int i = tid; i < nps; i += kScanThreads) {
-            const int id = (int)(keys[i] & 8191u);
-            unsigned u0, u1;
-            units_of(id, u0, u1);
-            order[i] = make_int4(id, (int)u0, (int)(u1 - u0), 0);
-        }
-    }
-    if (tid == 0) meta[0] = nonempty;
+    order_items(offs, nbins, M, g, sg, order, meta, buf, &nonempty);
 }
 
 // a-4 (3/3): scatter electron ids into bin order (order inside a bin is arbitrary; the
@@ -342,16 +355,14 @@ __device__ __forceinline__ void column_weights(const Geom& g, const AX& ax, int 
     cw = g.diag ? make_float4(p00, __fmul_rn(g.J[0], p10), __fmul_rn(g.J[4], p01), la) : make_float4(p00, p10, p01, la);
 }
 
-// Warp-cooperative a-1 + a-2 for electron `e` into `rec` (shared memory).  `ax` is per-warp
-// scratch.  All 32 lanes call it.
-__device__ __forceinline__ void warp_prepare(const Geom& g, const double* __restrict__ pos, int e,
+// Warp-cooperative a-2 for electron `e` into `rec` (shared memory) from its cell map: lanes
+// 0..11 hold (axis a = lane / 4, site m = lane % 4) and are given i_a, f_a of their axis.  `ax`
+// is per-warp scratch.  All 32 lanes call it.
+__device__ __forceinline__ void warp_weights(const Geom& g, int e, int ia, float fa, bool ok,
                                              float (&ax)[3][3][4], ElecRec& rec, int lane)
 {
-    const double x = pos[3 * (size_t)e], y = pos[3 * (size_t)e + 1], z = pos[3 * (size_t)e + 2];
     if (lane < 12) {
         const int a = lane >> 2, m = lane & 3;
-        int ia; float fa;
-        const bool ok = cell_map_axis(g, a, x, y, z, ia, fa);
         float w, d1, d2;
         phi_site(fa, m, w, d1, d2);
         ax[a][0][m] = w; ax[a][1][m] = d1; ax[a][2][m] = d2;
@@ -371,19 +382,22 @@ __device__ __forceinline__ void warp_prepare(const Geom& g, const double* __rest
     __syncwarp();
 }
 
-// a-4 (3/3) + a-1 + a-2 for the staged path: one thread per electron takes its slot in bin
-// order and writes the electron's record there (384 B; read back through L2 by the staged
-// kernel once per orbital chunk).  On return offs[b] is the END of bin b.
-__global__ void __launch_bounds__(128)
-scatter_prep_kernel(Geom g, StagedGeom sg, int tile_floats, const double* __restrict__ pos,
-                    const int* __restrict__ bin, unsigned* __restrict__ offs, long long M,
-                    float4* __restrict__ recs)
+// Warp-cooperative a-1 + a-2 for electron `e` into `rec` (shared memory).  All 32 lanes call it.
+__device__ __forceinline__ void warp_prepare(const Geom& g, const double* __restrict__ pos, int e,
+                                             float (&ax)[3][3][4], ElecRec& rec, int lane)
 {
-    wait_for_predecessor();
-    const long long el = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-    if (el >= M) return;
-    const int e = (int)el;
-    const unsigned s = atomicAdd(&offs[bin[e]], 1u);
+    const double x = pos[3 * (size_t)e], y = pos[3 * (size_t)e + 1], z = pos[3 * (size_t)e + 2];
+    int ia = 0; float fa = 0.f; bool ok = true;
+    if (lane < 12) ok = cell_map_axis(g, lane >> 2, x, y, z, ia, fa);
+    warp_weights(g, e, ia, fa, ok, ax, rec, lane);
+}
+
+// a-1 + a-2 for the staged path: the record of electron e (384 B; read back through L2 by the
+// staged kernel once per orbital chunk), written to slot s of the sorted order.
+__device__ __forceinline__ void write_staged_record(const Geom& g, const StagedGeom& sg, int tile_floats,
+                                                    const double* __restrict__ pos, int e, unsigned s,
+                                                    float4* __restrict__ recs)
+{
     const double x = pos[3 * (size_t)e], y = pos[3 * (size_t)e + 1], z = pos[3 * (size_t)e + 2];
     float ax[3][3][4]; int ic[3];
 #pragma unroll
@@ -419,6 +433,164 @@ scatter_prep_kernel(Geom g, StagedGeom sg, int tile_floats, const double* __rest
         off = ((ic[1] % sg.by) * (sg.bz + 3) + (ic[2] % sg.bz)) * tile_floats * 4;
     }
     out[23] = make_float4(__int_as_float(pl), __int_as_float(off), 0.f, __int_as_float(e));
+}
+
+// a-4 (3/3) for the staged path, three-kernel form: one thread per electron takes its slot in
+// bin order and writes the electron's record there.  On return offs[b] is the END of bin b.
+__global__ void __launch_bounds__(128)
+scatter_prep_kernel(Geom g, StagedGeom sg, int tile_floats, const double* __restrict__ pos,
+                    const int* __restrict__ bin, unsigned* __restrict__ offs, long long M,
+                    float4* __restrict__ recs)
+{
+    wait_for_predecessor();
+    const long long el = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (el >= M) return;
+    const int e = (int)el;
+    const unsigned s = atomicAdd(&offs[bin[e]], 1u);
+    write_staged_record(g, sg, tile_floats, pos, e, s, recs);
+}
+
+// ---------------------------------------------------------------------------------------
+// a-4 in ONE launch (cooperative: every CTA is resident, so the CTAs can wait for one another):
+//   phase 1   every electron: cell -> bin, count[bin] += 1 (and the optional cell output);
+//   barrier   over the grid (arrival counter + generation word in global memory);
+//   phase 2   every CTA scans the whole histogram into its own shared memory (a few thousand
+//             bins: cheaper than a second barrier around a one-CTA scan), then every electron
+//             takes slot start[bin] + cursor[bin]++ and writes its record (staged path) or its
+//             index (direct path) there; CTA 0 orders the work items instead.
+// The three launches of the other form (bin, scan, scatter: ~31 us of a 480 us TiO2 step, mostly
+// launch-to-launch latency) become one of ~12 us.
+//
+// State between calls, all on the device, so that a captured call can be replayed: the counter
+// arrays come in two groups {count, cursor}; a call uses the group selected by the parity of
+// the barrier generation, which it finds all zero, and zeroes the other group, which the
+// previous call left dirty.  gstate = {arrivals, generation}.
+// Shared memory: (nbins + 1) words for the scan, dynamic.
+// ---------------------------------------------------------------------------------------
+template <bool STAGED>
+__global__ void __launch_bounds__(kScanThreads, 1)
+group_kernel(Geom g, StagedGeom sg, int tile_floats, const double* __restrict__ pos, long long M,
+             unsigned* __restrict__ counters /* [4][nalloc] */, int nalloc, int nbins, unsigned* __restrict__ gstate,
+             int4* __restrict__ order, int* __restrict__ meta, float4* __restrict__ recs, int* __restrict__ perm,
+             int* __restrict__ cell)
+{
+    extern __shared__ __align__(16) unsigned start[];        // [nbins + 1] exclusive scan of the counts
+    __shared__ unsigned wsum[kScanThreads / 32];
+    __shared__ unsigned keybuf[STAGED ? kScanChunk : 1];   // CTA 0 of the staged form sorts the work items here
+    __shared__ int nonempty;
+    __shared__ unsigned gen_s;
+    const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
+    if (tid == 0) { gen_s = *reinterpret_cast<volatile unsigned*>(gstate + 1); nonempty = 0; }
+    __syncthreads();
+    const unsigned gen = gen_s;
+    unsigned* count = counters + (size_t)(2 * (gen & 1u)) * nalloc;
+    unsigned* cursor = count + nalloc;
+    unsigned* stale = counters + (size_t)(2 * ((gen & 1u) ^ 1u)) * nalloc;     // both arrays of the other group
+    const long long nthreads = (long long)gridDim.x * kScanThreads;
+    const long long gtid = (long long)blockIdx.x * kScanThreads + tid;
+
+    auto bin_of = [&](long long e, int (&ic)[3]) -> int {
+        const double x = pos[3 * e], y = pos[3 * e + 1], z = pos[3 * e + 2];
+        float f;
+        bool ok = cell_map_axis(g, 0, x, y, z, ic[0], f);
+        ok = cell_map_axis(g, 1, x, y, z, ic[1], f) && ok;
+        ok = cell_map_axis(g, 2, x, y, z, ic[2], f) && ok;
+        if (!ok) { ic[0] = ic[1] = ic[2] = -1; return 0; }
+        return STAGED ? staged_key(g, sg, ic[0], ic[1], ic[2]) : brick_of(g, ic[0], ic[1], ic[2]);
+    };
+    // ---- phase 1 (an equal share of the electrons per CTA)
+    {
+        const long long share1 = (M + gridDim.x - 1) / gridDim.x;
+        const long long a0 = (long long)blockIdx.x * share1, a1 = min(a0 + share1, M);
+        for (long long e = a0 + tid; e < a1; e += kScanThreads) {
+            int ic[3];
+            const int b = bin_of(e, ic);
+            if (cell) { cell[3 * e] = ic[0]; cell[3 * e + 1] = ic[1]; cell[3 * e + 2] = ic[2]; }
+            atomicAdd(&count[b], 1u);
+        }
+    }
+    for (long long i = gtid; i < 2LL * nalloc; i += nthreads) stale[i] = 0u;
+    // ---- grid barrier
+    __syncthreads();
+    if (tid == 0) {
+        __threadfence();
+        const unsigned arrived = atomicAdd(gstate, 1u);
+        if (arrived == gridDim.x - 1) {
+            *reinterpret_cast<volatile unsigned*>(gstate) = 0u;
+            __threadfence();
+            atomicAdd(gstate + 1, 1u);
+        } else {
+            while (*reinterpret_cast<volatile unsigned*>(gstate + 1) == gen) __nanosleep(40);
+        }
+        __threadfence();
+    }
+    __syncthreads();
+    // ---- phase 2: exclusive scan of count[0 .. nbins) into shared memory (every CTA, redundantly)
+    for (int base = 0; base < nbins; base += 8 * kScanThreads) {      // 8 independent loads per thread in flight
+        unsigned v[8];
+#pragma unroll
+        for (int k = 0; k < 8; ++k) {
+            const int i = base + tid + k * kScanThreads;
+            v[k] = (i < nbins) ? __ldcg(count + i) : 0u;
+        }
+#pragma unroll
+        for (int k = 0; k < 8; ++k) {
+            const int i = base + tid + k * kScanThreads;
+            if (i < nbins) start[i] = v[k];
+        }
+    }
+    __syncthreads();
+    const int per = ((nbins + kScanThreads - 1) / kScanThreads) | 1;     // odd: consecutive threads start in different banks
+    const int b0 = min(tid * per, nbins), b1 = min(b0 + per, nbins);
+    unsigned sum = 0;
+    for (int b = b0; b < b1; ++b) { const unsigned v = start[b]; start[b] = sum; sum += v; }
+    unsigned inc = sum;
+#pragma unroll
+    for (int d = 1; d < 32; d <<= 1) {
+        const unsigned t = __shfl_up_sync(0xffffffffu, inc, d);
+        if (lane >= d) inc += t;
+    }
+    if (lane == 31) wsum[wid] = inc;
+    __syncthreads();
+    if (wid == 0) {
+        unsigned w = wsum[lane], winc = w;
+#pragma unroll
+        for (int d = 1; d < 32; d <<= 1) {
+            const unsigned t = __shfl_up_sync(0xffffffffu, winc, d);
+            if (lane >= d) winc += t;
+        }
+        wsum[lane] = winc - w;
+    }
+    __syncthreads();
+    const unsigned toff = wsum[wid] + inc - sum;
+    for (int b = b0; b < b1; ++b) start[b] += toff;
+    if (tid == 0) start[nbins] = (unsigned)M;
+    __syncthreads();
+    if (STAGED && blockIdx.x == 0) {                         // CTA 0: the work items of the staged kernel
+        order_items(start, nbins + 1, M, g, sg, order, meta, keybuf, &nonempty);
+        if (gridDim.x > 1) return;
+    }
+    // ---- phase 2: scatter (CTAs 1.. when CTA 0 orders the items), an equal share of the electrons per CTA
+    const int first = (STAGED && gridDim.x > 1) ? 1 : 0;
+    const long long nc = (long long)gridDim.x - first;
+    const long long share = (M + nc - 1) / nc;
+    const long long e0 = (long long)(blockIdx.x - first) * share, e1 = min(e0 + share, M);
+    if (STAGED) {
+        // a thread per electron: every electron of the CTA's share is in flight at once (position
+        // load, fp64 cell map, slot atomic, weights, 24 float4 stores)
+        for (long long e = e0 + tid; e < e1; e += kScanThreads) {
+            int ic[3];
+            const int b = bin_of(e, ic);
+            const unsigned slot = start[b] + atomicAdd(&cursor[b], 1u);
+            write_staged_record(g, sg, tile_floats, pos, (int)e, slot, recs);
+        }
+    } else {
+        for (long long e = e0 + tid; e < e1; e += kScanThreads) {
+            int ic[3];
+            const int b = bin_of(e, ic);
+            perm[start[b] + atomicAdd(&cursor[b], 1u)] = (int)e;
+        }
+    }
 }
 
 // ---------------------------------------------------------------------------------------

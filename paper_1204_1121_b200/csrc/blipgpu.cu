@@ -258,6 +258,10 @@ extern "C" int blipgpu_create(const double* lattice, const int* grid, int norb,
     if (rc == BLIPGPU_OK && (e = cudaMalloc(&t->hist, sizeof(unsigned) * (size_t)t->nbins)) != cudaSuccess) fail(e);
     if (rc == BLIPGPU_OK && (e = cudaMalloc(&t->offs, sizeof(unsigned) * (size_t)t->nbins)) != cudaSuccess) fail(e);
     if (rc == BLIPGPU_OK && (e = cudaMemsetAsync(t->hist, 0, sizeof(unsigned) * (size_t)t->nbins, s)) != cudaSuccess) fail(e);
+    if (rc == BLIPGPU_OK && (e = cudaMalloc(&t->counters, 4 * sizeof(unsigned) * (size_t)t->nbins)) != cudaSuccess) fail(e);
+    if (rc == BLIPGPU_OK && (e = cudaMemsetAsync(t->counters, 0, 4 * sizeof(unsigned) * (size_t)t->nbins, s)) != cudaSuccess) fail(e);
+    if (rc == BLIPGPU_OK && (e = cudaMalloc(&t->gstate, 2 * sizeof(unsigned))) != cudaSuccess) fail(e);
+    if (rc == BLIPGPU_OK && (e = cudaMemsetAsync(t->gstate, 0, 2 * sizeof(unsigned), s)) != cudaSuccess) fail(e);
     if (rc == BLIPGPU_OK && (e = cudaMalloc(&t->order, sizeof(int4) * (size_t)(t->sg.nps + 1))) != cudaSuccess) fail(e);
     if (rc == BLIPGPU_OK && (e = cudaMalloc(&t->meta, sizeof(int) * 2)) != cudaSuccess) fail(e);
     if (rc == BLIPGPU_OK && !coeffs_on_device) {
@@ -282,6 +286,18 @@ extern "C" int blipgpu_create(const double* lattice, const int* grid, int norb,
             if (e == cudaSuccess) t->staged_ok = 1; else (void)cudaGetLastError();
         }
     }
+    if (rc == BLIPGPU_OK) {
+        // one-launch grouping: needs a cooperative launch of one 1,024-thread CTA per SM and the
+        // histogram (+ 1 word) in dynamic shared memory next to the kernel's static 33 KB
+        int coop = 0;
+        const size_t need = sizeof(unsigned) * ((size_t)t->nbins + 1);
+        const size_t room = (size_t)prop.sharedMemPerBlockOptin - 40 * 1024;    // the attribute is per function, not per table: always the maximum
+        if (cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, dev) == cudaSuccess && coop && need <= room &&
+            cudaFuncSetAttribute(blip::group_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)room) == cudaSuccess &&
+            cudaFuncSetAttribute(blip::group_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)room) == cudaSuccess)
+            t->fused_ok = 1;
+        (void)cudaGetLastError();
+    }
     if (rc != BLIPGPU_OK) { blipgpu_destroy(t); return rc; }
     *out = t;
     return BLIPGPU_OK;
@@ -290,7 +306,7 @@ extern "C" int blipgpu_create(const double* lattice, const int* grid, int norb,
 extern "C" int blipgpu_destroy(blipgpu_table* t)
 {
     if (!t) return BLIPGPU_OK;
-    cudaFree(t->table); cudaFree(t->bin); cudaFree(t->perm); cudaFree(t->recs); cudaFree(t->hist); cudaFree(t->offs);
+    cudaFree(t->table); cudaFree(t->bin); cudaFree(t->perm); cudaFree(t->recs); cudaFree(t->hist); cudaFree(t->offs); cudaFree(t->counters); cudaFree(t->gstate);
     cudaFree(t->order); cudaFree(t->meta); cudaFree(t->kvec);
     cudaFree(t->d_pos); cudaFree(t->d_val); cudaFree(t->d_grad); cudaFree(t->d_lap); cudaFree(t->d_cell);
     for (int k = 0; k < 3; ++k) if (t->pe[k]) cudaEventDestroy(t->pe[k]);
@@ -372,6 +388,24 @@ static int launch_eval(blipgpu_table* t, const double* positions, long long M, i
         int rc = ensure_workspace(t, M, s);
         if (rc != BLIPGPU_OK) return rc;
         const int nbins = staged ? t->nbins_staged : t->nbins_direct;
+        if (t->fused_ok) {
+            // a-4 in one cooperative launch (blip::group_kernel): count, grid barrier, scan + scatter
+            cudaLaunchConfig_t cfg = {};
+            cfg.gridDim = dim3((unsigned)t->nsm); cfg.blockDim = dim3(blip::kScanThreads);
+            cfg.dynamicSmemBytes = sizeof(unsigned) * ((size_t)nbins + 1); cfg.stream = s;
+            cudaLaunchAttribute attr[1];
+            attr[0].id = cudaLaunchAttributeCooperative;
+            attr[0].val.cooperative = 1;
+            cfg.attrs = attr; cfg.numAttrs = 1;
+            if (staged)
+                CK(t, cudaLaunchKernelEx(&cfg, blip::group_kernel<true>, t->g, t->sg, (int)kSC, positions, M, t->counters, t->nbins,
+                                         nbins, t->gstate, t->order, t->meta, t->recs, t->perm, cell));
+            else
+                CK(t, cudaLaunchKernelEx(&cfg, blip::group_kernel<false>, t->g, t->sg, (int)kSC, positions, M, t->counters, t->nbins,
+                                         nbins, t->gstate, t->order, t->meta, t->recs, t->perm, cell));
+            t->launches += 1;
+        } else {
+        // three launches (tables whose histogram does not fit in shared memory).
         // t->hist is zero here: blipgpu_create cleared it and the scan kernel of every call puts
         // back to zero what it reads, so the call is self-contained in stream order (no host-side
         // state: a captured call can be replayed).  Only a launch failure half-way leaves it dirty.
@@ -391,6 +425,7 @@ static int launch_eval(blipgpu_table* t, const double* positions, long long M, i
         else
             CK(t, launch_pdl(blip::scatter_kernel, nb, 256, 0, s, (const int*)t->bin, t->offs, M, t->perm));
         t->launches += 3;
+        }
         perm = t->perm;
         cell = nullptr;                                  // already written by bin_kernel
     }

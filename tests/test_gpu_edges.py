@@ -76,7 +76,7 @@ def test_staged_path_matches_oracle_and_direct_path(torch_cuda, blip, grid, L, M
         blip.blipgpu_set_tuning(t.handle, path=2)
         n0 = t.launch_count()
         staged = run_gpu(torch_cuda, blip, A, grid, c, pos, mode=mode, table=t)
-        assert t.launch_count() - n0 == 4                # bin, scan, scatter+prep, staged eval
+        assert t.launch_count() - n0 == 2                # grouping (one cooperative launch), staged eval
         compare(A, grid, c, pos, staged, mode=mode)
         blip.blipgpu_set_tuning(t.handle, path=1)
         direct = run_gpu(torch_cuda, blip, A, grid, c, pos, mode=mode, table=t)
@@ -241,7 +241,7 @@ def test_eval_host_staged_path_large_batch(torch_cuda, blip):
     hlap = torch.empty((M, ld), dtype=torch.float32).pin_memory()
     n0 = t.launch_count()
     blip.blipgpu_eval_host(t.handle, hpos, M, blip.VGL, hval, hgrad, hlap, ld, None)
-    assert t.launch_count() - n0 == 4 and blip.blipgpu_last_path(t.handle) == 2
+    assert t.launch_count() - n0 == 2 and blip.blipgpu_last_path(t.handle) == 2
     assert np.array_equal(hval.numpy()[:, :L], dev[0])
     assert np.array_equal(hgrad.numpy()[:, :, :L], dev[1])
     assert np.array_equal(hlap.numpy()[:, :L], dev[2])
