@@ -987,9 +987,11 @@ eval_direct_kernel(Geom g, const float4* __restrict__ table4, const double* __re
 // ---------------------------------------------------------------------------------------
 // Split kernel, for small batches (the paper's particle-by-particle end of the sweep,
 // PAPER.md:268 kernel (1), where a call is a handful of electrons and the cost is latency):
-// CTA = (electron, 128 orbitals), 4 warps; warp m1 takes the 16 rows of plane i1 + m1, issues
-// all 16 loads at once (one memory round trip instead of eight dependent ones), folds them,
-// and the four partial sums are added in plane order through shared memory.
+// CTA = (electron, 128 orbitals), 4 warps; warp m1 takes the 16 rows of plane i1 + m1.  Every
+// warp maps the position to its cell itself (a-1, fp64) and issues its 16 loads at once — one
+// memory round trip, started as early as possible — and only then computes the weights (a-2),
+// while the loads are in flight; the four partial sums are added in plane order through shared
+// memory.  One block barrier per CTA.
 // ---------------------------------------------------------------------------------------
 template <int MODE>
 __global__ void __launch_bounds__(128)
@@ -998,36 +1000,41 @@ eval_split_kernel(Geom g, const float4* __restrict__ table4, const double* __res
                   long long ld, const float* __restrict__ dvec, long long ldd, float* __restrict__ cout,
                   int* __restrict__ cell_out, const double* __restrict__ kvec)
 {
-    __shared__ DirectScratch ws;
+    __shared__ DirectScratch wsw[4];                         // one per warp
     __shared__ u64 part[3][5 * 2][32];                       // partial sums of warps 1..3
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int e = perm ? perm[blockIdx.x] : (int)blockIdx.x;
     const ulonglong2* __restrict__ table = reinterpret_cast<const ulonglong2*>(table4);
     const int quad = blockIdx.y * 32 + lane;
     const unsigned off[1] = {(unsigned)min(quad, g.pitch4 - 1)};
-    if (warp == 0) warp_prepare(g, pos, e, ws.ax, ws.rec, lane);
-    __syncthreads();
-    const int i1 = ws.rec.i[0], i2 = ws.rec.i[1], i3 = ws.rec.i[2];
+    DirectScratch& ws = wsw[warp];
+    // a-1: lanes 0..11 = (axis lane / 4, site lane % 4); lanes 0, 4, 8 hold the three cell indices
+    const double x = pos[3 * (size_t)e], y = pos[3 * (size_t)e + 1], z = pos[3 * (size_t)e + 2];
+    int ia = 0; float fa = 0.f; bool okl = true;
+    if (lane < 12) okl = cell_map_axis(g, lane >> 2, x, y, z, ia, fa);
+    const int i1 = __shfl_sync(0xffffffffu, ia, 0), i2 = __shfl_sync(0xffffffffu, ia, 4), i3 = __shfl_sync(0xffffffffu, ia, 8);
     const bool ok = (i1 | i2 | i3) >= 0;
-    if (cell_out && blockIdx.y == 0 && threadIdx.x < 3) cell_out[3 * (size_t)e + threadIdx.x] = ok ? ws.rec.i[threadIdx.x] : -1;
+    if (cell_out && blockIdx.y == 0 && warp == 0 && lane < 12 && (lane & 3) == 0) cell_out[3 * (size_t)e + (lane >> 2)] = ok ? ia : -1;
 
     PairAcc acc[1][2];
 #pragma unroll
     for (int h = 0; h < 2; ++h) acc[0][h].val = acc[0][h].t1 = acc[0][h].t2 = acc[0][h].t3 = acc[0][h].lp = 0ull;
+    ulonglong2 buf[4][4];
+    if (ok) {                                                // all 16 rows of plane i1 + warp in flight
+        const unsigned s2 = (unsigned)g.np[2];
+        const unsigned row0 = ((unsigned)(i1 + warp) * g.np[1] + i2) * g.np[2] + i3;
+#pragma unroll
+        for (int m2 = 0; m2 < 4; ++m2) load_column<1>(table, off, row0 + m2 * s2, g.pitch4, buf[m2]);
+    }
+    warp_weights(g, e, ia, fa, okl, ws.ax, ws.rec, lane);    // a-2, while the loads are in flight
     if (ok) {
         float wz[3][4];
 #pragma unroll
         for (int k = 0; k < 3; ++k)
 #pragma unroll
             for (int m = 0; m < 4; ++m) wz[k][m] = ws.rec.wz[k][m];
-        const unsigned s1 = (unsigned)g.np[1] * g.np[2], s2 = (unsigned)g.np[2];
-        const unsigned row0 = ((unsigned)(i1 + warp) * g.np[1] + i2) * g.np[2] + i3;
-        ulonglong2 buf[4][4];
-#pragma unroll
-        for (int m2 = 0; m2 < 4; ++m2) load_column<1>(table, off, row0 + m2 * s2, g.pitch4, buf[m2]);
 #pragma unroll
         for (int m2 = 0; m2 < 4; ++m2) fold_column<MODE, 1>(ws.rec, 4 * warp + m2, wz, buf[m2], acc);
-        (void)s1;
     }
     if (warp > 0) {
 #pragma unroll

@@ -327,18 +327,13 @@ static int check_eval_args(const blipgpu_table* t, const double* positions, long
     return BLIPGPU_OK;
 }
 
-// The accuracy / Hessian kernel (blip_f64.cuh): T = float or double, mode VALUE / VGL / VGH.
+// Mode VGH (value, gradient, full Cartesian Hessian): blip::eval_full_kernel<T, 2>, T = float or double.
 template <typename T>
-static int launch_full(blipgpu_table* t, const double* positions, long long M, int mode,
-                       T* val, T* grad, T* third, long long ld, int* cell, cudaStream_t s)
+static int launch_hess(blipgpu_table* t, const double* positions, long long M,
+                       T* val, T* grad, T* hess, long long ld, int* cell, cudaStream_t s)
 {
     const dim3 grid((unsigned)M, (unsigned)((t->g.pitch4 + 31) / 32));
-    if (mode == BLIPGPU_VALUE)
-        blip::eval_full_kernel<T, 0><<<grid, 128, 0, s>>>(t->g, t->g64, t->table, positions, M, val, grad, third, ld, cell);
-    else if (mode == BLIPGPU_VGL)
-        blip::eval_full_kernel<T, 1><<<grid, 128, 0, s>>>(t->g, t->g64, t->table, positions, M, val, grad, third, ld, cell);
-    else
-        blip::eval_full_kernel<T, 2><<<grid, 128, 0, s>>>(t->g, t->g64, t->table, positions, M, val, grad, third, ld, cell);
+    blip::eval_full_kernel<T, 2><<<grid, 128, 0, s>>>(t->g, t->g64, t->table, positions, M, val, grad, hess, ld, cell);
     t->launches += 1;
     t->last_path = 4;
     CK(t, cudaGetLastError());
@@ -377,7 +372,7 @@ static int launch_eval(blipgpu_table* t, const double* positions, long long M, i
                        const double* kvec = nullptr)
 {
     if (mode == BLIPGPU_VGH)                                  // full Hessian: the per-position kernel, fp32
-        return launch_full<float>(t, positions, M, mode, val, grad, lap, ld, cell, s);
+        return launch_hess<float>(t, positions, M, val, grad, lap, ld, cell, s);
     const int* perm = nullptr;
     const bool staged = use_staged(t, M);
     const int kmode = mode == BLIPGPU_VALUE ? 0 : (t->diag ? 2 : 1);      // kernel template MODE
@@ -534,7 +529,17 @@ extern "C" int blipgpu_eval_f64(blipgpu_table* t, const double* positions, long 
     if (((uintptr_t)val & 15) || (mode != BLIPGPU_VALUE && (((uintptr_t)grad & 15) || ((uintptr_t)lap & 15))))
         return BLIPGPU_EINVAL;
     if (M >= (1LL << 31)) return BLIPGPU_EINVAL;
-    return launch_full<double>(t, positions, M, mode, val, grad, lap, ld, cell, (cudaStream_t)stream);
+    cudaStream_t s = (cudaStream_t)stream;
+    if (mode == BLIPGPU_VGH) return launch_hess<double>(t, positions, M, val, grad, lap, ld, cell, s);
+    const dim3 grid((unsigned)M, (unsigned)((t->g.pitch4 + 31) / 32));
+    if (mode == BLIPGPU_VALUE)
+        blip::eval_f64_kernel<0><<<grid, 128, 0, s>>>(t->g, t->g64, t->table, positions, M, val, grad, lap, ld, cell);
+    else
+        blip::eval_f64_kernel<1><<<grid, 128, 0, s>>>(t->g, t->g64, t->table, positions, M, val, grad, lap, ld, cell);
+    t->launches += 1;
+    t->last_path = 4;
+    CK(t, cudaGetLastError());
+    return BLIPGPU_OK;
 }
 
 extern "C" int blipgpu_reserve(blipgpu_table* t, long long M_max)

@@ -359,3 +359,20 @@ def test_distinct_handles_on_distinct_streams(torch_cuda, blip):
             assert torch.equal(o[0][:, :L], ref[0]) and torch.equal(o[1][:, :, :L], ref[1]) and torch.equal(o[2][:, :L], ref[2])
     for t, *_ in cases:
         t.close()
+
+
+def test_grouping_with_more_bins_than_fit_in_shared_memory(torch_cuda, blip):
+    """A 200^3 grid has 125,000 bricks: the histogram does not fit in the shared memory of the
+    one-launch grouping kernel, so the call goes through the three-kernel form (bin, scan,
+    scatter); twice, to check that it leaves its histogram clean."""
+    grid, L, M = (200, 200, 200), 4, 6000
+    lat = ((40.0, 0.0, 0.0), (1.0, 41.0, 0.0), (0.5, 0.25, 39.0))
+    A, c, pos = workloads.small_case(grid, L, M, lat, seed=31, spread=1.5)
+    t = blip.BlipTable(A, grid, L, c)
+    blip.blipgpu_set_tuning(t.handle, path=1)
+    for _ in range(2):
+        n0 = t.launch_count()
+        out = run_gpu(torch_cuda, blip, A, grid, c, pos, table=t)
+        assert t.launch_count() - n0 == 4 and blip.blipgpu_last_path(t.handle) == 1
+        compare(A, grid, c, pos, out)
+    t.close()
