@@ -253,6 +253,7 @@ scatter_kernel(const int* __restrict__ bin, unsigned* __restrict__ offs, long lo
     long long e = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (e >= M) return;
     unsigned slot = atomicAdd(&offs[bin[e]], 1u);
+    BLIP_ASSERT((long long)slot < M);
     perm[slot] = (int)e;
 }
 
@@ -447,6 +448,7 @@ scatter_prep_kernel(Geom g, StagedGeom sg, int tile_floats, const double* __rest
     if (el >= M) return;
     const int e = (int)el;
     const unsigned s = atomicAdd(&offs[bin[e]], 1u);
+    BLIP_ASSERT((long long)s < M);
     write_staged_record(g, sg, tile_floats, pos, e, s, recs);
 }
 
@@ -505,6 +507,7 @@ group_kernel(Geom g, StagedGeom sg, int tile_floats, const double* __restrict__ 
         for (long long e = a0 + tid; e < a1; e += kScanThreads) {
             int ic[3];
             const int b = bin_of(e, ic);
+            BLIP_ASSERT(b >= 0 && b < nbins);
             if (cell) { cell[3 * e] = ic[0]; cell[3 * e + 1] = ic[1]; cell[3 * e + 2] = ic[2]; }
             atomicAdd(&count[b], 1u);
         }
@@ -582,13 +585,16 @@ group_kernel(Geom g, StagedGeom sg, int tile_floats, const double* __restrict__ 
             int ic[3];
             const int b = bin_of(e, ic);
             const unsigned slot = start[b] + atomicAdd(&cursor[b], 1u);
+            BLIP_ASSERT(slot < start[b + 1] && (long long)slot < M);
             write_staged_record(g, sg, tile_floats, pos, (int)e, slot, recs);
         }
     } else {
         for (long long e = e0 + tid; e < e1; e += kScanThreads) {
             int ic[3];
             const int b = bin_of(e, ic);
-            perm[start[b] + atomicAdd(&cursor[b], 1u)] = (int)e;
+            const unsigned slot = start[b] + atomicAdd(&cursor[b], 1u);
+            BLIP_ASSERT(slot < start[b + 1] && (long long)slot < M);
+            perm[slot] = (int)e;
         }
     }
 }
@@ -692,6 +698,7 @@ __device__ __forceinline__ void store_pairs(const Geom& g, const PairAcc (&acc)[
     }
     const size_t o = (size_t)e * (size_t)ld + (size_t)col0;
     const size_t og = (size_t)e * 3 * (size_t)ld + (size_t)col0;
+    BLIP_ASSERT(e >= 0 && (long long)e < g.M && col0 >= 0 && (long long)col0 + 2 * NP <= ld);
     if (NP == 2) {
         st_stream4(val + o, v[0], v[1], v[2], v[3]);
         if (MODE != 0) {
@@ -776,6 +783,7 @@ __device__ __forceinline__ void store_pairs_complex(const Geom& g, const PairAcc
     }
     const size_t o = (size_t)e * (size_t)ld + (size_t)col0;
     const size_t og = (size_t)e * 3 * (size_t)ld + (size_t)col0;
+    BLIP_ASSERT(e >= 0 && (long long)e < g.M && col0 >= 0 && (long long)col0 + 4 <= ld);
     st_stream4(val + o, v[0], v[1], v[2], v[3]);
     if (MODE != 0) {
         st_stream4(grad + og, gx[0], gx[1], gx[2], gx[3]);
@@ -882,9 +890,11 @@ struct DirectScratch {
 
 template <int NQ>
 __device__ __forceinline__ void load_column(const ulonglong2* __restrict__ table, const unsigned (&off)[NQ],
-                                            unsigned colrow, int pitch4, ulonglong2 (&buf)[4 * NQ])
+                                            unsigned colrow, int pitch4, ulonglong2 (&buf)[4 * NQ],
+                                            long long nrows_checked = 0)
 {
     const unsigned base = colrow * (unsigned)pitch4;
+    BLIP_ASSERT((unsigned long long)colrow + 3 < (unsigned long long)nrows_checked);
 #pragma unroll
     for (int m = 0; m < 4; ++m)
 #pragma unroll
@@ -948,15 +958,15 @@ eval_direct_kernel(Geom g, const float4* __restrict__ table4, const double* __re
         const unsigned row0 = ((unsigned)i1 * g.np[1] + i2) * g.np[2] + i3;
         const unsigned s1 = (unsigned)g.np[1] * g.np[2], s2 = (unsigned)g.np[2];
         ulonglong2 buf0[4 * NQ], buf1[4 * NQ];
-        load_column<NQ>(table, off, row0, g.pitch4, buf0);
+        load_column<NQ>(table, off, row0, g.pitch4, buf0, (long long)g.np[0] * g.np[1] * g.np[2]);
 #pragma unroll 1
         for (int c = 0; c < 16; c += 2) {
             const unsigned r1 = row0 + (c >> 2) * s1 + ((c + 1) & 3) * s2;
-            load_column<NQ>(table, off, r1, g.pitch4, buf1);
+            load_column<NQ>(table, off, r1, g.pitch4, buf1, (long long)g.np[0] * g.np[1] * g.np[2]);
             fold_column<MODE, NQ>(ws.rec, c, wz, buf0, acc);
             if (c + 2 < 16) {
                 const unsigned r2 = row0 + ((c + 2) >> 2) * s1 + ((c + 2) & 3) * s2;
-                load_column<NQ>(table, off, r2, g.pitch4, buf0);
+                load_column<NQ>(table, off, r2, g.pitch4, buf0, (long long)g.np[0] * g.np[1] * g.np[2]);
             }
             fold_column<MODE, NQ>(ws.rec, c + 1, wz, buf1, acc);
         }
@@ -1024,7 +1034,7 @@ eval_split_kernel(Geom g, const float4* __restrict__ table4, const double* __res
         const unsigned s2 = (unsigned)g.np[2];
         const unsigned row0 = ((unsigned)(i1 + warp) * g.np[1] + i2) * g.np[2] + i3;
 #pragma unroll
-        for (int m2 = 0; m2 < 4; ++m2) load_column<1>(table, off, row0 + m2 * s2, g.pitch4, buf[m2]);
+        for (int m2 = 0; m2 < 4; ++m2) load_column<1>(table, off, row0 + m2 * s2, g.pitch4, buf[m2], (long long)g.np[0] * g.np[1] * g.np[2]);
     }
     warp_weights(g, e, ia, fa, okl, ws.ax, ws.rec, lane);    // a-2, while the loads are in flight
     if (ok) {
@@ -1383,7 +1393,9 @@ eval_staged_kernel(const __grid_constant__ CUtensorMap tmap, Geom g, StagedGeom 
             __syncwarp();
         }
         const StagedRec& rec = reinterpret_cast<const StagedRec&>(sm.rec[warp]);
-        const int4 loc = rec.loc;                            // {plane in item or -1, byte offset in plane, -, electron}
+        const int4 loc = rec.loc;
+        BLIP_ASSERT((long long)((it_rsrc - recs) / (kRecFloats / 4)) + u < g.M && loc.w >= 0 && (long long)loc.w < g.M);
+        BLIP_ASSERT(loc.x < it_nplanes - 3 && loc.y >= 0 && loc.y + 3 * (Cfg::PZ * Cfg::C * 4) + 4 * Cfg::C * 4 <= Cfg::PLANE_BYTES);                            // {plane in item or -1, byte offset in plane, -, electron}
         const bool ok = loc.x >= 0;                          // non-finite positions (bin 0) touch no plane
         const unsigned sq = it_seq0 + (unsigned)loc.x;
         // planes i1, i1+1 resident, earlier ones released; planes i1+2 and i1+3 are waited for
@@ -1442,6 +1454,7 @@ eval_staged_kernel(const __grid_constant__ CUtensorMap tmap, Geom g, StagedGeom 
             for (int m1 = 0; m1 < 4; ++m1) {
                 // planes i1+2, i1+3 just before their quarter of the loop
                 if (m1 >= 2) wait_plane(sq + m1);
+                BLIP_ASSERT(sq + m1 < waited && sq + m1 >= released && sq + m1 - released < RU);   // landed, not given back
                 const unsigned pp = plane0 + ((sq + m1) % RU) * (unsigned)Cfg::PLANE_BYTES + off;
 #pragma unroll
                 for (int m2 = 0; m2 < 4; ++m2) {

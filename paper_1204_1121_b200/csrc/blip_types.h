@@ -5,6 +5,24 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 
+// Checked build (-DBLIP_CHECKED; tests/harness builds it as libblipgpu_checked.so): every table
+// row index, sorted-slot, unit, plane and output index the kernels compute is compared with its
+// bound, a violation prints the expression and traps.  It stands in for compute-sanitizer's
+// memcheck on a pool where that tool is closed (profiles/r2_checks.md); the shipped build has none.
+#ifdef BLIP_CHECKED
+#include <cstdio>
+#define BLIP_ASSERT(cond)                                                                      \
+    do {                                                                                       \
+        if (!(cond)) {                                                                         \
+            printf("BLIP_ASSERT failed: %s  (%s:%d, block %d thread %d)\n", #cond, __FILE__, __LINE__, \
+                   (int)blockIdx.x, (int)threadIdx.x);                                         \
+            __trap();                                                                          \
+        }                                                                                      \
+    } while (0)
+#else
+#define BLIP_ASSERT(cond) do { } while (0)
+#endif
+
 namespace blip {
 
 constexpr int kWarpsPerBlock = 8;          // direct kernel: 8 electrons per CTA
@@ -22,6 +40,7 @@ struct Geom {
     int L;              // orbitals
     int pitch4;         // table row pitch in float4 (= ceil(L/4))
     int diag;           // J diagonal (lattice vectors along the Cartesian axes): the kernels' MODE 2
+    long long M;        // positions of the current call (set per launch; read by the BLIP_CHECKED build only)
 };
 
 // Geometry of the staged path: pencils of BY x BZ cells running along axis 1, cut into

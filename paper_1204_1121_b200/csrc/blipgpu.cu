@@ -374,6 +374,7 @@ static int launch_eval(blipgpu_table* t, const double* positions, long long M, i
     if (mode == BLIPGPU_VGH)                                  // full Hessian: the per-position kernel, fp32
         return launch_hess<float>(t, positions, M, val, grad, lap, ld, cell, s);
     const int* perm = nullptr;
+    t->g.M = M;                                              // bound of the checked build's asserts
     const bool staged = use_staged(t, M);
     const int kmode = mode == BLIPGPU_VALUE ? 0 : (t->diag ? 2 : 1);      // kernel template MODE
     if (t->profiling) CK(t, cudaEventRecord(t->pe[0], s));

@@ -9,6 +9,8 @@
  *                                  far more table rows than the L2 holds), so the rows come from
  *                                  HBM, not from a cache warmed by the previous call.  One JSON
  *                                  line on stdout.
+ *   blip_harness fullsize          the TiO2-sized launch configuration (49,152 x 768, staged kernel)
+ *                                  three times through eval / eval_contract: for the checked build.
  *   blip_harness selftest          every kernel once on a small table (staged, direct, split,
  *                                  fp64, contraction; both modes): exit code 0 iff all calls
  *                                  return OK, the results are finite and the staged kernel
@@ -232,10 +234,51 @@ static int run_selftest(void)
     return fails ? 1 : 0;
 }
 
+/* The TiO2-sized shape in the launch configuration bench.py times (49,152 positions x 768
+ * orbitals, staged kernel), three calls of each entry point: for the checked build. */
+static int run_fullsize(void)
+{
+    const double A[9] = {17.4, 0, 0, 0, 17.4, 0, 0, 0, 11.2};
+    const int n[3] = {64, 64, 40};
+    const int L = 768;
+    const long long ld = 768, M = 49152;
+    blipgpu_table* t = make_table(A, n, L);
+    double* hpos = make_positions(A, M, 0.5);
+    double* dpos = NULL;
+    float *val = NULL, *grad = NULL, *lap = NULL, *cout = NULL;
+    CUDA_OK(cudaMalloc((void**)&dpos, sizeof(double) * 3 * (size_t)M));
+    CUDA_OK(cudaMemcpy(dpos, hpos, sizeof(double) * 3 * (size_t)M, cudaMemcpyHostToDevice));
+    CUDA_OK(cudaMalloc((void**)&val, sizeof(float) * (size_t)M * ld));
+    CUDA_OK(cudaMalloc((void**)&grad, sizeof(float) * 3 * (size_t)M * ld));
+    CUDA_OK(cudaMalloc((void**)&lap, sizeof(float) * (size_t)M * ld));
+    CUDA_OK(cudaMalloc((void**)&cout, sizeof(float) * 8 * (size_t)M));
+    int fails = 0;
+    for (int rep = 0; rep < 3; ++rep) {
+        BLIP_OK(blipgpu_eval(t, dpos, M, BLIPGPU_VGL, val, grad, lap, ld, NULL, NULL));
+        BLIP_OK(blipgpu_eval(t, dpos, M, BLIPGPU_VALUE, val, NULL, NULL, ld, NULL, NULL));
+        BLIP_OK(blipgpu_eval_contract(t, dpos, M, BLIPGPU_VGL, lap, ld, cout, NULL, NULL));
+        CUDA_OK(cudaDeviceSynchronize());
+    }
+    printf("fullsize: kernel=%d\n", blipgpu_last_path(t));
+    fails += blipgpu_last_path(t) != 2;
+    {
+        float* h = (float*)malloc(sizeof(float) * (size_t)M * ld);
+        CUDA_OK(cudaMemcpy(h, val, sizeof(float) * (size_t)M * ld, cudaMemcpyDeviceToHost));
+        fails += !all_finite(h, (size_t)M * ld);
+        free(h);
+    }
+    free(hpos);
+    cudaFree(dpos); cudaFree(val); cudaFree(grad); cudaFree(lap); cudaFree(cout);
+    BLIP_OK(blipgpu_destroy(t));
+    printf("fullsize: %d failure(s)\n", fails);
+    return fails ? 1 : 0;
+}
+
 int main(int argc, char** argv)
 {
     if (argc >= 2 && strcmp(argv[1], "latency") == 0) return run_latency(argc >= 3 ? atoi(argv[2]) : 400);
     if (argc >= 2 && strcmp(argv[1], "selftest") == 0) return run_selftest();
-    fprintf(stderr, "usage: %s latency [calls] | selftest\n", argv[0]);
+    if (argc >= 2 && strcmp(argv[1], "fullsize") == 0) return run_fullsize();
+    fprintf(stderr, "usage: %s latency [calls] | selftest | fullsize\n", argv[0]);
     return 64;
 }

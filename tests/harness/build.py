@@ -12,22 +12,33 @@ EXE = os.path.join(HERE, "blip_harness")
 CUDA = os.environ.get("CUDA_HOME", "/usr/local/cuda")
 
 
-def build(force=False):
+def build(force=False, checked=False):
+    """checked=True: the library is compiled with -DBLIP_CHECKED (every index the kernels compute is
+    compared with its bound and a violation traps; csrc/blip_types.h) into
+    tests/harness/libblipgpu_checked.so and the harness is linked against that."""
     if ROOT not in sys.path:
         sys.path.insert(0, ROOT)
     from paper_1204_1121_b200 import _build
-    lib = _build.build()
+    if checked:
+        lib = os.path.join(HERE, "libblipgpu_checked.so")
+        if force or not os.path.exists(lib) or any(os.path.getmtime(d) > os.path.getmtime(lib) for d in _build.DEPS):
+            subprocess.run([_build.nvcc(), *_build.NVCC_FLAGS, "-DBLIP_CHECKED", "-I", os.path.join(ROOT, "include"),
+                            "-o", lib, *_build.SOURCES], check=True)
+        exe, name = EXE + "_checked", "blipgpu_checked"
+    else:
+        lib = _build.build()
+        exe, name = EXE, "blipgpu"
     libdir = os.path.dirname(lib)
     deps = [SRC, lib, os.path.join(ROOT, "include", "blipgpu.h"), os.path.join(ROOT, "include", "blipgpu_dev.h")]
-    if not force and os.path.exists(EXE) and all(os.path.getmtime(EXE) >= os.path.getmtime(d) for d in deps):
-        return EXE
+    if not force and os.path.exists(exe) and all(os.path.getmtime(exe) >= os.path.getmtime(d) for d in deps):
+        return exe
     cmd = ["gcc", "-O2", "-std=c11", "-D_POSIX_C_SOURCE=200809L", "-Wall", "-Wextra", "-I", os.path.join(ROOT, "include"),
-           "-I", os.path.join(CUDA, "include"), "-o", EXE, SRC, "-L", libdir, "-lblipgpu",
+           "-I", os.path.join(CUDA, "include"), "-o", exe, SRC, "-L", libdir, "-l" + name,
            "-L", os.path.join(CUDA, "lib64"), "-lcudart", "-lm",
            "-Wl,-rpath," + libdir, "-Wl,-rpath," + os.path.join(CUDA, "lib64")]
     subprocess.run(cmd, check=True)
-    return EXE
+    return exe
 
 
 if __name__ == "__main__":
-    print(build(force=True))
+    print(build(force=True, checked="--checked" in sys.argv))

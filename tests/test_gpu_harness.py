@@ -30,6 +30,20 @@ def test_harness_selftest():
 
 
 @pytest.mark.gpu
+def test_harness_selftest_on_the_checked_build():
+    """The same self-test against the library compiled with -DBLIP_CHECKED: every table row, sorted
+    slot, unit, staged plane and output index is compared with its bound inside the kernels and a
+    violation traps (the stand-in for compute-sanitizer memcheck, which is closed on this pool)."""
+    exe = harness_build.build(checked=True)
+    r = subprocess.run([exe, "selftest"], capture_output=True, text=True, timeout=900)
+    assert r.returncode == 0, r.stdout + r.stderr
+    assert "selftest: 0 failure(s)" in r.stdout and "BLIP_ASSERT" not in r.stdout + r.stderr
+    r = subprocess.run([exe, "fullsize"], capture_output=True, text=True, timeout=900)
+    assert r.returncode == 0, r.stdout + r.stderr
+    assert "fullsize: 0 failure(s)" in r.stdout and "BLIP_ASSERT" not in r.stdout + r.stderr
+
+
+@pytest.mark.gpu
 def test_harness_latency_rows():
     r = subprocess.run([harness_build.build(), "latency", "60"], capture_output=True, text=True, timeout=900)
     assert r.returncode == 0, r.stdout + r.stderr
