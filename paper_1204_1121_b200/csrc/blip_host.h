@@ -37,6 +37,7 @@ struct blipgpu_table {
     unsigned* counters = nullptr;    // [4][nbins], zero at creation
     unsigned* gstate = nullptr;      // [2] {barrier arrivals, barrier generation}
     int fused_ok = 0;                // cooperative launch available and the histogram fits in shared memory
+    long long fused_room = 0;        // dynamic shared memory the grouping kernel may use
     // complex orbitals (blipgpu_set_kpoints): Cartesian k of complex orbital m, device [L/2][3] fp64
     double* kvec = nullptr;
     // staging for blipgpu_eval_host (device)

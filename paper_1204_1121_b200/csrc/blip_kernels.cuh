@@ -397,7 +397,7 @@ __device__ __forceinline__ void warp_prepare(const Geom& g, const double* __rest
 // staged kernel once per orbital chunk), written to slot s of the sorted order.
 __device__ __forceinline__ void write_staged_record(const Geom& g, const StagedGeom& sg, int tile_floats,
                                                     const double* __restrict__ pos, int e, unsigned s,
-                                                    float4* __restrict__ recs)
+                                                    float4* recs, int pitch4 = kRecFloats / 4)
 {
     const double x = pos[3 * (size_t)e], y = pos[3 * (size_t)e + 1], z = pos[3 * (size_t)e + 2];
     float ax[3][3][4]; int ic[3];
@@ -409,7 +409,7 @@ __device__ __forceinline__ void write_staged_record(const Geom& g, const StagedG
 #pragma unroll
         for (int m = 0; m < 4; ++m) phi_site(fa, m, ax[a][0][m], ax[a][1][m], ax[a][2][m]);
     }
-    float4* out = recs + (size_t)s * (kRecFloats / 4);
+    float4* out = recs + (size_t)s * pitch4;
     float lb[16];
 #pragma unroll
     for (int col = 0; col < 16; ++col) {
@@ -474,9 +474,9 @@ __global__ void __launch_bounds__(kScanThreads, 1)
 group_kernel(Geom g, StagedGeom sg, int tile_floats, const double* __restrict__ pos, long long M,
              unsigned* __restrict__ counters /* [4][nalloc] */, int nalloc, int nbins, unsigned* __restrict__ gstate,
              int4* __restrict__ order, int* __restrict__ meta, float4* __restrict__ recs, int* __restrict__ perm,
-             int* __restrict__ cell)
+             int* __restrict__ cell, int nstage)
 {
-    extern __shared__ __align__(16) unsigned start[];        // [nbins + 1] exclusive scan of the counts
+    extern __shared__ __align__(16) unsigned start[];        // [nbins + 1] exclusive scan of the counts, then record staging
     __shared__ unsigned wsum[kScanThreads / 32];
     __shared__ unsigned keybuf[STAGED ? kScanChunk : 1];   // CTA 0 of the staged form sorts the work items here
     __shared__ int nonempty;
@@ -579,14 +579,30 @@ group_kernel(Geom g, StagedGeom sg, int tile_floats, const double* __restrict__ 
     const long long share = (M + nc - 1) / nc;
     const long long e0 = (long long)(blockIdx.x - first) * share, e1 = min(e0 + share, M);
     if (STAGED) {
-        // a thread per electron: every electron of the CTA's share is in flight at once (position
-        // load, fp64 cell map, slot atomic, weights, 24 float4 stores)
-        for (long long e = e0 + tid; e < e1; e += kScanThreads) {
-            int ic[3];
-            const int b = bin_of(e, ic);
-            const unsigned slot = start[b] + atomicAdd(&cursor[b], 1u);
-            BLIP_ASSERT(slot < start[b + 1] && (long long)slot < M);
-            write_staged_record(g, sg, tile_floats, pos, (int)e, slot, recs);
+        // A thread per electron (position load, fp64 cell map, slot atomic, weights: every electron
+        // of the round in flight at once) builds its record in shared memory — 24 float4 per thread
+        // straight to global memory would be 24 stores of 32 scattered 16-byte pieces per warp, and
+        // took 9 us — and then the whole CTA copies the records out, 384 contiguous bytes each.
+        constexpr int RW = kRecFloats / 4 + 1;               // float4 per staged record: 24 + 1 pad (bank spread)
+        float4* stage = reinterpret_cast<float4*>(start + (((size_t)nbins + 1 + 3) & ~(size_t)3));
+        unsigned* slots = reinterpret_cast<unsigned*>(stage + (size_t)nstage * RW);
+        for (long long r0 = e0; r0 < e1; r0 += nstage) {
+            const int nr = (int)min((long long)nstage, e1 - r0);
+            for (int r = tid; r < nr; r += kScanThreads) {
+                const long long e = r0 + r;
+                int ic[3];
+                const int b = bin_of(e, ic);
+                const unsigned slot = start[b] + atomicAdd(&cursor[b], 1u);
+                BLIP_ASSERT(slot < start[b + 1] && (long long)slot < M);
+                slots[r] = slot;
+                write_staged_record(g, sg, tile_floats, pos, (int)e, (unsigned)r, stage, RW);
+            }
+            __syncthreads();
+            for (int i = tid; i < nr * (kRecFloats / 4); i += kScanThreads) {
+                const int r = i / (kRecFloats / 4), q = i - r * (kRecFloats / 4);
+                recs[(size_t)slots[r] * (kRecFloats / 4) + q] = stage[(size_t)r * RW + q];
+            }
+            __syncthreads();
         }
     } else {
         for (long long e = e0 + tid; e < e1; e += kScanThreads) {

@@ -290,8 +290,9 @@ extern "C" int blipgpu_create(const double* lattice, const int* grid, int norb,
         // one-launch grouping: needs a cooperative launch of one 1,024-thread CTA per SM and the
         // histogram (+ 1 word) in dynamic shared memory next to the kernel's static 33 KB
         int coop = 0;
-        const size_t need = sizeof(unsigned) * ((size_t)t->nbins + 1);
+        const size_t need = sizeof(unsigned) * ((size_t)t->nbins + 8) + 64 * 404;      // histogram + room to stage 64 records
         const size_t room = (size_t)prop.sharedMemPerBlockOptin - 40 * 1024;    // the attribute is per function, not per table: always the maximum
+        t->fused_room = (long long)room;
         if (cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, dev) == cudaSuccess && coop && need <= room &&
             cudaFuncSetAttribute(blip::group_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)room) == cudaSuccess &&
             cudaFuncSetAttribute(blip::group_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)room) == cudaSuccess)
@@ -388,17 +389,25 @@ static int launch_eval(blipgpu_table* t, const double* positions, long long M, i
             // a-4 in one cooperative launch (blip::group_kernel): count, grid barrier, scan + scatter
             cudaLaunchConfig_t cfg = {};
             cfg.gridDim = dim3((unsigned)t->nsm); cfg.blockDim = dim3(blip::kScanThreads);
-            cfg.dynamicSmemBytes = sizeof(unsigned) * ((size_t)nbins + 1); cfg.stream = s;
+            // dynamic shared memory: the histogram scan, then (staged form) as many 400-byte records
+            // as fit, up to the CTA's share of the batch, + their slots
+            const size_t hist_bytes = sizeof(unsigned) * (((size_t)nbins + 1 + 3) & ~(size_t)3);
+            const long long share = (M + t->nsm - 2) / (t->nsm > 1 ? t->nsm - 1 : 1);
+            long long nstage = ((long long)t->fused_room - (long long)hist_bytes) / (400 + 4);
+            if (nstage > share) nstage = share;
+            if (nstage < 1) nstage = 1;
+            cfg.dynamicSmemBytes = staged ? hist_bytes + (size_t)nstage * (400 + 4) : hist_bytes;
+            cfg.stream = s;
             cudaLaunchAttribute attr[1];
             attr[0].id = cudaLaunchAttributeCooperative;
             attr[0].val.cooperative = 1;
             cfg.attrs = attr; cfg.numAttrs = 1;
             if (staged)
                 CK(t, cudaLaunchKernelEx(&cfg, blip::group_kernel<true>, t->g, t->sg, (int)kSC, positions, M, t->counters, t->nbins,
-                                         nbins, t->gstate, t->order, t->meta, t->recs, t->perm, cell));
+                                         nbins, t->gstate, t->order, t->meta, t->recs, t->perm, cell, (int)nstage));
             else
                 CK(t, cudaLaunchKernelEx(&cfg, blip::group_kernel<false>, t->g, t->sg, (int)kSC, positions, M, t->counters, t->nbins,
-                                         nbins, t->gstate, t->order, t->meta, t->recs, t->perm, cell));
+                                         nbins, t->gstate, t->order, t->meta, t->recs, t->perm, cell, 0));
             t->launches += 1;
         } else {
         // three launches (tables whose histogram does not fit in shared memory).
