@@ -32,6 +32,14 @@ def stale():
 
 
 def build(force=False, verbose=False):
+    # BLIPGPU_LIBRARY (read here, by the Python binding, not by the library): load this build of the
+    # same ABI instead, e.g. tests/harness/libblipgpu_checked.so to run the GPU suite with the
+    # kernels' bounds asserts on (profiles/r2_checks.md)
+    override = os.environ.get("BLIPGPU_LIBRARY")
+    if override:
+        if not os.path.exists(override):
+            raise FileNotFoundError(f"BLIPGPU_LIBRARY={override} does not exist")
+        return override
     if not force and not stale():
         return LIB
     cmd = [nvcc(), *NVCC_FLAGS, "-I", os.path.join(ROOT, "include"), "-o", LIB, *SOURCES]
