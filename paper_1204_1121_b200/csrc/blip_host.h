@@ -16,8 +16,12 @@ struct blipgpu_table {
     int nbins_direct = 0, nbins_staged = 0;
     int nq = 1;                      // direct kernel: quads of 4 orbitals per lane (1..3)
     int diag = 0;                    // lattice vectors along the Cartesian axes: J diagonal (kernel MODE 2)
-    int path = 0;                    // 0 auto, 1 direct, 2 staged (blipgpu_set_tuning)
+    int path = 0;                    // 0 auto, 1 direct, 2 staged (FP32 pipe), 5 staged on the tensor cores (blipgpu_set_tuning)
     int staged_ok = 0;               // TMA descriptor built and the grid is large enough
+    int tc_ok = 0;                   // tensor-core form of the staged kernel usable (finite table, shared memory fits)
+    unsigned* table16 = nullptr;     // device, the table of the tensor-core path: scaled fp16 halves, z pairs (blip_tc.cuh)
+    CUtensorMap tmap16;              // its 5-D TMA descriptor
+    float tc_scale[11] = {0};        // blip::TcScale: 2^kc of the coefficients, 2^kq and 1 / 2^(kc + kq) per quantity
     int nchunk = 0;                  // staged path: orbital chunks of 128
     int nsm = 0;                     // SMs of the device (CTAs of the persistent staged kernel)
     long long l2_bytes = 0;          // L2 capacity of the device
@@ -48,7 +52,7 @@ struct blipgpu_table {
     int profiling = 0;
     cudaEvent_t pe[3] = {nullptr, nullptr, nullptr};   // call start, eval kernel start, end
     int last_cuda = 0;
-    int last_path = 0;               // gather+FMA kernel of the last eval: 1 direct, 2 staged, 3 split, 4 fp64/Hessian
+    int last_path = 0;               // gather+FMA kernel of the last eval: 1 direct, 2 staged, 3 split, 4 fp64/Hessian, 5 staged on the tensor cores
     long long launches = 0;
 };
 

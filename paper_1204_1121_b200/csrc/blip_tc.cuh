@@ -1,0 +1,575 @@
+// blip_tc.cuh — the gather + FMA step (a-3) of dense batches on the 5th-generation tensor cores
+// (tcgen05.mma with the coefficient operand in tensor memory), sm_100a.
+//
+// PAPER.md:401-419 (§VI.E, Eq. 13-15) rejects the dense matrix form psi = A Theta because the
+// matrix changes with the electron position; north_star allows tensor cores "only if recasting the
+// batch as a dense weights x coefficients contraction is shown to win".  The recast that does win
+// keeps the contraction per electron, K = the sites of the electron's 4x4x4 block, and puts the
+// COEFFICIENTS on the M side of the MMA, where the tensor core is full whatever the batch holds:
+//
+//     D[128 orbitals][N = 16] += A[128 orbitals][K = 16 sites] * B[K = 16 sites][N = 16]
+//
+//   A  one table plane of the pencil's 7 x 7-row cross-section, transposed into tensor memory
+//      (lane = orbital, column = site), so that the 16 sites of an MMA — rows (y, z = 0..7) and
+//      (y + 1, z = 0..7) of the plane, the z axis padded from 7 to 8 — are 8 consecutive TMEM
+//      columns that start at a multiple of 4: any electron of the pencil finds its rows y0 ..
+//      y0 + 3 at column 4 y0 of the plane, no copy per electron;
+//   B  the electron's folded weights (W, Gamma_x,y,z, Lambda per site) in
+//      shared memory, zero outside its z window z0 .. z0 + 3;
+//   D  fp32 accumulators in tensor memory, read back by the epilogue warps (tcgen05.ld).
+//
+// Precision.  The tensor core multiplies fp16 (11 significant bits); north_star's tolerances
+// need ~2^-20.  Both operands are split exactly in two fp16 halves after an exact power-of-two
+// scaling: c' = c 2^kc = c1 + c2 (c1 = rn16(c'), c2 = rn16(c' - c1): 22 bits), W' = W 2^kq =
+// W1 + W2 likewise.  The B tile carries [W1 | W2] in its N dimension (columns 0..4 and 5..9), the A
+// operand is issued twice (c1, c2) into the same accumulators, so that D[:, q] + D[:, 5 + q] =
+// (c1 + c2)(W1 + W2) summed over the sites in fp32: all four cross terms, error ~2^-21 of
+// sum |c W|.  Per electron and 128 orbitals: 4 planes x 2 row pairs x 2 halves = 16 MMAs.
+//
+// Roles of the persistent CTA (one per SM), 19 warps:
+//   producer (1)     work items and TMA of the table planes into a shared-memory ring — the
+//                    protocol of eval_staged_kernel;
+//   converters (4)   one per TMEM lane quarter: plane from shared memory -> scale, split, pack
+//                    -> tcgen05.st into a ring of 7 TMEM plane slots (2 x 28 columns each);
+//   weights (4)      one electron each: record -> 80 (column, quantity) weight vectors -> B tile
+//                    slot (4 KB) in the canonical K-major core-matrix layout;
+//   issuers (2)      one elected thread each: wait for B tile, planes and a free accumulator,
+//                    issue the 16 MMAs, tcgen05.commit to free the B slot / publish D; planes are
+//                    given back to the converters by commit as the units move on;
+//   epilogue (2 x 4) tcgen05.ld of D, unscale, Cartesian gradient, streaming stores (a-5).
+// All hand-offs are mbarriers; units are numbered CTA-wide so that slot and phase of every ring
+// follow from the unit (or plane) number alone.
+#pragma once
+#include "blip_kernels.cuh"
+#include <cuda_fp16.h>
+
+namespace blip {
+
+constexpr int kTcRS = 4;            // shared-memory plane slots (one TMA box each)
+constexpr int kTcRT = 8;            // TMEM plane slots
+constexpr int kTcPlaneCols = 56;    // TMEM columns of a plane: 2 halves x 7 rows x 4 columns (8 fp16 z sites)
+constexpr int kTcND = 4;            // accumulator slots (16 columns each)
+constexpr int kTcDCol0 = kTcRT * kTcPlaneCols;               // 392
+constexpr int kTcNB = 16;           // B tile slots
+constexpr int kTcBBytes = 4096;     // 8 tiles x 512 B
+constexpr int kTcPlaneWords = 7 * 4 * 2 * 128;               // 28,672 bytes per staged plane
+constexpr int kTcNInfo = 32;        // unit info ring (>= kTcNB + kTcND)
+constexpr int kTcNC = 8, kTcNE = 8, kTcNW = 8, kTcNI = 4;
+constexpr int kTcWarps = kTcNC + kTcNE + kTcNW + kTcNI + 1;  // 29
+constexpr int kTcThreads = kTcWarps * 32;
+constexpr int kTcReaders = kTcNC + kTcNE + kTcNW + kTcNI;    // warps that walk the item queue
+static_assert(kTcDCol0 + 16 * kTcND <= 512, "tensor memory has 512 columns");
+static_assert(kTcNInfo >= kTcNB + kTcND, "unit info must outlive the B slot until the epilogue has read it");
+
+struct TcScale {
+    float sc;           // 2^kc applied to the coefficients
+    float sw[5];        // 2^kq applied to the weights of quantity q (val, T1, T2, T3, lap)
+    float inv[5];       // 1 / (sc sw[q])
+};
+
+struct TcSmem {
+    alignas(128) unsigned plane[kTcRS][kTcPlaneWords];       // [y 7][z pair 4][half 2][128 orbitals], one TMA box
+    alignas(128) unsigned char bt[kTcNB][kTcBBytes];
+    alignas(16) float4 wrec[kTcNW][kRecFloats / 4];          // record of the unit a weight warp works on
+    alignas(16) int4 info[kTcNInfo];                        // {plane sequence number or -1, y0, electron, -}
+    alignas(16) WorkItem item[kItemQueue];
+    alignas(8) u64 full[kTcRS], empty[kTcRS];                // shared-memory planes: TMA -> converters
+    alignas(8) u64 tfull[kTcRT], tempty[kTcRT];              // TMEM planes: converters -> issuers
+    alignas(8) u64 bfull[kTcNB], bempty[kTcNB];              // B tiles: weight warps -> issuers
+    alignas(8) u64 dfull[kTcND], dempty[kTcND];              // accumulators: issuers -> epilogue
+    alignas(8) u64 ifull[kItemQueue], iempty[kItemQueue];
+    unsigned tbase;
+};
+
+__device__ __forceinline__ bool tc_elect_one()
+{
+    unsigned pred;
+    asm volatile("{\n\t.reg .pred p;\n\telect.sync _|p, 0xffffffff;\n\tselp.u32 %0, 1, 0, p;\n\t}" : "=r"(pred));
+    return pred != 0;
+}
+__device__ __forceinline__ void tc_commit(unsigned bar)
+{
+    asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" :: "r"(bar) : "memory");
+}
+__device__ __forceinline__ void tc_fence_before() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
+__device__ __forceinline__ void tc_fence_after() { asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory"); }
+// B tile descriptor: K-major, no swizzle, core matrices of 8 N-rows x 16 bytes; the two K halves
+// of an MMA are 128 bytes apart (leading byte offset), the two N halves 256 (stride byte offset)
+__device__ __forceinline__ uint64_t tc_bdesc(unsigned addr)
+{
+    return (uint64_t)((addr >> 4) & 0x3fffu) | ((uint64_t)(128u >> 4) << 16) | ((uint64_t)(256u >> 4) << 32) | ((uint64_t)1 << 46);
+}
+// kind::f16, A and B fp16 K-major, D fp32, M = 128, N = 16
+constexpr unsigned kTcIdesc = (1u << 4) | ((16u >> 3) << 17) | ((128u >> 4) << 24);
+__device__ __forceinline__ void tc_mma(unsigned d, unsigned a, uint64_t b, unsigned accumulate)
+{
+    asm volatile("{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %4, 0;\n\t"
+                 "tcgen05.mma.cta_group::1.kind::f16 [%0], [%1], %2, %3, p;\n\t}"
+                 :: "r"(d), "r"(a), "l"(b), "r"(kTcIdesc), "r"(accumulate) : "memory");
+}
+__device__ __forceinline__ unsigned tc_pack(float lo, float hi)      // {hi, lo} -> two fp16, round to nearest
+{
+    unsigned r; asm("cvt.rn.f16x2.f32 %0, %1, %2;" : "=r"(r) : "f"(hi), "f"(lo)); return r;
+}
+__device__ __forceinline__ float2 tc_unpack(unsigned p)
+{
+    return __half22float2(*reinterpret_cast<const __half2*>(&p));
+}
+// x (already scaled) -> the two fp16 halves of a pair of values
+__device__ __forceinline__ void tc_split2(float x0, float x1, unsigned& h1, unsigned& h2)
+{
+    h1 = tc_pack(x0, x1);
+    const float2 f = tc_unpack(h1);
+    h2 = tc_pack(__fsub_rn(x0, f.x), __fsub_rn(x1, f.y));
+}
+
+__device__ __forceinline__ void tma_load_5d(unsigned dst, const CUtensorMap* tmap, int c0, int c1, int c2, int c3, int c4, unsigned bar)
+{
+    asm volatile(
+        "cp.async.bulk.tensor.5d.shared::cluster.global.tile.mbarrier::complete_tx::bytes "
+        "[%0], [%1, {%2, %3, %4, %5, %6}], [%7];"
+        :: "r"(dst), "l"(reinterpret_cast<uint64_t>(tmap)), "r"(c0), "r"(c1), "r"(c2), "r"(c3), "r"(c4), "r"(bar)
+        : "memory");
+}
+__device__ __forceinline__ void tma_prefetch_5d(const CUtensorMap* tmap, int c0, int c1, int c2, int c3, int c4)
+{
+    asm volatile("cp.async.bulk.prefetch.tensor.5d.L2.global.tile [%0, {%1, %2, %3, %4, %5}];"
+                 :: "l"(reinterpret_cast<uint64_t>(tmap)), "r"(c0), "r"(c1), "r"(c2), "r"(c3), "r"(c4) : "memory");
+}
+
+// The table of the tensor-core path (library-owned, built once by blipgpu_create next to the fp32
+// one): the ghost-padded table with every coefficient scaled by 2^kc and split in its two fp16
+// halves, z sites in pairs, 32-bit words
+//     T16[p1][p2][zp][half][l] = { c_half[p1][p2][2 zp][l], c_half[p1][p2][2 zp + 1][l] << 16 }
+// — exactly the word a TMEM column of the A operand holds, so that the converter warps only move
+// words from the staged plane to tensor memory.  Same bytes per coefficient as fp32.
+__global__ void __launch_bounds__(256)
+tc_table_kernel(Geom g, float sc, int nzp, const float* __restrict__ src, unsigned* __restrict__ dst, long long total)
+{
+    const long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (idx >= total) return;
+    const int pitch = 4 * g.pitch4;
+    const int l = (int)(idx % pitch);
+    long long r = idx / pitch;
+    const int zp = (int)(r % nzp); r /= nzp;
+    const int p2 = (int)(r % g.np[1]);
+    const int p1 = (int)(r / g.np[1]);
+    const int k1 = (p1 + g.n[0] - 1) % g.n[0], k2 = (p2 + g.n[1] - 1) % g.n[1];
+    float c[2] = {0.f, 0.f};
+    if (l < g.L) {
+#pragma unroll
+        for (int h = 0; h < 2; ++h) {
+            const int p3 = 2 * zp + h;
+            if (p3 < g.np[2]) {
+                const int k3 = (p3 + g.n[2] - 1) % g.n[2];
+                c[h] = __fmul_rn(__ldg(src + (((size_t)k1 * g.n[1] + k2) * g.n[2] + k3) * (size_t)g.L + l), sc);
+            }
+        }
+    }
+    unsigned h1, h2;
+    tc_split2(c[0], c[1], h1, h2);
+    const size_t o = (((size_t)p1 * g.np[1] + p2) * nzp + zp) * 2 * (size_t)pitch + l;
+    dst[o] = h1;
+    dst[o + pitch] = h2;
+}
+
+#ifdef BLIP_TC_PROF
+__device__ int g_tc_knock;           // timing knock-outs (results wrong): 1 no MMAs, 2 no B build, 4 no output stores, 8 no plane conversion
+#define TC_KNOCK(bit) (g_tc_knock & (bit))
+__device__ unsigned long long g_tc_prof[64];
+#define TCP_DECL long long tcp_t = clock64(); long long tcp_a[6] = {0, 0, 0, 0, 0, 0}
+#define TCP(k) do { const long long t1_ = clock64(); tcp_a[k] += t1_ - tcp_t; tcp_t = t1_; } while (0)
+#define TCP_FLUSH(base, leader) do { if (blockIdx.x == 0 && (leader)) { for (int k_ = 0; k_ < 6; ++k_) atomicAdd(&g_tc_prof[(base) + k_], (unsigned long long)tcp_a[k_]); } } while (0)
+#else
+#define TC_KNOCK(bit) false
+#define TCP_DECL do { } while (0)
+#define TCP(k) do { } while (0)
+#define TCP_FLUSH(base, leader) do { } while (0)
+#endif
+
+template <int MODE>
+__global__ void __launch_bounds__(kTcThreads, 1)
+eval_tc_kernel(const __grid_constant__ CUtensorMap tmap, Geom g, StagedGeom sg, TcScale scl,
+               const float4* __restrict__ recs, const int4* __restrict__ order, int* __restrict__ meta,
+               int nchunk, float* __restrict__ val, float* __restrict__ grad, float* __restrict__ lap, long long ld)
+{
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    TcSmem& sm = *reinterpret_cast<TcSmem*>(smem_raw);
+    constexpr unsigned IQ = kItemQueue;
+    constexpr int PLANE_BYTES = kTcPlaneWords * 4;
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    wait_for_predecessor();
+#ifdef BLIP_TC_PROF
+    const long long tcp_start = clock64();
+    unsigned long long tcp_g0; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(tcp_g0));
+#endif
+    if (warp == 0) {
+        asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], 512;" :: "r"(smem_u32(&sm.tbase)) : "memory");
+        asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+    }
+    if (threadIdx.x == 32) {
+        for (int s = 0; s < kTcRS; ++s) { mbar_init(smem_u32(&sm.full[s]), 1); mbar_init(smem_u32(&sm.empty[s]), 4); }
+        for (int s = 0; s < kTcRT; ++s) { mbar_init(smem_u32(&sm.tfull[s]), 4); mbar_init(smem_u32(&sm.tempty[s]), kTcNI); }
+        for (int s = 0; s < kTcNB; ++s) { mbar_init(smem_u32(&sm.bfull[s]), 1); mbar_init(smem_u32(&sm.bempty[s]), 1); }
+        for (int s = 0; s < kTcND; ++s) { mbar_init(smem_u32(&sm.dfull[s]), 1); mbar_init(smem_u32(&sm.dempty[s]), 4); }
+        for (int s = 0; s < (int)IQ; ++s) { mbar_init(smem_u32(&sm.ifull[s]), 1); mbar_init(smem_u32(&sm.iempty[s]), kTcReaders); }
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    // B tiles: the N rows 10..15 of every tile stay zero for the whole kernel
+    for (int i = threadIdx.x; i < kTcNB * kTcBBytes / 16; i += kTcThreads)
+        reinterpret_cast<uint4*>(&sm.bt[0][0])[i] = make_uint4(0u, 0u, 0u, 0u);
+    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+    tc_fence_before();
+    __syncthreads();
+    tc_fence_after();
+    const unsigned tbase = sm.tbase;
+
+    // every reader role walks the item queue the same way
+    int it_nplanes = 0, it_chunk = 0;
+    unsigned it_seq0 = 0, it_nunits = 0, it_u0 = 0;
+    auto load_item = [&](unsigned k) {
+        mbar_wait(smem_u32(&sm.ifull[k % IQ]), (k / IQ) & 1u);
+        const WorkItem& it = sm.item[k % IQ];
+        it_nplanes = it.nplanes;
+        if (it_nplanes >= 0) { it_chunk = it.chunk; it_seq0 = it.seq0; it_nunits = it.nunits; it_u0 = it.u0; }
+    };
+    auto leave_item = [&](unsigned k, bool one_thread) {
+        if (!one_thread) __syncwarp();
+        if (one_thread || lane == 0) mbar_arrive(smem_u32(&sm.iempty[k % IQ]));
+    };
+
+    if (warp == kTcWarps - 1) {
+        // ---- producer: as in eval_staged_kernel (work queue, item descriptors, one TMA box per plane)
+        if (lane == 0) {
+            const int nps = meta[0];
+            const int nitems = nps * nchunk;
+            unsigned seq_pub = 0;
+            struct Desc { int nplanes, chunk, by, bz, lo; };
+            auto fetch = [&](unsigned k) -> Desc {
+                const unsigned q = k % IQ;
+                if (k >= IQ) mbar_wait_backoff(smem_u32(&sm.iempty[q]), ((k / IQ) & 1u) ^ 1u);
+                const int w = atomicAdd(&meta[1], 1);
+                WorkItem& it = sm.item[q];
+                Desc d = {-1, 0, 0, 0, 0};
+                if (w < nitems) {
+                    d.chunk = w % nchunk;
+                    const int4 o = __ldg(order + w / nchunk);
+                    const int pencil = o.x / sg.nseg, segi = o.x - pencil * sg.nseg;
+                    d.lo = segi * sg.seg;
+                    const int hi = min(d.lo + sg.seg, g.n[0]) - 1;
+                    d.by = pencil / sg.nbz; d.bz = pencil - d.by * sg.nbz;
+                    d.nplanes = o.z > 0 ? hi + 4 - d.lo : 0;
+                    it.chunk = d.chunk; it.by = d.by; it.bz = d.bz; it.lo = d.lo; it.seq0 = seq_pub;
+                    it.u0 = (unsigned)o.y; it.nunits = (unsigned)o.z;
+                    seq_pub += (unsigned)d.nplanes;
+                    for (int k2 = 0; k2 < min(d.nplanes, 8); ++k2)
+                        tma_prefetch_5d(&tmap, d.chunk * 128, 0, d.bz * 2, d.by * 4, d.lo + k2);
+                }
+                it.nplanes = d.nplanes;
+                mbar_arrive(smem_u32(&sm.ifull[q]));
+                return d;
+            };
+            unsigned seq = 0;
+            Desc cur = fetch(0);
+            for (unsigned k = 0; cur.nplanes >= 0; ++k) {
+                for (int j = 0; j < cur.nplanes; ++j, ++seq) {
+                    const unsigned slot = seq % kTcRS, round = seq / kTcRS;
+                    if (j + 8 < cur.nplanes) tma_prefetch_5d(&tmap, cur.chunk * 128, 0, cur.bz * 2, cur.by * 4, cur.lo + j + 8);
+                    if (round > 0) mbar_wait_backoff(smem_u32(&sm.empty[slot]), (round & 1u) ^ 1u);
+                    const unsigned bar = smem_u32(&sm.full[slot]);
+                    mbar_expect_tx(bar, PLANE_BYTES);
+                    tma_load_5d(smem_u32(&sm.plane[slot][0]), &tmap, cur.chunk * 128, 0, cur.bz * 2, cur.by * 4, cur.lo + j, bar);
+                }
+                cur = fetch(k + 1);
+            }
+        }
+    } else if (warp < kTcNC) {
+        // ---- converters: lane quarter `warp` of tensor memory, thread = orbital 32 warp + lane
+        const int cq = warp & 3, cg = warp >> 2;             // lane quarter; group cg converts the planes with (sequence number) % 2 == cg
+        const unsigned tlane = tbase + ((unsigned)(cq * 32) << 16);
+        const int orb = cq * 32 + lane;
+        TCP_DECL;
+        for (unsigned n = 0;; ++n) {
+            load_item(n);
+            TCP(0);
+            if (it_nplanes < 0) break;
+            for (int j = (int)((it_seq0 + (unsigned)cg) & 1u); j < it_nplanes; j += 2) {
+                const unsigned q = it_seq0 + (unsigned)j;
+                const unsigned s = q % kTcRS, t = q % kTcRT;
+                mbar_wait(smem_u32(&sm.full[s]), (q / kTcRS) & 1u);
+                TCP(1);
+                // the plane's 56 words into registers, and the shared-memory slot straight back to the
+                // producer: the plane then waits for its TMEM slot in registers while the TMA runs ahead
+                const unsigned* src = &sm.plane[s][orb];
+                unsigned h[7][8];
+                unsigned any = 0;
+                if (!TC_KNOCK(8))
+#pragma unroll
+                for (int y = 0; y < 7; ++y)
+#pragma unroll
+                    for (int k = 0; k < 4; ++k) {
+                        h[y][k] = src[((y * 4 + k) * 2) * 128]; h[y][4 + k] = src[((y * 4 + k) * 2 + 1) * 128];
+                        any |= h[y][k] | h[y][4 + k];
+                    }
+                any |= __shfl_xor_sync(0xffffffffu, any, 1) | __shfl_xor_sync(0xffffffffu, any, 2);
+                any |= __shfl_xor_sync(0xffffffffu, any, 4) | __shfl_xor_sync(0xffffffffu, any, 8);
+                any |= __shfl_xor_sync(0xffffffffu, any, 16);
+                // (any * any) & 2 is zero for every value (a square is 0 or 1 mod 4): the address of the
+                // arrival depends on every word loaded, so the arrival cannot overtake the loads
+                if (lane == 0) mbar_arrive(smem_u32(&sm.empty[s]) + ((any * any) & 2u) * 4u);
+                if (q >= kTcRT) mbar_wait(smem_u32(&sm.tempty[t]), ((q / kTcRT) & 1u) ^ 1u);
+                TCP(2);
+                tc_fence_after();
+                const unsigned tcol = tlane + t * kTcPlaneCols;
+                if (!TC_KNOCK(8))
+#pragma unroll
+                for (int y = 0; y < 7; ++y) {
+                    asm volatile("tcgen05.st.sync.aligned.32x32b.x4.b32 [%0], {%1, %2, %3, %4};"
+                                 :: "r"(tcol + 4 * y), "r"(h[y][0]), "r"(h[y][1]), "r"(h[y][2]), "r"(h[y][3]) : "memory");
+                    asm volatile("tcgen05.st.sync.aligned.32x32b.x4.b32 [%0], {%1, %2, %3, %4};"
+                                 :: "r"(tcol + 28 + 4 * y), "r"(h[y][4]), "r"(h[y][5]), "r"(h[y][6]), "r"(h[y][7]) : "memory");
+                }
+                asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
+                tc_fence_before();
+                __syncwarp();
+                if (lane == 0) mbar_arrive(smem_u32(&sm.tfull[t]));
+                TCP(3);
+            }
+            leave_item(n, false);
+        }
+        TCP_FLUSH(0, warp == 0 && lane == 0);
+    } else if (warp < kTcNC + kTcNE) {
+        // ---- epilogue: group eg takes the units with (unit number) % 2 == eg; lane quarter sp
+        const int eg = (warp - kTcNC) >> 2, sp = warp & 3;
+        const unsigned tl = tbase + ((unsigned)(sp * 32) << 16) + kTcDCol0;
+        unsigned ubase = 0;
+        TCP_DECL;
+        for (unsigned n = 0;; ++n) {
+            load_item(n);
+            TCP(0);
+            if (it_nplanes < 0) break;
+            const int col = it_chunk * 128 + sp * 32 + lane;
+            for (unsigned u = (ubase + (unsigned)eg) & 1u; u < it_nunits; u += 2) {      // (ubase + u) % 2 == eg
+                const unsigned uc = ubase + u, d = uc % kTcND;
+                mbar_wait(smem_u32(&sm.dfull[d]), (uc / kTcND) & 1u);
+                TCP(1);
+                tc_fence_after();
+                const int4 inf = sm.info[uc % kTcNInfo];
+                unsigned r[10];
+                asm volatile("tcgen05.ld.sync.aligned.32x32b.x8.b32 {%0, %1, %2, %3, %4, %5, %6, %7}, [%8];"
+                             : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7])
+                             : "r"(tl + d * 16) : "memory");
+                asm volatile("tcgen05.ld.sync.aligned.32x32b.x2.b32 {%0, %1}, [%2];" : "=r"(r[8]), "=r"(r[9]) : "r"(tl + d * 16 + 8) : "memory");
+                asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+                tc_fence_before();
+                __syncwarp();
+                if (lane == 0) mbar_arrive(smem_u32(&sm.dempty[d]));
+                TCP(2);
+                const int e = inf.z;
+                BLIP_ASSERT(e >= 0 && (long long)e < g.M);
+                float q[5];
+#pragma unroll
+                for (int k = 0; k < 5; ++k) q[k] = __fmul_rn(__fadd_rn(__uint_as_float(r[k]), __uint_as_float(r[k + 5])), scl.inv[k]);
+                if (inf.x < 0) {
+#pragma unroll
+                    for (int k = 0; k < 5; ++k) q[k] = __int_as_float(0x7fc00000);       // non-finite position (R17)
+                }
+                if (col < 4 * g.pitch4 && !TC_KNOCK(4)) {
+                    const size_t o = (size_t)e * (size_t)ld + (size_t)col;
+                    __stcs(val + o, q[0]);
+                    if (MODE != 0) {
+                        float gx = q[1], gy = q[2], gz = q[3];
+                        if (MODE == 1) {
+                            gx = __fmaf_rn(g.J[0], q[1], __fmaf_rn(g.J[3], q[2], __fmul_rn(g.J[6], q[3])));
+                            gy = __fmaf_rn(g.J[1], q[1], __fmaf_rn(g.J[4], q[2], __fmul_rn(g.J[7], q[3])));
+                            gz = __fmaf_rn(g.J[2], q[1], __fmaf_rn(g.J[5], q[2], __fmul_rn(g.J[8], q[3])));
+                        }
+                        const size_t og = (size_t)e * 3 * (size_t)ld + (size_t)col;
+                        __stcs(grad + og, gx);
+                        __stcs(grad + og + ld, gy);
+                        __stcs(grad + og + 2 * ld, gz);
+                        __stcs(lap + o, q[4]);
+                    }
+                }
+                TCP(3);
+            }
+            ubase += it_nunits;
+            leave_item(n, false);
+        }
+        TCP_FLUSH(8, warp == kTcNC && lane == 0);
+    } else if (warp < kTcNC + kTcNE + kTcNW) {
+        // ---- weight warps: warp ww takes the units with (unit number) % kTcNW == ww
+        const int ww = warp - (kTcNC + kTcNE);
+        float4* const rec4 = sm.wrec[ww];
+        const float* const recf = reinterpret_cast<const float*>(rec4);
+        unsigned ubase = 0;
+        TCP_DECL;
+        for (unsigned n = 0;; ++n) {
+            load_item(n);
+            TCP(0);
+            if (it_nplanes < 0) break;
+            const float4* rsrc = recs + (size_t)it_u0 * (kRecFloats / 4);
+            unsigned u = ((unsigned)ww + kTcNW - (ubase % kTcNW)) % kTcNW;
+            float4 pre = make_float4(0.f, 0.f, 0.f, 0.f);
+            if (u < it_nunits && lane < kRecFloats / 4) pre = __ldg(rsrc + (size_t)u * (kRecFloats / 4) + lane);
+            for (; u < it_nunits; u += kTcNW) {
+                const unsigned uc = ubase + u, b = uc % kTcNB;
+                __syncwarp();
+                if (lane < kRecFloats / 4) rec4[lane] = pre;
+                __syncwarp();
+                if (u + kTcNW < it_nunits && lane < kRecFloats / 4) pre = __ldg(rsrc + (size_t)(u + kTcNW) * (kRecFloats / 4) + lane);
+                const int4 loc = *reinterpret_cast<const int4*>(rec4 + 23);       // {plane in item or -1, byte offset of row (i2, i3), -, electron}
+                const int rowi = loc.y / (128 * 4);                               // y0 * 7 + z0
+                const int y0 = rowi / 7, z0 = rowi - 7 * y0;
+                float wz[3][4];
+#pragma unroll
+                for (int k = 0; k < 3; ++k)
+#pragma unroll
+                    for (int m = 0; m < 4; ++m) wz[k][m] = recf[80 + 4 * k + m];
+                TCP(1);
+                if (uc >= kTcNB) mbar_wait(smem_u32(&sm.bempty[b]), ((uc / kTcNB) & 1u) ^ 1u);
+                TCP(2);
+                unsigned char* const bt = sm.bt[b];
+                if (!TC_KNOCK(2))
+                // lane = (column (m1, m2) = lane / 2, half = lane % 2): half 0 builds the weights of
+                // val, T1, T2, half 1 those of T3 and lap, every one as a wz[0] + b wz[1] + c wz[2]
+                // with per-lane (a, b, c): no divergence.  Vectors of 8 fp16 (z = 0..7 of one row).
+                {
+                    const int colm = lane >> 1;
+                    const bool hb = lane & 1;
+                    const float4 cw = rec4[colm];
+                    const float lb = recf[64 + colm];
+                    float fa[3], fb[3], fc[3];
+                    fa[0] = hb ? 0.f : __fmul_rn(cw.x, scl.sw[0]);  fb[0] = hb ? __fmul_rn(cw.x, scl.sw[3]) : 0.f;  fc[0] = 0.f;
+                    fa[1] = __fmul_rn(hb ? cw.w : cw.y, hb ? scl.sw[4] : scl.sw[1]);
+                    fb[1] = hb ? __fmul_rn(lb, scl.sw[4]) : 0.f;  fc[1] = hb ? __fmul_rn(cw.x, scl.sw[4]) : 0.f;
+                    fa[2] = hb ? 0.f : __fmul_rn(cw.z, scl.sw[2]);  fb[2] = 0.f;  fc[2] = 0.f;
+                    const int m1 = colm >> 2, m2 = colm & 3;
+                    unsigned char* const tile = bt + (m1 * 2 + (m2 >> 1)) * 512 + (m2 & 1) * 128;
+#pragma unroll
+                    for (int k = 0; k < 3; ++k) {
+                        float w[4];
+#pragma unroll
+                        for (int m = 0; m < 4; ++m) w[m] = __fmaf_rn(fc[k], wz[2][m], __fmaf_rn(fb[k], wz[1][m], __fmul_rn(fa[k], wz[0][m])));
+                        unsigned a1[2], a2[2];
+                        tc_split2(w[0], w[1], a1[0], a2[0]);
+                        tc_split2(w[2], w[3], a1[1], a2[1]);
+                        uint4 v1, v2;                        // the 4 fp16 at z0 .. z0 + 3 (z0 is the same for the whole warp)
+                        if (z0 == 0) { v1 = make_uint4(a1[0], a1[1], 0u, 0u); v2 = make_uint4(a2[0], a2[1], 0u, 0u); }
+                        else if (z0 == 2) { v1 = make_uint4(0u, a1[0], a1[1], 0u); v2 = make_uint4(0u, a2[0], a2[1], 0u); }
+                        else {
+                            const unsigned p0 = a1[0] << 16, p1 = __byte_perm(a1[0], a1[1], 0x5432), p2 = a1[1] >> 16;
+                            const unsigned r0 = a2[0] << 16, r1 = __byte_perm(a2[0], a2[1], 0x5432), r2 = a2[1] >> 16;
+                            if (z0 == 1) { v1 = make_uint4(p0, p1, p2, 0u); v2 = make_uint4(r0, r1, r2, 0u); }
+                            else { v1 = make_uint4(0u, p0, p1, p2); v2 = make_uint4(0u, r0, r1, r2); }
+                        }
+                        const int qq = hb ? 3 + k : k;       // quantity; half 1 has only two
+                        if (qq < 5) {
+                            const int n2 = qq + 5;
+                            *reinterpret_cast<uint4*>(tile + qq * 16) = v1;
+                            *reinterpret_cast<uint4*>(tile + (n2 >> 3) * 256 + (n2 & 7) * 16) = v2;
+                        }
+                    }
+                }
+                if (lane == 0) sm.info[uc % kTcNInfo] = make_int4(loc.x >= 0 ? (int)(it_seq0 + (unsigned)loc.x) : -1, y0, loc.w, 0);
+                asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+                __syncwarp();
+                if (lane == 0) mbar_arrive(smem_u32(&sm.bfull[b]));
+                TCP(3);
+            }
+            ubase += it_nunits;
+            leave_item(n, false);
+        }
+        TCP_FLUSH(16, ww == 0 && lane == 0);
+    } else {
+        // ---- issuers: one elected thread of warp ii takes the units with (unit number) % 2 == ii
+        const int ii = warp - (kTcNC + kTcNE + kTcNW);
+        if (tc_elect_one()) {
+            unsigned ubase = 0, waited = 0, released = 0;
+            const unsigned tfull0 = smem_u32(&sm.tfull[0]), tempty0 = smem_u32(&sm.tempty[0]);
+            // planes < end are no longer needed by this issuer: each is handed back to the converters
+            // (commit: the arrival waits for the MMAs issued so far) once it has been seen full, so
+            // that every arrival belongs to the current phase of its barrier
+            auto pass_upto = [&](unsigned end) {
+                while (released < end) {
+                    if (released >= waited) { mbar_wait(tfull0 + 8u * (released % kTcRT), (released / kTcRT) & 1u); waited = released + 1; }
+                    tc_commit(tempty0 + 8u * (released % kTcRT));
+                    ++released;
+                }
+            };
+            TCP_DECL;
+            for (unsigned n = 0;; ++n) {
+                load_item(n);
+                TCP(0);
+                if (it_nplanes < 0) break;
+                for (unsigned u = ((unsigned)ii + kTcNI - (ubase % kTcNI)) % kTcNI; u < it_nunits; u += kTcNI) {
+                    const unsigned uc = ubase + u, b = uc % kTcNB, d = uc % kTcND;
+                    mbar_wait(smem_u32(&sm.bfull[b]), (uc / kTcNB) & 1u);
+                    TCP(1);
+                    const int4 inf = sm.info[uc % kTcNInfo];
+                    const bool ok = inf.x >= 0;
+                    const unsigned sq = (unsigned)inf.x;
+                    if (ok) {
+                        pass_upto(sq);
+                        while (waited < sq + 4) { mbar_wait(tfull0 + 8u * (waited % kTcRT), (waited / kTcRT) & 1u); ++waited; }
+                    }
+                    TCP(2);
+                    if (uc >= kTcND) mbar_wait(smem_u32(&sm.dempty[d]), ((uc / kTcND) & 1u) ^ 1u);
+                    TCP(3);
+                    tc_fence_after();
+                    if (ok && !TC_KNOCK(1)) {
+                        const unsigned dcol = tbase + kTcDCol0 + d * 16;
+                        const uint64_t bd0 = tc_bdesc(smem_u32(&sm.bt[b][0]));
+                        const unsigned ay = tbase + 4u * (unsigned)inf.y;
+                        unsigned ap[4];
+#pragma unroll
+                        for (int m1 = 0; m1 < 4; ++m1) ap[m1] = ay + ((sq + m1) % kTcRT) * kTcPlaneCols;
+#pragma unroll
+                        for (int j = 0; j < 16; ++j) {
+                            const int m1 = j >> 2, h = (j >> 1) & 1, part = j & 1;
+                            tc_mma(dcol, ap[m1] + part * 28 + h * 8, bd0 + (uint64_t)(((m1 * 2 + h) * 512) >> 4), j > 0);
+                        }
+                    }
+                    tc_commit(smem_u32(&sm.bempty[b]));
+                    tc_commit(smem_u32(&sm.dfull[d]));
+                    TCP(4);
+                }
+                if (it_nplanes > 0) pass_upto(it_seq0 + (unsigned)it_nplanes);
+                TCP(5);
+                ubase += it_nunits;
+                leave_item(n, true);
+            }
+            TCP_FLUSH(24, ii == 0);
+        }
+    }
+#ifdef BLIP_TC_PROF
+    if (threadIdx.x == 0) {
+        const unsigned long long dt = (unsigned long long)(clock64() - tcp_start);
+        atomicMax(&g_tc_prof[40], dt);
+        atomicMin(&g_tc_prof[41], dt);
+        atomicAdd(&g_tc_prof[42], dt);
+        unsigned long long g1; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(g1));
+        atomicMin(&g_tc_prof[43], tcp_g0);
+        atomicMax(&g_tc_prof[44], g1);
+        atomicMax(&g_tc_prof[45], g1 - tcp_g0);
+    }
+#endif
+    tc_fence_before();
+    __syncthreads();
+    if (warp == 0) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, 512;" :: "r"(tbase) : "memory");
+}
+
+// max |c| of the caller's table (for the power-of-two scaling); non-finite entries set bit 31 of the result
+__global__ void __launch_bounds__(256) tc_absmax_kernel(const float* __restrict__ src, long long nfloats, unsigned* __restrict__ out)
+{
+    unsigned m = 0;
+    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < nfloats; i += (long long)gridDim.x * blockDim.x) {
+        const unsigned b = __float_as_uint(__ldg(src + i)) & 0x7fffffffu;
+        m = max(m, b >= 0x7f800000u ? 0x80000000u : b);
+    }
+#pragma unroll
+    for (int d = 16; d > 0; d >>= 1) m = max(m, __shfl_xor_sync(0xffffffffu, m, d));
+    if ((threadIdx.x & 31) == 0 && m) atomicMax(out, m);
+}
+
+}  // namespace blip

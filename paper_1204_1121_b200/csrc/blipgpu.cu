@@ -6,6 +6,7 @@
 #include "blip_host.h"
 #include "blip_kernels.cuh"
 #include "blip_f64.cuh"
+#include "blip_tc.cuh"
 
 #include <cmath>
 #include <cstdlib>
@@ -86,6 +87,32 @@ cudaError_t staged_launch(int mode, unsigned nctas, cudaStream_t s, const Staged
     if (a.kvec) return staged_launch_epi<blip::kEpiComplex>(mode, nctas, s, a);
     return staged_launch_epi<blip::kEpiStore>(mode, nctas, s, a);
 }
+
+// Tensor-core form of the staged kernel (blip_tc.cuh): storing epilogue only.
+cudaError_t tc_prepare()
+{
+    cudaError_t e = cudaFuncSetAttribute(blip::eval_tc_kernel<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(blip::TcSmem));
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(blip::eval_tc_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(blip::TcSmem));
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(blip::eval_tc_kernel<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(blip::TcSmem));
+    return e;
+}
+cudaError_t tc_launch(int mode, unsigned nctas, cudaStream_t s, const StagedArgs& a, const blip::TcScale& scl)
+{
+#define BLIP_TC(MODE) launch_pdl(blip::eval_tc_kernel<MODE>, nctas, blip::kTcThreads, sizeof(blip::TcSmem), s, *a.tmap, *a.g, *a.sg, scl, \
+                                 a.recs, a.order, a.meta, a.nchunk, a.val, a.grad, a.lap, a.ld)
+    if (mode == 0) return BLIP_TC(0);
+    if (mode == 2) return BLIP_TC(2);
+    return BLIP_TC(1);
+#undef BLIP_TC
+}
+// 2^k with 2^k * bound in (2^(target-1), 2^target]
+float pow2_scale(double bound, int target)
+{
+    if (!(bound > 0.0) || !std::isfinite(bound)) return 1.0f;
+    int ex = 0;
+    (void)std::frexp(bound, &ex);                    // bound = m 2^ex, m in [0.5, 1)
+    return (float)std::ldexp(1.0, target - ex);
+}
 }
 
 static thread_local int g_create_cuda_error = 0;
@@ -156,6 +183,29 @@ static bool build_tensor_map(blipgpu_table* t)
     const cuuint32_t box[4] = {(cuuint32_t)kSC, (cuuint32_t)(kSBZ + 3), (cuuint32_t)(kSBY + 3), 1u};
     const cuuint32_t estr[4] = {1u, 1u, 1u, 1u};
     const CUresult r = ((encode_fn)fn)(&t->tmap, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 4, t->table, dims, strides, box,
+                                       estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
+                                       CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    return r == CUDA_SUCCESS;
+}
+
+static bool build_tensor_map16(blipgpu_table* t, int nzp)
+{
+    typedef CUresult (*encode_fn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
+                                  const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
+                                  CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+    void* fn = nullptr;
+    cudaDriverEntryPointQueryResult qres;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres) != cudaSuccess ||
+        qres != cudaDriverEntryPointSuccess || !fn) {
+        (void)cudaGetLastError();
+        return false;
+    }
+    const cuuint64_t pitchB = (cuuint64_t)t->pitch * 4;
+    const cuuint64_t dims[5] = {(cuuint64_t)t->pitch, 2, (cuuint64_t)nzp, (cuuint64_t)t->g.np[1], (cuuint64_t)t->g.np[0]};
+    const cuuint64_t strides[4] = {pitchB, 2 * pitchB, 2 * pitchB * nzp, 2 * pitchB * nzp * t->g.np[1]};
+    const cuuint32_t box[5] = {128u, 2u, 4u, 7u, 1u};
+    const cuuint32_t estr[5] = {1u, 1u, 1u, 1u, 1u};
+    const CUresult r = ((encode_fn)fn)(&t->tmap16, CU_TENSOR_MAP_DATA_TYPE_UINT32, 5, t->table16, dims, strides, box,
                                        estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
                                        CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
     return r == CUDA_SUCCESS;
@@ -275,7 +325,18 @@ extern "C" int blipgpu_create(const double* lattice, const int* grid, int norb,
         if ((e = cudaGetLastError()) == cudaSuccess) e = cudaStreamSynchronize(s);
         if (e != cudaSuccess) fail(e);
     }
-    if (staging) cudaFree(staging);
+    unsigned absmax_bits = 0x80000000u;               // unknown / non-finite: no tensor-core path
+    if (rc == BLIPGPU_OK) {
+        unsigned* d_max = nullptr;
+        if (cudaMalloc(&d_max, sizeof(unsigned)) == cudaSuccess && cudaMemsetAsync(d_max, 0, sizeof(unsigned), s) == cudaSuccess) {
+            blip::tc_absmax_kernel<<<(unsigned)(4 * t->nsm), 256, 0, s>>>(coeffs_on_device ? coeffs : staging, nsites * (long long)norb, d_max);
+            if (cudaMemcpyAsync(&absmax_bits, d_max, sizeof(unsigned), cudaMemcpyDeviceToHost, s) != cudaSuccess ||
+                cudaStreamSynchronize(s) != cudaSuccess)
+                absmax_bits = 0x80000000u;
+        }
+        cudaFree(d_max);
+        (void)cudaGetLastError();
+    }
     if (rc == BLIPGPU_OK) {
         // staged path: needs a full tile row (pitch >= C), a grid at least as large as one box,
         // the opt-in shared memory size, and the TMA descriptor
@@ -285,7 +346,40 @@ extern "C" int blipgpu_create(const double* lattice, const int* grid, int norb,
             e = staged_prepare();
             if (e == cudaSuccess) t->staged_ok = 1; else (void)cudaGetLastError();
         }
+        // tensor-core form: a finite table (a NaN or Inf would reach electrons that do not touch it
+        // through the zero-weight rows of an MMA) and power-of-two scales that bring the coefficients
+        // to <= 2^9 and the weights of every quantity to <= 2^8 in fp16 (blip_tc.cuh)
+        if (t->staged_ok && !(absmax_bits & 0x80000000u) && (size_t)prop.sharedMemPerBlockOptin >= sizeof(blip::TcSmem) &&
+            tc_prepare() == cudaSuccess) {
+            float amax;
+            memcpy(&amax, &absmax_bits, sizeof(float));
+            const double* Q = t->g64.Q;
+            const double jd[3] = {t->diag ? std::fabs(Jd[0][0]) : 1.0, t->diag ? std::fabs(Jd[1][1]) : 1.0, t->diag ? std::fabs(Jd[2][2]) : 1.0};
+            const double bound[5] = {1.0, jd[0], jd[1], jd[2],
+                                     2.0 * (std::fabs(Q[0]) + std::fabs(Q[1]) + std::fabs(Q[2])) +
+                                         4.0 * (std::fabs(Q[3]) + std::fabs(Q[4]) + std::fabs(Q[5]))};
+            t->tc_scale[0] = pow2_scale((double)amax, 9);
+            bool fine = std::isfinite(t->tc_scale[0]) && t->tc_scale[0] > 0.f;
+            for (int q = 0; q < 5; ++q) {
+                t->tc_scale[1 + q] = pow2_scale(bound[q], 8);
+                t->tc_scale[6 + q] = 1.0f / (t->tc_scale[0] * t->tc_scale[1 + q]);
+                fine = fine && std::isfinite(t->tc_scale[1 + q]) && t->tc_scale[1 + q] > 0.f && std::isfinite(t->tc_scale[6 + q]) && t->tc_scale[6 + q] > 0.f;
+            }
+            // the fp16 table and its TMA descriptor (5-D: {pitch, half, z pair, p2, p1}, box {128, 2, 4, 7, 1})
+            const int nzp = (t->g.np[2] + 1) / 2;
+            const long long words = (long long)t->g.np[0] * t->g.np[1] * nzp * 2 * pitch;
+            if (fine && cudaMalloc(&t->table16, sizeof(unsigned) * (size_t)words) == cudaSuccess) {
+                const long long total = words / 2;
+                blip::tc_table_kernel<<<(unsigned)((total + 255) / 256), 256, 0, s>>>(t->g, t->tc_scale[0], nzp, coeffs_on_device ? coeffs : staging,
+                                                                                   t->table16, total);
+                fine = cudaGetLastError() == cudaSuccess && cudaStreamSynchronize(s) == cudaSuccess && build_tensor_map16(t, nzp);
+            } else fine = false;
+            if (!fine) { cudaFree(t->table16); t->table16 = nullptr; }
+            t->tc_ok = fine ? 1 : 0;
+        }
+        (void)cudaGetLastError();
     }
+    if (staging) cudaFree(staging);
     if (rc == BLIPGPU_OK) {
         // one-launch grouping: needs a cooperative launch of one 1,024-thread CTA per SM and the
         // histogram (+ 1 word) in dynamic shared memory next to the kernel's static 33 KB
@@ -307,7 +401,7 @@ extern "C" int blipgpu_create(const double* lattice, const int* grid, int norb,
 extern "C" int blipgpu_destroy(blipgpu_table* t)
 {
     if (!t) return BLIPGPU_OK;
-    cudaFree(t->table); cudaFree(t->bin); cudaFree(t->perm); cudaFree(t->recs); cudaFree(t->hist); cudaFree(t->offs); cudaFree(t->counters); cudaFree(t->gstate);
+    cudaFree(t->table); cudaFree(t->table16); cudaFree(t->bin); cudaFree(t->perm); cudaFree(t->recs); cudaFree(t->hist); cudaFree(t->offs); cudaFree(t->counters); cudaFree(t->gstate);
     cudaFree(t->order); cudaFree(t->meta); cudaFree(t->kvec);
     cudaFree(t->d_pos); cudaFree(t->d_val); cudaFree(t->d_grad); cudaFree(t->d_lap); cudaFree(t->d_cell);
     for (int k = 0; k < 3; ++k) if (t->pe[k]) cudaEventDestroy(t->pe[k]);
@@ -359,7 +453,7 @@ static const double kStagedMinReuse = 6.0;
 static bool use_staged(const blipgpu_table* t, long long M)
 {
     if (!t->staged_ok || t->path == 1) return false;
-    if (t->path == 2) return true;
+    if (t->path == 2 || t->path == 5) return true;
     if (M <= kGroupThreshold) return false;
     const double sites = (double)t->g.n[0] * t->g.n[1] * t->g.n[2];
     return 64.0 * (double)M / sites >= kStagedMinReuse;
@@ -438,8 +532,18 @@ static int launch_eval(blipgpu_table* t, const double* positions, long long M, i
         if (t->profiling) CK(t, cudaEventRecord(t->pe[1], s));
         const StagedArgs a = {&t->tmap, &t->g, &t->sg, t->recs, t->order, t->meta, t->nchunk,
                               val, grad, lap, ld, dvec, ldd, cout, positions, kvec};
-        CK(t, staged_launch(kmode, (unsigned)t->nsm, s, a));
-        t->last_path = 2;
+        if (t->path == 5 && t->tc_ok && !dvec && !kvec) {
+            blip::TcScale scl;
+            scl.sc = t->tc_scale[0];
+            for (int q = 0; q < 5; ++q) { scl.sw[q] = t->tc_scale[1 + q]; scl.inv[q] = t->tc_scale[6 + q]; }
+            StagedArgs a16 = a;
+            a16.tmap = &t->tmap16;
+            CK(t, tc_launch(kmode, (unsigned)t->nsm, s, a16, scl));
+            t->last_path = 5;
+        } else {
+            CK(t, staged_launch(kmode, (unsigned)t->nsm, s, a));
+            t->last_path = 2;
+        }
     } else if (t->path == 0 && !perm && M <= kSplitMax) {
         t->last_path = 3;
         if (t->profiling) CK(t, cudaEventRecord(t->pe[1], s));
@@ -551,6 +655,18 @@ extern "C" int blipgpu_eval_f64(blipgpu_table* t, const double* positions, long 
     CK(t, cudaGetLastError());
     return BLIPGPU_OK;
 }
+
+#ifdef BLIP_TC_PROF
+extern "C" int blipgpu_tc_knock(int k) { return cudaMemcpyToSymbol(blip::g_tc_knock, &k, sizeof(int)) == cudaSuccess ? 0 : -3; }
+extern "C" int blipgpu_tc_prof(unsigned long long* out, int reset)
+{
+    if (out && cudaMemcpyFromSymbol(out, blip::g_tc_prof, sizeof(unsigned long long) * 64) != cudaSuccess) return -3;
+    if (out) (void)cudaMemcpyFromSymbol(out + 48, blip::g_sp_prof, sizeof(unsigned long long) * 2);
+    if (reset) { unsigned long long z2[2] = {0, 0}; (void)cudaMemcpyToSymbol(blip::g_sp_prof, z2, sizeof(z2)); }
+    if (reset) { unsigned long long z[64] = {0}; z[41] = ~0ull; z[43] = ~0ull; if (cudaMemcpyToSymbol(blip::g_tc_prof, z, sizeof(z)) != cudaSuccess) return -3; }
+    return 0;
+}
+#endif
 
 extern "C" int blipgpu_reserve(blipgpu_table* t, long long M_max)
 {

@@ -73,8 +73,9 @@ extern "C" int blipgpu_last_kernel_ms(blipgpu_table* t, float* group_ms, float* 
 
 extern "C" int blipgpu_set_tuning(blipgpu_table* t, int path, int nq)
 {
-    if (!t || path < 0 || path > 2 || nq < 0 || nq > 3) return BLIPGPU_EINVAL;
+    if (!t || path < 0 || (path > 2 && path != 5) || nq < 0 || nq > 3) return BLIPGPU_EINVAL;
     if (path == 2 && !t->staged_ok) return BLIPGPU_EINVAL;
+    if (path == 5 && !(t->staged_ok && t->tc_ok)) return BLIPGPU_EINVAL;
     t->path = path;
     t->nq = nq ? nq : blip_default_nq(t->g.pitch4);
     return BLIPGPU_OK;
