@@ -87,6 +87,20 @@ __device__ __forceinline__ bool tc_elect_one()
     asm volatile("{\n\t.reg .pred p;\n\telect.sync _|p, 0xffffffff;\n\tselp.u32 %0, 1, 0, p;\n\t}" : "=r"(pred));
     return pred != 0;
 }
+constexpr unsigned kTcWaitHintNs = 100;
+// wait of a role that runs ahead of / behind the issuers: the hardware may park the warp for up to
+// ~1 us per poll instead of spinning in the issue slots the other roles need
+__device__ __forceinline__ void mbar_wait_relaxed(unsigned bar, unsigned parity)
+{
+    asm volatile(
+        "{\n\t.reg .pred p;\n\t"
+        "WAIT_%=:\n\t"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1, %2;\n\t"
+        "@p bra DONE_%=;\n\t"
+        "bra WAIT_%=;\n\t"
+        "DONE_%=:\n\t}"
+        :: "r"(bar), "r"(parity), "r"(kTcWaitHintNs) : "memory");
+}
 __device__ __forceinline__ void tc_commit(unsigned bar)
 {
     asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" :: "r"(bar) : "memory");
@@ -180,7 +194,17 @@ __device__ unsigned long long g_tc_prof[64];
 #define TCP_DECL long long tcp_t = clock64(); long long tcp_a[6] = {0, 0, 0, 0, 0, 0}
 #define TCP(k) do { const long long t1_ = clock64(); tcp_a[k] += t1_ - tcp_t; tcp_t = t1_; } while (0)
 #define TCP_FLUSH(base, leader) do { if (blockIdx.x == 0 && (leader)) { for (int k_ = 0; k_ < 6; ++k_) atomicAdd(&g_tc_prof[(base) + k_], (unsigned long long)tcp_a[k_]); } } while (0)
+// wait that records: [0] calls satisfied at once, [1] calls that had to wait, [2] cycles waited
+__device__ __forceinline__ void mbar_wait_prof(unsigned bar, unsigned parity, long long* c)
+{
+    if (mbar_test(bar, parity)) { c[0] += 1; return; }
+    const long long t0 = clock64();
+    mbar_wait(bar, parity);
+    c[1] += 1; c[2] += clock64() - t0;
+}
+#define TCW(bar, par, c) mbar_wait_prof(bar, par, c)
 #else
+#define TCW(bar, par, c) mbar_wait(bar, par)
 #define TC_KNOCK(bit) false
 #define TCP_DECL do { } while (0)
 #define TCP(k) do { } while (0)
@@ -252,8 +276,11 @@ eval_tc_kernel(const __grid_constant__ CUtensorMap tmap, Geom g, StagedGeom sg, 
                 WorkItem& it = sm.item[q];
                 Desc d = {-1, 0, 0, 0, 0};
                 if (w < nitems) {
-                    d.chunk = w % nchunk;
-                    const int4 o = __ldg(order + w / nchunk);
+                    // chunk-major: every pencil of one 128-orbital chunk before the next chunk, so that the CTAs
+                    // in flight work on neighbouring pencils of ONE slice of the table and find each other's
+                    // halo rows in L2 (the kernel is close to the DRAM bound; blip_tc.cuh header)
+                    d.chunk = w / nps;
+                    const int4 o = __ldg(order + (w - d.chunk * nps));
                     const int pencil = o.x / sg.nseg, segi = o.x - pencil * sg.nseg;
                     d.lo = segi * sg.seg;
                     const int hi = min(d.lo + sg.seg, g.n[0]) - 1;
@@ -296,43 +323,42 @@ eval_tc_kernel(const __grid_constant__ CUtensorMap tmap, Geom g, StagedGeom sg, 
             for (int j = (int)((it_seq0 + (unsigned)cg) & 1u); j < it_nplanes; j += 2) {
                 const unsigned q = it_seq0 + (unsigned)j;
                 const unsigned s = q % kTcRS, t = q % kTcRT;
-                mbar_wait(smem_u32(&sm.full[s]), (q / kTcRS) & 1u);
+                mbar_wait_relaxed(smem_u32(&sm.full[s]), (q / kTcRS) & 1u);
                 TCP(1);
-                // the plane's 56 words into registers, and the shared-memory slot straight back to the
-                // producer: the plane then waits for its TMEM slot in registers while the TMA runs ahead
+                // rows 0..3 of the plane (32 words, all loads in flight at once) wait in registers for the
+                // TMEM slot; rows 4..6 follow behind the first stores (56 words at once do not fit in the
+                // 64 registers a thread of this 928-thread CTA has)
                 const unsigned* src = &sm.plane[s][orb];
-                unsigned h[7][8];
-                unsigned any = 0;
-                if (!TC_KNOCK(8))
+                const unsigned tcol = tlane + t * kTcPlaneCols;
+                auto ld_rows = [&](unsigned (&h)[4][8], int y0, int ny) {
 #pragma unroll
-                for (int y = 0; y < 7; ++y)
+                    for (int y = 0; y < 4; ++y)
+                        if (y < ny)
 #pragma unroll
-                    for (int k = 0; k < 4; ++k) {
-                        h[y][k] = src[((y * 4 + k) * 2) * 128]; h[y][4 + k] = src[((y * 4 + k) * 2 + 1) * 128];
-                        any |= h[y][k] | h[y][4 + k];
-                    }
-                any |= __shfl_xor_sync(0xffffffffu, any, 1) | __shfl_xor_sync(0xffffffffu, any, 2);
-                any |= __shfl_xor_sync(0xffffffffu, any, 4) | __shfl_xor_sync(0xffffffffu, any, 8);
-                any |= __shfl_xor_sync(0xffffffffu, any, 16);
-                // (any * any) & 2 is zero for every value (a square is 0 or 1 mod 4): the address of the
-                // arrival depends on every word loaded, so the arrival cannot overtake the loads
-                if (lane == 0) mbar_arrive(smem_u32(&sm.empty[s]) + ((any * any) & 2u) * 4u);
-                if (q >= kTcRT) mbar_wait(smem_u32(&sm.tempty[t]), ((q / kTcRT) & 1u) ^ 1u);
+                            for (int k = 0; k < 4; ++k) {
+                                h[y][k] = src[(((y0 + y) * 4 + k) * 2) * 128]; h[y][4 + k] = src[(((y0 + y) * 4 + k) * 2 + 1) * 128];
+                            }
+                };
+                auto st_rows = [&](const unsigned (&h)[4][8], int y0, int ny) {
+#pragma unroll
+                    for (int y = 0; y < 4; ++y)
+                        if (y < ny) {
+                            asm volatile("tcgen05.st.sync.aligned.32x32b.x4.b32 [%0], {%1, %2, %3, %4};"
+                                         :: "r"(tcol + 4 * (y0 + y)), "r"(h[y][0]), "r"(h[y][1]), "r"(h[y][2]), "r"(h[y][3]) : "memory");
+                            asm volatile("tcgen05.st.sync.aligned.32x32b.x4.b32 [%0], {%1, %2, %3, %4};"
+                                         :: "r"(tcol + 28 + 4 * (y0 + y)), "r"(h[y][4]), "r"(h[y][5]), "r"(h[y][6]), "r"(h[y][7]) : "memory");
+                        }
+                };
+                unsigned ha[4][8], hb[4][8];
+                if (!TC_KNOCK(8)) ld_rows(ha, 0, 4);
+                if (q >= kTcRT) mbar_wait_relaxed(smem_u32(&sm.tempty[t]), ((q / kTcRT) & 1u) ^ 1u);
                 TCP(2);
                 tc_fence_after();
-                const unsigned tcol = tlane + t * kTcPlaneCols;
-                if (!TC_KNOCK(8))
-#pragma unroll
-                for (int y = 0; y < 7; ++y) {
-                    asm volatile("tcgen05.st.sync.aligned.32x32b.x4.b32 [%0], {%1, %2, %3, %4};"
-                                 :: "r"(tcol + 4 * y), "r"(h[y][0]), "r"(h[y][1]), "r"(h[y][2]), "r"(h[y][3]) : "memory");
-                    asm volatile("tcgen05.st.sync.aligned.32x32b.x4.b32 [%0], {%1, %2, %3, %4};"
-                                 :: "r"(tcol + 28 + 4 * y), "r"(h[y][4]), "r"(h[y][5]), "r"(h[y][6]), "r"(h[y][7]) : "memory");
-                }
+                if (!TC_KNOCK(8)) { st_rows(ha, 0, 4); ld_rows(hb, 4, 3); st_rows(hb, 4, 3); }
                 asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
                 tc_fence_before();
                 __syncwarp();
-                if (lane == 0) mbar_arrive(smem_u32(&sm.tfull[t]));
+                if (lane == 0) { mbar_arrive(smem_u32(&sm.tfull[t])); mbar_arrive(smem_u32(&sm.empty[s])); }
                 TCP(3);
             }
             leave_item(n, false);
@@ -351,7 +377,7 @@ eval_tc_kernel(const __grid_constant__ CUtensorMap tmap, Geom g, StagedGeom sg, 
             const int col = it_chunk * 128 + sp * 32 + lane;
             for (unsigned u = (ubase + (unsigned)eg) & 1u; u < it_nunits; u += 2) {      // (ubase + u) % 2 == eg
                 const unsigned uc = ubase + u, d = uc % kTcND;
-                mbar_wait(smem_u32(&sm.dfull[d]), (uc / kTcND) & 1u);
+                mbar_wait_relaxed(smem_u32(&sm.dfull[d]), (uc / kTcND) & 1u);
                 TCP(1);
                 tc_fence_after();
                 const int4 inf = sm.info[uc % kTcNInfo];
@@ -370,9 +396,8 @@ eval_tc_kernel(const __grid_constant__ CUtensorMap tmap, Geom g, StagedGeom sg, 
                 float q[5];
 #pragma unroll
                 for (int k = 0; k < 5; ++k) q[k] = __fmul_rn(__fadd_rn(__uint_as_float(r[k]), __uint_as_float(r[k + 5])), scl.inv[k]);
-                if (inf.x < 0) {
-#pragma unroll
-                    for (int k = 0; k < 5; ++k) q[k] = __int_as_float(0x7fc00000);       // non-finite position (R17)
+                if (inf.x < 0) {                             // non-finite position (R17): the same for the whole warp
+                    q[0] = q[1] = q[2] = q[3] = q[4] = __int_as_float(0x7fc00000);
                 }
                 if (col < 4 * g.pitch4 && !TC_KNOCK(4)) {
                     const size_t o = (size_t)e * (size_t)ld + (size_t)col;
@@ -427,7 +452,7 @@ eval_tc_kernel(const __grid_constant__ CUtensorMap tmap, Geom g, StagedGeom sg, 
 #pragma unroll
                     for (int m = 0; m < 4; ++m) wz[k][m] = recf[80 + 4 * k + m];
                 TCP(1);
-                if (uc >= kTcNB) mbar_wait(smem_u32(&sm.bempty[b]), ((uc / kTcNB) & 1u) ^ 1u);
+                if (uc >= kTcNB) mbar_wait_relaxed(smem_u32(&sm.bempty[b]), ((uc / kTcNB) & 1u) ^ 1u);
                 TCP(2);
                 unsigned char* const bt = sm.bt[b];
                 if (!TC_KNOCK(2))
@@ -486,13 +511,16 @@ eval_tc_kernel(const __grid_constant__ CUtensorMap tmap, Geom g, StagedGeom sg, 
         const int ii = warp - (kTcNC + kTcNE + kTcNW);
         if (tc_elect_one()) {
             unsigned ubase = 0, waited = 0, released = 0;
+#ifdef BLIP_TC_PROF
+            long long wc_t[3] = {0, 0, 0}, wc_b[3] = {0, 0, 0}, wc_d[3] = {0, 0, 0};
+#endif
             const unsigned tfull0 = smem_u32(&sm.tfull[0]), tempty0 = smem_u32(&sm.tempty[0]);
             // planes < end are no longer needed by this issuer: each is handed back to the converters
             // (commit: the arrival waits for the MMAs issued so far) once it has been seen full, so
             // that every arrival belongs to the current phase of its barrier
             auto pass_upto = [&](unsigned end) {
                 while (released < end) {
-                    if (released >= waited) { mbar_wait(tfull0 + 8u * (released % kTcRT), (released / kTcRT) & 1u); waited = released + 1; }
+                    if (released >= waited) { TCW(tfull0 + 8u * (released % kTcRT), (released / kTcRT) & 1u, wc_t); waited = released + 1; }
                     tc_commit(tempty0 + 8u * (released % kTcRT));
                     ++released;
                 }
@@ -504,17 +532,17 @@ eval_tc_kernel(const __grid_constant__ CUtensorMap tmap, Geom g, StagedGeom sg, 
                 if (it_nplanes < 0) break;
                 for (unsigned u = ((unsigned)ii + kTcNI - (ubase % kTcNI)) % kTcNI; u < it_nunits; u += kTcNI) {
                     const unsigned uc = ubase + u, b = uc % kTcNB, d = uc % kTcND;
-                    mbar_wait(smem_u32(&sm.bfull[b]), (uc / kTcNB) & 1u);
+                    TCW(smem_u32(&sm.bfull[b]), (uc / kTcNB) & 1u, wc_b);
                     TCP(1);
                     const int4 inf = sm.info[uc % kTcNInfo];
                     const bool ok = inf.x >= 0;
                     const unsigned sq = (unsigned)inf.x;
                     if (ok) {
                         pass_upto(sq);
-                        while (waited < sq + 4) { mbar_wait(tfull0 + 8u * (waited % kTcRT), (waited / kTcRT) & 1u); ++waited; }
+                        while (waited < sq + 4) { TCW(tfull0 + 8u * (waited % kTcRT), (waited / kTcRT) & 1u, wc_t); ++waited; }
                     }
                     TCP(2);
-                    if (uc >= kTcND) mbar_wait(smem_u32(&sm.dempty[d]), ((uc / kTcND) & 1u) ^ 1u);
+                    if (uc >= kTcND) TCW(smem_u32(&sm.dempty[d]), ((uc / kTcND) & 1u) ^ 1u, wc_d);
                     TCP(3);
                     tc_fence_after();
                     if (ok && !TC_KNOCK(1)) {
@@ -540,6 +568,10 @@ eval_tc_kernel(const __grid_constant__ CUtensorMap tmap, Geom g, StagedGeom sg, 
                 leave_item(n, true);
             }
             TCP_FLUSH(24, ii == 0);
+#ifdef BLIP_TC_PROF
+            if (blockIdx.x == 0 && ii == 0)
+                for (int k = 0; k < 3; ++k) { g_tc_prof[52 + k] = wc_b[k]; g_tc_prof[55 + k] = wc_t[k]; g_tc_prof[58 + k] = wc_d[k]; }
+#endif
         }
     }
 #ifdef BLIP_TC_PROF
