@@ -19,10 +19,16 @@ extern "C" {
  *   path  0: automatic (staged for dense batches; else the split kernel up to 16,384 positions
  *            or the direct kernel, after grouping by cell brick when the table exceeds L2);
  *         1: always the direct-gather kernel (grouped above 2,048 positions);
- *         2: always the shared-memory staged kernel (EINVAL if this table cannot use it: fewer
- *            than 128 orbitals, a grid smaller than one staging box, or no TMA descriptor)
+ *         2: always the shared-memory staged kernel on the FP32 pipe (EINVAL if this table cannot
+ *            use it: fewer than 128 orbitals, a grid smaller than one staging box, or no TMA
+ *            descriptor);
+ *         5: always the tensor-core staged kernel (EINVAL if the table cannot use it: as for 2, or
+ *            a table with a non-finite coefficient); the contraction and complex-orbital entry
+ *            points run the kernel of path 2 instead
  *   nq    direct kernel: quads of 4 orbitals per lane, 1..3; 0 restores the default.
- * The direct and the staged kernel run the same arithmetic sequence and return the same bits;
+ * The direct and the FP32 staged kernel run the same arithmetic sequence and return the same bits;
+ * the tensor-core kernel multiplies exact two-term fp16 splits of coefficients and weights and
+ * accumulates in fp32 in the tensor core, so its results differ from theirs in the last bits;
  * the split kernel adds the four plane partial sums last, so its results differ from theirs
  * in the last bits (all are within the stated tolerances of the fp64 definition). */
 int blipgpu_set_tuning(blipgpu_table* t, int path, int nq);
@@ -45,7 +51,7 @@ int blipgpu_probe_tensor(blipgpu_table* t, int units_per_sm, double* ms, void* s
 
 /* blipgpu_last_path — which gather+FMA kernel the last blipgpu_eval / blipgpu_eval_host of this
  * handle launched: 1 direct (one warp per electron, rows from L2/HBM), 2 staged (table planes
- * through shared memory), 3 split (four warps per electron, small batches), 4 the fp64 kernel of blipgpu_eval_f64; 0 before
+ * through shared memory, FP32 pipe), 5 staged on the tensor cores (table planes through tensor memory), 3 split (four warps per electron, small batches), 4 the fp64 kernel of blipgpu_eval_f64; 0 before
  * any call. */
 int blipgpu_last_path(const blipgpu_table* t);
 

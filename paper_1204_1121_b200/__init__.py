@@ -171,7 +171,8 @@ def blipgpu_destroy(handle):
 
 
 def blipgpu_set_tuning(handle, path=0, nq=0):
-    """path: 0 auto, 1 direct-gather kernel, 2 staged kernel; nq: direct kernel quads per lane (0 = default)."""
+    """path: 0 auto, 1 direct-gather kernel, 2 staged kernel (FP32 pipe), 5 staged kernel on the tensor cores;
+    nq: direct kernel quads per lane (0 = default)."""
     _check(lib().blipgpu_set_tuning(handle, int(path), int(nq)), "blipgpu_set_tuning", handle)
 
 

@@ -187,6 +187,61 @@ tc_table_kernel(Geom g, float sc, int nzp, const float* __restrict__ src, unsign
     dst[o + pitch] = h2;
 }
 
+// The B tiles of one electron (unit): lane = (column (m1, m2) = lane / 2, half = lane % 2).  Half 0
+// builds the weight vectors of val, T1, T2 (P00, P10, P01 times the z weights w3), half 1 those of
+// T3 (P00 w3') and lap (La w3 + Lb w3' + P00 Q22 w3''), each scaled by its power of two, split in
+// two fp16 halves and placed at z sites Z0 .. Z0 + 3 of the row's 8 (zero elsewhere).
+template <int Z0>
+__device__ __forceinline__ uint4 tc_place(unsigned a0, unsigned a1)
+{
+    if (Z0 == 0) return make_uint4(a0, a1, 0u, 0u);
+    if (Z0 == 2) return make_uint4(0u, a0, a1, 0u);
+    const unsigned p0 = a0 << 16, p1 = __byte_perm(a0, a1, 0x5432), p2 = a1 >> 16;
+    return Z0 == 1 ? make_uint4(p0, p1, p2, 0u) : make_uint4(0u, p0, p1, p2);
+}
+template <int Z0>
+__device__ __forceinline__ void tc_store_vec(unsigned char* tile, int n, const float (&w)[4])
+{
+    unsigned a1[2], a2[2];
+    tc_split2(w[0], w[1], a1[0], a2[0]);
+    tc_split2(w[2], w[3], a1[1], a2[1]);
+    const int n2 = n + 5;
+    *reinterpret_cast<uint4*>(tile + n * 16) = tc_place<Z0>(a1[0], a1[1]);
+    *reinterpret_cast<uint4*>(tile + (n2 >> 3) * 256 + (n2 & 7) * 16) = tc_place<Z0>(a2[0], a2[1]);
+}
+template <int Z0>
+__device__ __forceinline__ void tc_build_tile(const float4* rec4, const float* recf, const float (&wz)[3][4], const TcScale& scl,
+                                              unsigned char* bt, int lane)
+{
+    const int colm = lane >> 1;
+    const bool hb = lane & 1;
+    const float4 cw = rec4[colm];
+    const int m1 = colm >> 2, m2 = colm & 3;
+    unsigned char* const tile = bt + (m1 * 2 + (m2 >> 1)) * 512 + (m2 & 1) * 128;
+    float w[4];
+    {   // val (half 0) / T3 (half 1): P00 times w3 or w3'
+        const float f = __fmul_rn(cw.x, hb ? scl.sw[3] : scl.sw[0]);
+#pragma unroll
+        for (int m = 0; m < 4; ++m) w[m] = __fmul_rn(f, hb ? wz[1][m] : wz[0][m]);
+        tc_store_vec<Z0>(tile, hb ? 3 : 0, w);
+    }
+    if (hb) {   // lap
+        const float lb = recf[64 + colm];
+        const float fa = __fmul_rn(cw.w, scl.sw[4]), fb = __fmul_rn(lb, scl.sw[4]), fc = __fmul_rn(cw.x, scl.sw[4]);
+#pragma unroll
+        for (int m = 0; m < 4; ++m) w[m] = __fmaf_rn(fc, wz[2][m], __fmaf_rn(fb, wz[1][m], __fmul_rn(fa, wz[0][m])));
+        tc_store_vec<Z0>(tile, 4, w);
+    } else {    // T1, T2
+        const float f1 = __fmul_rn(cw.y, scl.sw[1]), f2 = __fmul_rn(cw.z, scl.sw[2]);
+#pragma unroll
+        for (int m = 0; m < 4; ++m) w[m] = __fmul_rn(f1, wz[0][m]);
+        tc_store_vec<Z0>(tile, 1, w);
+#pragma unroll
+        for (int m = 0; m < 4; ++m) w[m] = __fmul_rn(f2, wz[0][m]);
+        tc_store_vec<Z0>(tile, 2, w);
+    }
+}
+
 #ifdef BLIP_TC_PROF
 __device__ int g_tc_knock;           // timing knock-outs (results wrong): 1 no MMAs, 2 no B build, 4 no output stores, 8 no plane conversion
 #define TC_KNOCK(bit) (g_tc_knock & (bit))
@@ -375,6 +430,9 @@ eval_tc_kernel(const __grid_constant__ CUtensorMap tmap, Geom g, StagedGeom sg, 
             TCP(0);
             if (it_nplanes < 0) break;
             const int col = it_chunk * 128 + sp * 32 + lane;
+            float* const vcol = val + col;
+            float* const gcol = grad + col;
+            float* const lcol = lap + col;
             for (unsigned u = (ubase + (unsigned)eg) & 1u; u < it_nunits; u += 2) {      // (ubase + u) % 2 == eg
                 const unsigned uc = ubase + u, d = uc % kTcND;
                 mbar_wait_relaxed(smem_u32(&sm.dfull[d]), (uc / kTcND) & 1u);
@@ -400,8 +458,8 @@ eval_tc_kernel(const __grid_constant__ CUtensorMap tmap, Geom g, StagedGeom sg, 
                     q[0] = q[1] = q[2] = q[3] = q[4] = __int_as_float(0x7fc00000);
                 }
                 if (col < 4 * g.pitch4 && !TC_KNOCK(4)) {
-                    const size_t o = (size_t)e * (size_t)ld + (size_t)col;
-                    __stcs(val + o, q[0]);
+                    const size_t o = (size_t)(unsigned)e * (size_t)(unsigned)ld;
+                    __stcs(vcol + o, q[0]);
                     if (MODE != 0) {
                         float gx = q[1], gy = q[2], gz = q[3];
                         if (MODE == 1) {
@@ -409,11 +467,11 @@ eval_tc_kernel(const __grid_constant__ CUtensorMap tmap, Geom g, StagedGeom sg, 
                             gy = __fmaf_rn(g.J[1], q[1], __fmaf_rn(g.J[4], q[2], __fmul_rn(g.J[7], q[3])));
                             gz = __fmaf_rn(g.J[2], q[1], __fmaf_rn(g.J[5], q[2], __fmul_rn(g.J[8], q[3])));
                         }
-                        const size_t og = (size_t)e * 3 * (size_t)ld + (size_t)col;
-                        __stcs(grad + og, gx);
-                        __stcs(grad + og + ld, gy);
-                        __stcs(grad + og + 2 * ld, gz);
-                        __stcs(lap + o, q[4]);
+                        float* const gp = gcol + 3 * o;
+                        __stcs(gp, gx);
+                        __stcs(gp + ld, gy);
+                        __stcs(gp + 2 * ld, gz);
+                        __stcs(lcol + o, q[4]);
                     }
                 }
                 TCP(3);
@@ -455,45 +513,12 @@ eval_tc_kernel(const __grid_constant__ CUtensorMap tmap, Geom g, StagedGeom sg, 
                 if (uc >= kTcNB) mbar_wait_relaxed(smem_u32(&sm.bempty[b]), ((uc / kTcNB) & 1u) ^ 1u);
                 TCP(2);
                 unsigned char* const bt = sm.bt[b];
-                if (!TC_KNOCK(2))
-                // lane = (column (m1, m2) = lane / 2, half = lane % 2): half 0 builds the weights of
-                // val, T1, T2, half 1 those of T3 and lap, every one as a wz[0] + b wz[1] + c wz[2]
-                // with per-lane (a, b, c): no divergence.  Vectors of 8 fp16 (z = 0..7 of one row).
-                {
-                    const int colm = lane >> 1;
-                    const bool hb = lane & 1;
-                    const float4 cw = rec4[colm];
-                    const float lb = recf[64 + colm];
-                    float fa[3], fb[3], fc[3];
-                    fa[0] = hb ? 0.f : __fmul_rn(cw.x, scl.sw[0]);  fb[0] = hb ? __fmul_rn(cw.x, scl.sw[3]) : 0.f;  fc[0] = 0.f;
-                    fa[1] = __fmul_rn(hb ? cw.w : cw.y, hb ? scl.sw[4] : scl.sw[1]);
-                    fb[1] = hb ? __fmul_rn(lb, scl.sw[4]) : 0.f;  fc[1] = hb ? __fmul_rn(cw.x, scl.sw[4]) : 0.f;
-                    fa[2] = hb ? 0.f : __fmul_rn(cw.z, scl.sw[2]);  fb[2] = 0.f;  fc[2] = 0.f;
-                    const int m1 = colm >> 2, m2 = colm & 3;
-                    unsigned char* const tile = bt + (m1 * 2 + (m2 >> 1)) * 512 + (m2 & 1) * 128;
-#pragma unroll
-                    for (int k = 0; k < 3; ++k) {
-                        float w[4];
-#pragma unroll
-                        for (int m = 0; m < 4; ++m) w[m] = __fmaf_rn(fc[k], wz[2][m], __fmaf_rn(fb[k], wz[1][m], __fmul_rn(fa[k], wz[0][m])));
-                        unsigned a1[2], a2[2];
-                        tc_split2(w[0], w[1], a1[0], a2[0]);
-                        tc_split2(w[2], w[3], a1[1], a2[1]);
-                        uint4 v1, v2;                        // the 4 fp16 at z0 .. z0 + 3 (z0 is the same for the whole warp)
-                        if (z0 == 0) { v1 = make_uint4(a1[0], a1[1], 0u, 0u); v2 = make_uint4(a2[0], a2[1], 0u, 0u); }
-                        else if (z0 == 2) { v1 = make_uint4(0u, a1[0], a1[1], 0u); v2 = make_uint4(0u, a2[0], a2[1], 0u); }
-                        else {
-                            const unsigned p0 = a1[0] << 16, p1 = __byte_perm(a1[0], a1[1], 0x5432), p2 = a1[1] >> 16;
-                            const unsigned r0 = a2[0] << 16, r1 = __byte_perm(a2[0], a2[1], 0x5432), r2 = a2[1] >> 16;
-                            if (z0 == 1) { v1 = make_uint4(p0, p1, p2, 0u); v2 = make_uint4(r0, r1, r2, 0u); }
-                            else { v1 = make_uint4(0u, p0, p1, p2); v2 = make_uint4(0u, r0, r1, r2); }
-                        }
-                        const int qq = hb ? 3 + k : k;       // quantity; half 1 has only two
-                        if (qq < 5) {
-                            const int n2 = qq + 5;
-                            *reinterpret_cast<uint4*>(tile + qq * 16) = v1;
-                            *reinterpret_cast<uint4*>(tile + (n2 >> 3) * 256 + (n2 & 7) * 16) = v2;
-                        }
+                if (!TC_KNOCK(2)) {
+                    switch (z0) {                              // the same for the whole warp: placement of the 4 fp16 at compile time
+                        case 0: tc_build_tile<0>(rec4, recf, wz, scl, bt, lane); break;
+                        case 1: tc_build_tile<1>(rec4, recf, wz, scl, bt, lane); break;
+                        case 2: tc_build_tile<2>(rec4, recf, wz, scl, bt, lane); break;
+                        default: tc_build_tile<3>(rec4, recf, wz, scl, bt, lane); break;
                     }
                 }
                 if (lane == 0) sm.info[uc % kTcNInfo] = make_int4(loc.x >= 0 ? (int)(it_seq0 + (unsigned)loc.x) : -1, y0, loc.w, 0);

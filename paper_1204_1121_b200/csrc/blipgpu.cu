@@ -280,7 +280,7 @@ extern "C" int blipgpu_create(const double* lattice, const int* grid, int norb,
     {
         int seg = grid[0];
         const long long pencils = (long long)t->sg.nby * t->sg.nbz * t->nchunk;
-        while (seg > 16 && pencils * ((grid[0] + seg - 1) / seg) < 4LL * t->nsm) seg = (seg + 1) / 2;
+        while (seg > 16 && pencils * ((grid[0] + seg - 1) / seg) < 8LL * t->nsm) seg = (seg + 1) / 2;
         t->sg.seg = seg;
     }
     t->sg.nseg = (grid[0] + t->sg.seg - 1) / t->sg.seg;
@@ -437,7 +437,10 @@ static int launch_hess(blipgpu_table* t, const double* positions, long long M,
 
 // Which kernel serves a call (path = 0, automatic):
 //   staged   M > 2,048 and every table row is wanted by >= 6 electrons on average: rows are
-//            staged once in shared memory for all electrons of a pencil;
+//            staged once on chip for all electrons of a pencil — in tensor memory, evaluated by
+//            tcgen05.mma (blip::eval_tc_kernel), when the results are stored and the table is
+//            finite; in shared memory, evaluated by packed FP32 FMAs (blip::eval_staged_kernel),
+//            for the contraction and complex-orbital epilogues;
 //   grouped  otherwise, if M > 2,048 and the table does not fit in L2: electrons sorted by
 //            4x4x4-cell brick so that neighbours run together, then the direct kernel;
 //   plain    otherwise (every electron of the batch is in flight at once, or L2 holds the
@@ -532,7 +535,7 @@ static int launch_eval(blipgpu_table* t, const double* positions, long long M, i
         if (t->profiling) CK(t, cudaEventRecord(t->pe[1], s));
         const StagedArgs a = {&t->tmap, &t->g, &t->sg, t->recs, t->order, t->meta, t->nchunk,
                               val, grad, lap, ld, dvec, ldd, cout, positions, kvec};
-        if (t->path == 5 && t->tc_ok && !dvec && !kvec) {
+        if ((t->path == 5 || t->path == 0) && t->tc_ok && !dvec && !kvec) {       // storing epilogue: on the tensor cores
             blip::TcScale scl;
             scl.sc = t->tc_scale[0];
             for (int q = 0; q < 5; ++q) { scl.sw[q] = t->tc_scale[1 + q]; scl.inv[q] = t->tc_scale[6 + q]; }

@@ -100,9 +100,9 @@ def test_axis_aligned_lattice_mode(torch_cuda, blip):
         compare(A, grid, c, pos, out[path])
     for a, b in zip(out[2], out[1]):
         assert np.array_equal(a, b)
-    blip.blipgpu_set_tuning(t.handle, path=0)             # automatic: dense batch -> staged, small batch -> split
-    run_gpu(torch_cuda, blip, A, grid, c, pos, table=t)
-    assert blip.blipgpu_last_path(t.handle) == 2
+    blip.blipgpu_set_tuning(t.handle, path=0)             # automatic: dense batch -> staged (tensor cores), small batch -> split
+    compare(A, grid, c, pos, run_gpu(torch_cuda, blip, A, grid, c, pos, table=t))
+    assert blip.blipgpu_last_path(t.handle) == 5
     compare(A, grid, c, pos[:150], run_gpu(torch_cuda, blip, A, grid, c, pos[:150], table=t))
     assert blip.blipgpu_last_path(t.handle) == 3
     t.close()

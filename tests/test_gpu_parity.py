@@ -116,16 +116,25 @@ def compare_all(A, grid, c, pos, gpu, mode=1, chunk=8192):
 
 
 def test_config_tio2_full_size_every_output(torch_cuda, blip, tio2):
-    """The full 49,152-position call in the launch configuration bench.py times (staged kernel):
-    cells and val / grad / lap of EVERY position and orbital against the oracle, both modes."""
+    """The full 49,152-position call in the launch configuration bench.py times (the staged kernel
+    on the tensor cores): cells and val / grad / lap of EVERY position and orbital against the
+    oracle, both modes; then the same for the FP32-pipe staged kernel."""
     cfg, A, c, table = tio2
     pos = workloads.positions(cfg)
     gpu = run_gpu(torch_cuda, blip, A, cfg.grid, c, pos, table=table)
-    assert blip.blipgpu_last_path(table.handle) == 2        # the staged kernel, as in bench.py
+    assert blip.blipgpu_last_path(table.handle) == 5        # the tensor-core staged kernel, as in bench.py
     worst = compare_all(A, cfg.grid, c, pos, gpu)
     assert max(worst.values()) < 0.5, worst                 # expected a few % of the tolerances
     val0, _, _, _ = run_gpu(torch_cuda, blip, A, cfg.grid, c, pos, mode=0, table=table, want_cell=False)
     compare_all(A, cfg.grid, c, pos, (val0, None, None, None), mode=0)
+    try:
+        blip.blipgpu_set_tuning(table.handle, path=2)
+        gpu = run_gpu(torch_cuda, blip, A, cfg.grid, c, pos, table=table)
+        assert blip.blipgpu_last_path(table.handle) == 2
+        worst = compare_all(A, cfg.grid, c, pos, gpu)
+        assert max(worst.values()) < 0.5, worst
+    finally:
+        blip.blipgpu_set_tuning(table.handle, path=0)
 
 
 def test_tio2_full_size_staged_equals_direct_and_is_repeatable(torch_cuda, blip, tio2):

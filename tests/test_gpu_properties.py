@@ -22,7 +22,7 @@ from test_gpu_parity import tolerances, torch_cuda, blip  # noqa: F401 (fixtures
 pytestmark = pytest.mark.gpu
 
 
-@pytest.mark.parametrize("name,path", [("tio2", 2), ("large", 1), ("small", 3)])
+@pytest.mark.parametrize("name,path", [("tio2", 5), ("tio2", 2), ("large", 1), ("small", 3)])
 def test_partition_of_unity_full_size(torch_cuda, blip, name, path):
     torch = torch_cuda
     cfg = workloads.CONFIGS[name]
@@ -31,6 +31,8 @@ def test_partition_of_unity_full_size(torch_cuda, blip, name, path):
     c = torch.full((*cfg.grid, cfg.norb), kappa, dtype=torch.float32, device="cuda")     # built on the device
     h = blip.blipgpu_create(A, cfg.grid, cfg.norb, c)
     del c
+    if path == 2:
+        blip.blipgpu_set_tuning(h, 2, 0)                     # the FP32-pipe staged kernel (automatic: tensor cores, path 5)
     pos = torch.from_numpy(workloads.positions(cfg)).cuda()
     M, L = pos.shape[0], cfg.norb
     val = torch.empty((M, L), dtype=torch.float32, device="cuda")
@@ -71,7 +73,7 @@ def test_periodicity_full_size_tio2(torch_cuda, blip):
     t.close()
 
 
-@pytest.mark.parametrize("name,path", [("tio2", 2), ("tio2", 1), ("small", 3)])
+@pytest.mark.parametrize("name,path", [("tio2", 5), ("tio2", 2), ("tio2", 1), ("small", 3)])
 def test_linear_ramp_table_full_size(torch_cuda, blip, name, path):
     """Ramp table (see module docstring) on every position of the config whose block of sites stays
     clear of the periodic seam, against the closed form evaluated here in fp64."""

@@ -1,0 +1,185 @@
+"""The tensor-core form of the staged kernel (blip::eval_tc_kernel, tuning path 5; the kernel the
+automatic choice takes for dense batches): parity with the oracle on every output, the cases its
+layout makes special (ragged orbital chunks, grids that are not a multiple of the 4 x 4 pencil,
+every z offset of an electron in its pencil, non-finite positions, tables of very different
+scale), run-to-run bit identity, and the fall-backs."""
+import numpy as np
+import pytest
+
+import oracle
+import workloads
+from test_gpu_parity import compare, compare_all, run_gpu, tolerances, torch_cuda, blip, tio2  # noqa: F401 (fixtures)
+
+pytestmark = pytest.mark.gpu
+
+TRICLINIC = ((20.0, 0.0, 0.0), (3.0, 19.0, 0.0), (2.0, 2.0, 24.0))
+ORTHO = ((10.0, 0.0, 0.0), (0.0, 9.0, 0.0), (0.0, 0.0, 8.0))
+
+
+def tc_table(blip, A, grid, c):
+    t = blip.BlipTable(A, grid, c.shape[3], c)
+    blip.blipgpu_set_tuning(t.handle, path=5)
+    return t
+
+
+@pytest.mark.parametrize("grid,L,lat", [((9, 10, 13), 130, TRICLINIC), ((12, 8, 8), 256, ORTHO), ((7, 5, 6), 128, TRICLINIC),
+                                        ((16, 11, 9), 389, ORTHO)])
+@pytest.mark.parametrize("mode", [0, 1])
+def test_every_output_against_the_oracle(torch_cuda, blip, grid, L, lat, mode):
+    """Grids that are not multiples of the pencil (TMA boxes hang over the table edge), orbital
+    counts that leave a ragged last chunk, both lattice kinds (kernel MODE 1 and 2), both modes."""
+    A, c, pos = workloads.small_case(grid, L, 4000, lat, seed=L + mode, spread=3.0)
+    t = tc_table(blip, A, grid, c)
+    gpu = run_gpu(torch_cuda, blip, A, grid, c, pos, mode=mode, table=t)
+    assert blip.blipgpu_last_path(t.handle) == 5
+    compare(A, grid, c, pos, gpu, mode=mode)
+    t.close()
+
+
+def test_every_cell_offset_in_a_pencil(torch_cuda, blip):
+    """One electron in every cell of an 8 x 8 x 8 grid (all 16 (y0, z0) offsets of a 4 x 4 pencil,
+    every plane) plus random ones: the weight tile is placed by z0, the A operand by y0."""
+    grid, L = (8, 8, 8), 128
+    A, c, _ = workloads.small_case(grid, L, 1, ORTHO, seed=5)
+    rng = np.random.default_rng(6)
+    cells = np.stack(np.meshgrid(*[np.arange(n) for n in grid], indexing="ij"), -1).reshape(-1, 3)
+    u = (cells + rng.random(cells.shape)) / np.asarray(grid)
+    pos = np.concatenate([u @ np.asarray(A).reshape(3, 3), rng.random((3000, 3)) @ np.asarray(A).reshape(3, 3)])
+    t = tc_table(blip, A, grid, c)
+    compare(A, grid, c, pos, run_gpu(torch_cuda, blip, A, grid, c, pos, table=t))
+    assert blip.blipgpu_last_path(t.handle) == 5
+    t.close()
+
+
+def test_non_finite_positions_and_far_away_ones(torch_cuda, blip):
+    grid, L = (9, 10, 13), 130
+    A, c, pos = workloads.small_case(grid, L, 3000, TRICLINIC, seed=9, spread=50.0)
+    pos[7] = np.nan
+    pos[1234, 1] = np.inf
+    t = tc_table(blip, A, grid, c)
+    val, grad, lap, cell = run_gpu(torch_cuda, blip, A, grid, c, pos, table=t)
+    assert blip.blipgpu_last_path(t.handle) == 5
+    for e in (7, 1234):
+        assert np.isnan(val[e]).all() and np.isnan(grad[e]).all() and np.isnan(lap[e]).all() and (cell[e] == -1).all()
+    ok = np.ones(len(pos), bool); ok[[7, 1234]] = False
+    compare(A, grid, c, pos[ok], (val[ok], grad[ok], lap[ok], cell[ok]))
+    t.close()
+
+
+@pytest.mark.parametrize("scale", [1e-12, 3e-4, 1.0, 7e5, 1e20])
+def test_table_scale(torch_cuda, blip, scale):
+    """The coefficients go through fp16 after a power-of-two scaling by the table's max |c|: tables
+    far outside the fp16 range keep north_star's tolerances (which are relative to max |c|)."""
+    grid, L = (9, 10, 13), 130
+    A, c, pos = workloads.small_case(grid, L, 3000, TRICLINIC, seed=11)
+    c = (c * np.float32(scale)).astype(np.float32)
+    t = tc_table(blip, A, grid, c)
+    compare(A, grid, c, pos, run_gpu(torch_cuda, blip, A, grid, c, pos, table=t))
+    assert blip.blipgpu_last_path(t.handle) == 5
+    t.close()
+
+
+def test_sparse_table_with_a_few_large_entries(torch_cuda, blip):
+    """Most coefficients tiny against max |c| (they fall into fp16's subnormal range after scaling):
+    the error bound is absolute in max |c|, so the tolerances hold."""
+    grid, L = (9, 10, 13), 130
+    A, c, pos = workloads.small_case(grid, L, 3000, TRICLINIC, seed=12)
+    c = (c * np.float32(1e-6)).astype(np.float32)
+    c[::7, ::3, ::5, ::11] = np.float32(3.0)
+    t = tc_table(blip, A, grid, c)
+    compare(A, grid, c, pos, run_gpu(torch_cuda, blip, A, grid, c, pos, table=t))
+    t.close()
+
+
+def test_non_finite_table_falls_back_to_the_fp32_kernel(torch_cuda, blip):
+    """A NaN in the table would reach electrons that do not touch it through the zero-weight rows
+    of an MMA: such a table never takes the tensor-core path (EINVAL when forced)."""
+    grid, L = (9, 10, 13), 130
+    A, c, pos = workloads.small_case(grid, L, 3000, TRICLINIC, seed=13)
+    c[4, 5, 6, 77] = np.nan
+    t = blip.BlipTable(A, grid, L, c)
+    assert blip.lib().blipgpu_set_tuning(t.handle, 5, 0) == blip.EINVAL
+    val, grad, lap, cell = run_gpu(torch_cuda, blip, A, grid, c, pos, table=t)
+    assert blip.blipgpu_last_path(t.handle) == 2
+    oval, ograd, olap, ocell = oracle.eval_fast(A, grid, c, pos)
+    assert np.array_equal(np.isnan(val), np.isnan(oval)) and np.isnan(oval).any() and not np.isnan(oval).all()
+    t.close()
+
+
+def test_contraction_and_complex_entry_points_keep_the_fp32_kernel(torch_cuda, blip):
+    torch = torch_cuda
+    grid, L = (9, 10, 13), 130
+    A, c, pos = workloads.small_case(grid, L, 3000, TRICLINIC, seed=14)
+    t = tc_table(blip, A, grid, c)
+    M = pos.shape[0]
+    d = torch.randn((M, t.ld), dtype=torch.float32, device="cuda")
+    out = torch.empty((M, 8), dtype=torch.float32, device="cuda")
+    blip.blipgpu_eval_contract(t.handle, torch.from_numpy(pos).cuda(), M, blip.VGL, d, t.ld, out)
+    torch.cuda.synchronize()
+    assert blip.blipgpu_last_path(t.handle) == 2
+    t.close()
+
+
+def test_tio2_full_size_repeatable_and_close_to_the_fp32_kernel(torch_cuda, blip, tio2):
+    """Full TiO2 batch: 20 repeated calls return the bits of the first (no atomics, a fixed MMA
+    order per electron: a stale plane, B tile or accumulator would show as a flicker), and the
+    results agree with the FP32-pipe staged kernel to a fraction of the tolerances."""
+    torch = torch_cuda
+    cfg, A, c, table = tio2
+    dpos = torch.from_numpy(workloads.positions(cfg)).cuda()
+    M, ld = dpos.shape[0], table.ld
+
+    def call():
+        val = torch.empty((M, ld), dtype=torch.float32, device="cuda")
+        grad = torch.empty((M, 3, ld), dtype=torch.float32, device="cuda")
+        lap = torch.empty((M, ld), dtype=torch.float32, device="cuda")
+        blip.blipgpu_eval(table.handle, dpos, M, blip.VGL, val, grad, lap, ld)
+        return val, grad, lap
+
+    try:
+        blip.blipgpu_set_tuning(table.handle, path=5)
+        first = call()
+        assert blip.blipgpu_last_path(table.handle) == 5
+        for _ in range(20):
+            again = call()
+            torch.cuda.synchronize()
+            for a, b in zip(first, again):
+                assert torch.equal(a, b)
+            del again
+        blip.blipgpu_set_tuning(table.handle, path=2)
+        ref = call()
+        torch.cuda.synchronize()
+        tv, tg, tl = tolerances(A, cfg.grid, float(np.abs(c).max()))
+        assert float((first[0] - ref[0]).abs().max()) < 0.1 * tv
+        assert float((first[1] - ref[1]).abs().max()) < 0.1 * tg
+        assert float((first[2] - ref[2]).abs().max()) < 0.1 * tl
+    finally:
+        blip.blipgpu_set_tuning(table.handle, path=0)
+
+
+def test_replayed_from_a_cuda_graph(torch_cuda, blip):
+    """Grouping + tensor-core kernel captured once and replayed (an odd number of times): all state
+    between calls lives on the device; the bits of the eager call."""
+    torch = torch_cuda
+    grid, L = (12, 8, 8), 256
+    A, c, pos = workloads.small_case(grid, L, 6000, ORTHO, seed=15)
+    t = tc_table(blip, A, grid, c)
+    dpos = torch.from_numpy(pos).cuda()
+    M, ld = pos.shape[0], t.ld
+    val = torch.empty((M, ld), dtype=torch.float32, device="cuda"); grad = torch.empty((M, 3, ld), dtype=torch.float32, device="cuda")
+    lap = torch.empty((M, ld), dtype=torch.float32, device="cuda")
+    blip.blipgpu_reserve(t.handle, M)
+    s = torch.cuda.Stream()
+    with torch.cuda.stream(s):
+        blip.blipgpu_eval(t.handle, dpos, M, blip.VGL, val, grad, lap, ld, stream=s)
+        s.synchronize()
+        eager = (val.clone(), grad.clone(), lap.clone())
+        g = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(g, stream=s):
+            blip.blipgpu_eval(t.handle, dpos, M, blip.VGL, val, grad, lap, ld, stream=s)
+        for _ in range(3):
+            val.zero_(); grad.zero_(); lap.zero_()
+            g.replay()
+            s.synchronize()
+            assert torch.equal(val, eager[0]) and torch.equal(grad, eager[1]) and torch.equal(lap, eager[2])
+    t.close()
