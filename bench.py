@@ -227,7 +227,8 @@ def needs_l2_flush(cfg, args):
 # ---------------------------------------------------------------------------------------------
 # GPU arm
 # ---------------------------------------------------------------------------------------------
-KERNEL_NAMES = {1: "blip::eval_direct_kernel", 2: "blip::eval_staged_kernel", 3: "blip::eval_split_kernel"}
+KERNEL_NAMES = {1: "blip::eval_direct_kernel", 2: "blip::eval_staged_kernel", 3: "blip::eval_split_kernel",
+                5: "blip::eval_tc_kernel (tcgen05.mma, coefficient planes in tensor memory)"}
 FMA_PER_EVAL_CONTRACT = {True: 320, False: 64}      # SURVEY.md §8d R_fp32: five weights per site x 64 sites
 
 
@@ -301,6 +302,11 @@ def roofline_block(torch, blip, handle, cfg, M, L, mode_vgl, k_ms, g_ms, n_rows,
         "fp32_peak_tflops_measured": fp32_meas / 1e12, "fp32_peak_tflops_nominal": fp32_nominal / 1e12,
         "hbm_peak_GBps": peak_hbm,
     }
+    if blip.blipgpu_last_path(handle) == 5:
+        out["executed_on"] = ("tensor cores: the algorithm's FMAs are issued as 16 tcgen05.mma (M 128, N 16, K 16, fp16 x fp16 "
+                              "-> fp32, two-term splits of both operands) per electron and 128 orbitals, not on the FP32 pipe; "
+                              "SURVEY.md §8d's binding bound max(R_compulsory, R_fp32) is kept as the yardstick (frac > 1 would "
+                              "mean faster than the FP32 pipe could be at its peak)")
     traffic_file = os.path.join(ROOT, "profiles", "traffic.json")     # written from ncu --set full captures
     try:
         with open(traffic_file) as fh:
@@ -513,11 +519,20 @@ def run_gpu(args):
             line["hessian"] = run_hessian(torch, blip, handle, cfg, w.dpos, stream)
             ups = -(-M * ((L + 127) // 128) // nsm)                       # units (electron x 128 orbitals) per SM of this step
             tc = blip.blipgpu_probe_tensor(handle, ups, stream)
+            fp32_staged = None
+            if "eval_tc_kernel" in roofline["kernel"]:                    # the FP32-pipe staged kernel on the same batch, same run
+                blip.blipgpu_set_tuning(handle, 2, 0)
+                k2, g2 = kernel_times(w, 10)
+                blip.blipgpu_set_tuning(handle, 0, 0)
+                fp32_staged = {"kernel": KERNEL_NAMES[2], "kernel_ms": k2, "tensor_core_kernel_ms": roofline["kernel_ms"],
+                               "speedup": k2 / roofline["kernel_ms"]}
             line["tensor_core_recast"] = {
+                "shipped": fp32_staged,
                 "units_per_sm": ups, "ms_fp32_ffma2_form": tc[0], "ms_tf32x3_mma_sync_form": tc[1], "ms_tf32x1_mma_sync_form": tc[2],
                 "note": "arithmetic of one step from a shared-memory tile, no TMA / plane hand-offs (csrc/blip_tcprobe.cuh): "
                         "the K = 64 per-electron recast D[128][5] = C^T[128][64] W[64][5] on mma.sync.m16n8k8 tf32 with the "
-                        "3-term split the tolerances need, against the packed-FP32 form the kernels use (SURVEY.md §8f NEXT-2)"}
+                        "3-term split the tolerances need, against the packed-FP32 form (SURVEY.md §8f NEXT-2); `shipped` = the "
+                        "tcgen05 kernel that replaced the FP32-pipe staged kernel for this workload, both timed here"}
             if L % 2 == 0:
                 line["complex"] = run_complex(torch, blip, w, args)
         if world == 1 and not args.no_configs:
