@@ -26,14 +26,20 @@
 // (c1 + c2)(W1 + W2) summed over the sites in fp32: all four cross terms, error ~2^-21 of
 // sum |c W|.  Per electron and 128 orbitals: 4 planes x 2 row pairs x 2 halves = 16 MMAs.
 //
-// Roles of the persistent CTA (one per SM), 19 warps:
-//   producer (1)     work items and TMA of the table planes into a shared-memory ring — the
-//                    protocol of eval_staged_kernel;
-//   converters (4)   one per TMEM lane quarter: plane from shared memory -> scale, split, pack
-//                    -> tcgen05.st into a ring of 7 TMEM plane slots (2 x 28 columns each);
-//   weights (4)      one electron each: record -> 80 (column, quantity) weight vectors -> B tile
-//                    slot (4 KB) in the canonical K-major core-matrix layout;
-//   issuers (2)      one elected thread each: wait for B tile, planes and a free accumulator,
+// The scaled, split, z-paired fp16 words of A are not computed per launch: blipgpu_create writes them
+// once into a second library-owned table (tc_table_kernel below; same bytes per coefficient as the
+// fp32 table), so that a staged plane is moved to tensor memory word for word.
+//
+// Roles of the persistent CTA (one per SM), 29 warps:
+//   producer (1)     work items (chunk-major: all pencils of one 128-orbital slice of the table are
+//                    in flight together and find each other's halo rows in L2) and one 5-D TMA box
+//                    per plane into a ring of 4 shared-memory slots — the protocol of eval_staged_kernel;
+//   converters (2x4) a group per plane parity, a warp per TMEM lane quarter: the plane's 56 words per
+//                    orbital from shared memory -> tcgen05.st into a ring of 8 TMEM plane slots
+//                    (2 halves x 28 columns each);
+//   weights (8)      one electron each: record -> 80 (column, quantity) weight vectors, scaled and
+//                    split -> B tile slot (4 KB) in the canonical K-major core-matrix layout;
+//   issuers (4)      one elected thread each: wait for B tile, planes and a free accumulator,
 //                    issue the 16 MMAs, tcgen05.commit to free the B slot / publish D; planes are
 //                    given back to the converters by commit as the units move on;
 //   epilogue (2 x 4) tcgen05.ld of D, unscale, Cartesian gradient, streaming stores (a-5).
@@ -60,6 +66,12 @@ constexpr int kTcThreads = kTcWarps * 32;
 constexpr int kTcReaders = kTcNC + kTcNE + kTcNW + kTcNI;    // warps that walk the item queue
 static_assert(kTcDCol0 + 16 * kTcND <= 512, "tensor memory has 512 columns");
 static_assert(kTcNInfo >= kTcNB + kTcND, "unit info must outlive the B slot until the epilogue has read it");
+// An mbarrier wait names its phase by parity only, so a waiter must see EVERY phase of the barriers
+// it waits on (a waiter that skips one takes the phase before its own for complete): every ring
+// slot is therefore always waited for by the same warp(s) —
+static_assert(kTcNC == 8 && kTcRS % 2 == 0 && kTcRT % 2 == 0, "two converter groups alternate planes: a slot must keep its plane parity");
+static_assert(kTcNB % kTcNW == 0 && kTcNB % kTcNI == 0, "a B slot belongs to one weight warp and one issuer");
+static_assert(kTcND % kTcNI == 0 && kTcND % 2 == 0, "an accumulator slot belongs to one issuer and one epilogue group");
 
 struct TcScale {
     float sc;           // 2^kc applied to the coefficients
