@@ -40,5 +40,17 @@ def build(force=False, checked=False):
     return exe
 
 
+def build_tcgen05_check(force=False):
+    """tests/harness/tcgen05_check.cu -> tests/harness/tcgen05_check (nvcc, sm_100a): the tensor-memory /
+    tcgen05.mma facts the tensor-core kernel relies on, checked against a host loop."""
+    if ROOT not in sys.path:
+        sys.path.insert(0, ROOT)
+    from paper_1204_1121_b200 import _build
+    src, exe = os.path.join(HERE, "tcgen05_check.cu"), os.path.join(HERE, "tcgen05_check")
+    if force or not os.path.exists(exe) or os.path.getmtime(src) > os.path.getmtime(exe):
+        subprocess.run([_build.nvcc(), "-gencode", "arch=compute_100a,code=sm_100a", "-O2", "-o", exe, src], check=True)
+    return exe
+
+
 if __name__ == "__main__":
     print(build(force=True, checked="--checked" in sys.argv))

@@ -3,6 +3,10 @@ automatic choice takes for dense batches): parity with the oracle on every outpu
 layout makes special (ragged orbital chunks, grids that are not a multiple of the 4 x 4 pencil,
 every z offset of an electron in its pencil, non-finite positions, tables of very different
 scale), run-to-run bit identity, and the fall-backs."""
+import os
+import subprocess
+import sys
+
 import numpy as np
 import pytest
 
@@ -11,6 +15,20 @@ import workloads
 from test_gpu_parity import compare, compare_all, run_gpu, tolerances, torch_cuda, blip, tio2  # noqa: F401 (fixtures)
 
 pytestmark = pytest.mark.gpu
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+sys.path.insert(0, os.path.join(ROOT, "tests", "harness"))
+import build as harness_build  # noqa: E402
+
+
+def test_tcgen05_facts_the_kernel_relies_on():
+    """tests/harness/tcgen05_check.cu: fp16 pairs per TMEM column (low half first), A operand start at
+    multiples of 4 columns, the K-major no-swizzle B descriptor, accumulate flag, fp32 accumulator
+    read-back — each against a host loop, for kind::f16 (shipped) and kind::tf32."""
+    exe = harness_build.build_tcgen05_check()
+    r = subprocess.run([exe], capture_output=True, text=True, timeout=120)
+    assert r.returncode == 0, r.stdout + r.stderr
+    assert "tcgen05_check: 0 failure(s)" in r.stdout
 
 TRICLINIC = ((20.0, 0.0, 0.0), (3.0, 19.0, 0.0), (2.0, 2.0, 24.0))
 ORTHO = ((10.0, 0.0, 0.0), (0.0, 9.0, 0.0), (0.0, 0.0, 8.0))
