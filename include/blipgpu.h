@@ -95,7 +95,9 @@ int blipgpu_create(const double* lattice, const int* grid, int norb, const float
  * non-finite position gives NaN outputs and cell = -1 for that position (no error code:
  * detecting it would need a synchronisation).  Output pointers must be 16-byte aligned.
  * One handle serves one stream at a time (it owns the grouping workspace); if the
- * workspace must grow the call synchronises `stream` once — blipgpu_reserve avoids that.
+ * workspace must grow the call synchronises `stream` once — blipgpu_reserve avoids that (the first
+ * dense batch of a handle also builds the library's second copy of the table, the fp16 form its
+ * tensor-core kernel reads; blipgpu_reserve with that batch size does it ahead of time).
  * The call keeps no state on the host between calls and leaves its device workspace as it
  * found it, so once the workspace is reserved it may be captured in a CUDA graph and
  * replayed.
@@ -196,7 +198,10 @@ int blipgpu_eval_complex(blipgpu_table* t, const double* positions, long long M,
 
 /* blipgpu_reserve — pre-size the grouping workspace (bins, permutation, per-electron records)
  * for batches of up to M_max positions, so that blipgpu_eval never has to grow it (growing
- * synchronises the stream once).  Optional.  The device staging buffers of blipgpu_eval_host
+ * synchronises the stream once), and, if batches of M_max positions are dense enough for the
+ * staged kernels, build the fp16 copy of the table the tensor-core kernel reads (as much device
+ * memory again as the table).  Optional; needed before a call is captured in a CUDA graph (a
+ * capture cannot allocate: a dense call captured without it runs the FP32-pipe kernel).  The device staging buffers of blipgpu_eval_host
  * are sized by that call itself.  Errors: EINVAL, ENOMEM, ECUDA. */
 int blipgpu_reserve(blipgpu_table* t, long long M_max);
 

@@ -26,8 +26,8 @@
 // (c1 + c2)(W1 + W2) summed over the sites in fp32: all four cross terms, error ~2^-21 of
 // sum |c W|.  Per electron and 128 orbitals: 4 planes x 2 row pairs x 2 halves = 16 MMAs.
 //
-// The scaled, split, z-paired fp16 words of A are not computed per launch: blipgpu_create writes them
-// once into a second library-owned table (tc_table_kernel below; same bytes per coefficient as the
+// The scaled, split, z-paired fp16 words of A are not computed per launch: the library writes them
+// once (first use of this path, or blipgpu_reserve) into a second table of its own (tc_table_kernel below; same bytes per coefficient as the
 // fp32 table), so that a staged plane is moved to tensor memory word for word.
 //
 // Roles of the persistent CTA (one per SM), 29 warps:
@@ -163,38 +163,32 @@ __device__ __forceinline__ void tma_prefetch_5d(const CUtensorMap* tmap, int c0,
                  :: "l"(reinterpret_cast<uint64_t>(tmap)), "r"(c0), "r"(c1), "r"(c2), "r"(c3), "r"(c4) : "memory");
 }
 
-// The table of the tensor-core path (library-owned, built once by blipgpu_create next to the fp32
-// one): the ghost-padded table with every coefficient scaled by 2^kc and split in its two fp16
+// The table of the tensor-core path (library-owned, built from the padded fp32 table when the handle
+// first takes this path, or by blipgpu_reserve): the ghost-padded table with every coefficient scaled by 2^kc and split in its two fp16
 // halves, z sites in pairs, 32-bit words
 //     T16[p1][p2][zp][half][l] = { c_half[p1][p2][2 zp][l], c_half[p1][p2][2 zp + 1][l] << 16 }
 // — exactly the word a TMEM column of the A operand holds, so that the converter warps only move
 // words from the staged plane to tensor memory.  Same bytes per coefficient as fp32.
 __global__ void __launch_bounds__(256)
-tc_table_kernel(Geom g, float sc, int nzp, const float* __restrict__ src, unsigned* __restrict__ dst, long long total)
+tc_table_kernel(Geom g, float sc, int nzp, const float* __restrict__ padded /* [np1][np2][np3][pitch], the fp32 table */,
+                unsigned* __restrict__ dst, long long total)
 {
     const long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (idx >= total) return;
     const int pitch = 4 * g.pitch4;
     const int l = (int)(idx % pitch);
-    long long r = idx / pitch;
-    const int zp = (int)(r % nzp); r /= nzp;
-    const int p2 = (int)(r % g.np[1]);
-    const int p1 = (int)(r / g.np[1]);
-    const int k1 = (p1 + g.n[0] - 1) % g.n[0], k2 = (p2 + g.n[1] - 1) % g.n[1];
+    const long long r = idx / pitch;                         // (p1 np2 + p2) nzp + zp
+    const int zp = (int)(r % nzp);
+    const long long p12 = r / nzp;
     float c[2] = {0.f, 0.f};
-    if (l < g.L) {
 #pragma unroll
-        for (int h = 0; h < 2; ++h) {
-            const int p3 = 2 * zp + h;
-            if (p3 < g.np[2]) {
-                const int k3 = (p3 + g.n[2] - 1) % g.n[2];
-                c[h] = __fmul_rn(__ldg(src + (((size_t)k1 * g.n[1] + k2) * g.n[2] + k3) * (size_t)g.L + l), sc);
-            }
-        }
+    for (int h = 0; h < 2; ++h) {
+        const int p3 = 2 * zp + h;
+        if (p3 < g.np[2]) c[h] = __fmul_rn(__ldg(padded + ((size_t)p12 * g.np[2] + p3) * (size_t)pitch + l), sc);
     }
     unsigned h1, h2;
     tc_split2(c[0], c[1], h1, h2);
-    const size_t o = (((size_t)p1 * g.np[1] + p2) * nzp + zp) * 2 * (size_t)pitch + l;
+    const size_t o = (size_t)r * 2 * (size_t)pitch + l;
     dst[o] = h1;
     dst[o + pitch] = h2;
 }

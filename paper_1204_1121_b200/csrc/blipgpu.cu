@@ -160,6 +160,34 @@ static int ensure_workspace(blipgpu_table* t, long long M, cudaStream_t s)
     return BLIPGPU_OK;
 }
 
+static bool build_tensor_map16(blipgpu_table* t, int nzp);
+
+// The fp16-pair table of the tensor-core kernel (blip_tc.cuh) and its TMA descriptor, built from the
+// padded fp32 table the first time the handle takes that path (or by blipgpu_reserve): tables that
+// never see a dense batch — the 6.3 GB one of the large config — do not pay for it.  Allocates and
+// synchronises, like a workspace growth.  On failure the handle keeps the FP32-pipe staged kernel.
+static bool ensure_tc_table(blipgpu_table* t, cudaStream_t s)
+{
+    if (t->table16) return true;
+    if (!t->tc_ok) return false;
+    cudaStreamCaptureStatus cap = cudaStreamCaptureStatusNone;
+    if (cudaStreamIsCapturing(s, &cap) != cudaSuccess || cap != cudaStreamCaptureStatusNone) {
+        (void)cudaGetLastError();
+        return false;                                     // no allocation inside a capture: this call runs the FP32 kernel
+    }
+    const int nzp = (t->g.np[2] + 1) / 2;
+    const long long words = (long long)t->g.np[0] * t->g.np[1] * nzp * 2 * t->pitch;
+    bool fine = cudaMalloc(&t->table16, sizeof(unsigned) * (size_t)words) == cudaSuccess;
+    if (fine) {
+        const long long total = words / 2;
+        blip::tc_table_kernel<<<(unsigned)((total + 255) / 256), 256, 0, s>>>(t->g, t->tc_scale[0], nzp, reinterpret_cast<const float*>(t->table),
+                                                                           t->table16, total);
+        fine = cudaGetLastError() == cudaSuccess && cudaStreamSynchronize(s) == cudaSuccess && build_tensor_map16(t, nzp);
+    }
+    if (!fine) { cudaFree(t->table16); t->table16 = nullptr; t->tc_ok = 0; (void)cudaGetLastError(); }
+    return fine;
+}
+
 // TMA descriptor of the padded table for the staged kernel: 4-D tensor {pitch, n3+3, n2+3,
 // n1+3} of fp32, box {C, BZ+3, BY+3, 1} (one plane of a pencil's cross-section), no swizzle,
 // out-of-range elements read as zero.  cuTensorMapEncodeTiled is fetched through the runtime
@@ -329,7 +357,7 @@ extern "C" int blipgpu_create(const double* lattice, const int* grid, int norb,
     if (rc == BLIPGPU_OK) {
         unsigned* d_max = nullptr;
         if (cudaMalloc(&d_max, sizeof(unsigned)) == cudaSuccess && cudaMemsetAsync(d_max, 0, sizeof(unsigned), s) == cudaSuccess) {
-            blip::tc_absmax_kernel<<<(unsigned)(4 * t->nsm), 256, 0, s>>>(coeffs_on_device ? coeffs : staging, nsites * (long long)norb, d_max);
+            blip::tc_absmax_kernel<<<(unsigned)(4 * t->nsm), 256, 0, s>>>(reinterpret_cast<const float*>(t->table), nrows * pitch, d_max);
             if (cudaMemcpyAsync(&absmax_bits, d_max, sizeof(unsigned), cudaMemcpyDeviceToHost, s) != cudaSuccess ||
                 cudaStreamSynchronize(s) != cudaSuccess)
                 absmax_bits = 0x80000000u;
@@ -365,16 +393,6 @@ extern "C" int blipgpu_create(const double* lattice, const int* grid, int norb,
                 t->tc_scale[6 + q] = 1.0f / (t->tc_scale[0] * t->tc_scale[1 + q]);
                 fine = fine && std::isfinite(t->tc_scale[1 + q]) && t->tc_scale[1 + q] > 0.f && std::isfinite(t->tc_scale[6 + q]) && t->tc_scale[6 + q] > 0.f;
             }
-            // the fp16 table and its TMA descriptor (5-D: {pitch, half, z pair, p2, p1}, box {128, 2, 4, 7, 1})
-            const int nzp = (t->g.np[2] + 1) / 2;
-            const long long words = (long long)t->g.np[0] * t->g.np[1] * nzp * 2 * pitch;
-            if (fine && cudaMalloc(&t->table16, sizeof(unsigned) * (size_t)words) == cudaSuccess) {
-                const long long total = words / 2;
-                blip::tc_table_kernel<<<(unsigned)((total + 255) / 256), 256, 0, s>>>(t->g, t->tc_scale[0], nzp, coeffs_on_device ? coeffs : staging,
-                                                                                   t->table16, total);
-                fine = cudaGetLastError() == cudaSuccess && cudaStreamSynchronize(s) == cudaSuccess && build_tensor_map16(t, nzp);
-            } else fine = false;
-            if (!fine) { cudaFree(t->table16); t->table16 = nullptr; }
             t->tc_ok = fine ? 1 : 0;
         }
         (void)cudaGetLastError();
@@ -535,7 +553,7 @@ static int launch_eval(blipgpu_table* t, const double* positions, long long M, i
         if (t->profiling) CK(t, cudaEventRecord(t->pe[1], s));
         const StagedArgs a = {&t->tmap, &t->g, &t->sg, t->recs, t->order, t->meta, t->nchunk,
                               val, grad, lap, ld, dvec, ldd, cout, positions, kvec};
-        if ((t->path == 5 || t->path == 0) && t->tc_ok && !dvec && !kvec) {       // storing epilogue: on the tensor cores
+        if ((t->path == 5 || t->path == 0) && t->tc_ok && !dvec && !kvec && ensure_tc_table(t, s)) {   // storing epilogue: on the tensor cores
             blip::TcScale scl;
             scl.sc = t->tc_scale[0];
             for (int q = 0; q < 5; ++q) { scl.sw[q] = t->tc_scale[1 + q]; scl.inv[q] = t->tc_scale[6 + q]; }
@@ -675,6 +693,7 @@ extern "C" int blipgpu_reserve(blipgpu_table* t, long long M_max)
 {
     if (!t || M_max < 0 || M_max >= (1LL << 31)) return BLIPGPU_EINVAL;
     if (M_max == 0) return BLIPGPU_OK;
+    if (use_staged(t, M_max) && t->tc_ok && (t->path == 0 || t->path == 5)) (void)ensure_tc_table(t, nullptr);
     return ensure_workspace(t, M_max, nullptr);
 }
 
