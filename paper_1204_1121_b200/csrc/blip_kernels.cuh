@@ -126,9 +126,16 @@ __device__ __forceinline__ void order_items(const unsigned* start, int nbins, lo
         if (i < nps) {
             unsigned u0, u1;
             units_of(i, u0, u1);
-            const unsigned cnt = min(u1 - u0, (1u << 19) - 1u);
-            key = (cnt << 13) | (unsigned)i;
-            mine += (cnt != 0);
+            // sort key: (segment index along the pencil, ascending — with up to 4 segments per pencil),
+            // then electron count, descending.  All CTAs then work in the same stretch of the table
+            // at a time — neighbouring pencils find each other's halo rows in L2 — and take the
+            // heaviest items of that stretch first.
+            const unsigned raw = u1 - u0;
+            unsigned cnt, pri = 0;
+            if (sg.nseg <= 4) { cnt = min(raw, (1u << 17) - 1u); pri = raw ? 3u - (unsigned)(i % sg.nseg) : 0u; }   // empty items stay last
+            else cnt = min(raw, (1u << 19) - 1u);
+            key = (pri << 30) | (cnt << 13) | (unsigned)i;
+            mine += (raw != 0);
         }
         keys[i] = key;
     }
