@@ -213,6 +213,26 @@ static int run_selftest(void)
             if (path == 1) ok = ok && memcmp(h_staged, h_other, sizeof(float) * (mode ? 5 : 1) * nv) == 0;
             printf("selftest mode=%d path=%d M=%lld kernel=%d: %s\n", mode, path, Mp, blipgpu_last_path(t), ok ? "ok" : "FAIL");
             fails += !ok;
+            if (path == 2) {
+                /* the tensor-core staged kernel (tuning path 5) on the same batch: finite, and close to the
+                   FP32-pipe kernel's results (both are within a few % of the tolerances of the fp64 definition) */
+                BLIP_OK(blipgpu_set_tuning(t, 5, 0));
+                CUDA_OK(cudaMemset(val, 0, sizeof(float) * nv));
+                BLIP_OK(blipgpu_eval(t, dpos, Mp, mode, val, grad, lap, ld, cell, NULL));
+                CUDA_OK(cudaDeviceSynchronize());
+                CUDA_OK(cudaMemcpy(h_other, val, sizeof(float) * nv, cudaMemcpyDeviceToHost));
+                double worst = 0.0, scale = 0.0;
+                for (size_t i = 0; i < used; ++i) {
+                    const double d = fabs((double)h_other[i] - (double)h_staged[i]);
+                    if (d > worst) worst = d;
+                    if (fabs((double)h_staged[i]) > scale) scale = fabs((double)h_staged[i]);
+                }
+                ok = all_finite(h_other, used) && blipgpu_last_path(t) == 5 && worst <= 1e-5 * scale;
+                printf("selftest mode=%d path=5 M=%lld kernel=%d: %s (largest |value - FP32-pipe value| %.2e of %.2e)\n", mode, Mp,
+                       blipgpu_last_path(t), ok ? "ok" : "FAIL", worst, scale);
+                fails += !ok;
+                BLIP_OK(blipgpu_set_tuning(t, path, 0));
+            }
             /* contraction epilogue of the same kernel */
             BLIP_OK(blipgpu_eval_contract(t, dpos, Mp, mode, dvec, ld, cout, NULL, NULL));
             CUDA_OK(cudaDeviceSynchronize());

@@ -26,7 +26,7 @@ def test_harness_selftest():
     r = subprocess.run([harness_build.build(), "selftest"], capture_output=True, text=True, timeout=600)
     assert r.returncode == 0, r.stdout + r.stderr
     assert "selftest: 0 failure(s)" in r.stdout
-    assert "kernel=2" in r.stdout and "kernel=1" in r.stdout and "kernel=3" in r.stdout
+    assert "kernel=2" in r.stdout and "kernel=1" in r.stdout and "kernel=3" in r.stdout and "kernel=5" in r.stdout
 
 
 @pytest.mark.gpu
