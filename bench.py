@@ -467,7 +467,10 @@ def run_gpu(args):
     value = whole_job_value(M, L, world, ms_step)
 
     # ---- dominant kernel (gather + FMA) timed by the library's own events on the same stream
+    # (after half a second of idle: the chip is power-managed within tens of milliseconds — a kernel
+    # timed right behind the K steps runs at the sagging clock of their end, not of their average)
     fb = torch.empty(512 * 1024 * 1024, dtype=torch.uint8, device="cuda") if flush else None
+    time.sleep(0.5)
     k_ms, g_ms = kernel_times(w, min(args.steps, 20), fb)
     del fb
     fp32_meas = blip.blipgpu_probe_fp32(handle, stream) * 1e12        # packed-FMA rate measured in this run
@@ -522,7 +525,8 @@ def run_gpu(args):
             fp32_staged = None
             if "eval_tc_kernel" in roofline["kernel"]:                    # the FP32-pipe staged kernel on the same batch, same run
                 blip.blipgpu_set_tuning(handle, 2, 0)
-                k2, g2 = kernel_times(w, 10)
+                time.sleep(0.5)
+                k2, g2 = kernel_times(w, 20)
                 blip.blipgpu_set_tuning(handle, 0, 0)
                 fp32_staged = {"kernel": KERNEL_NAMES[2], "kernel_ms": k2, "tensor_core_kernel_ms": roofline["kernel_ms"],
                                "speedup": k2 / roofline["kernel_ms"]}
