@@ -465,6 +465,7 @@ eval_tc_kernel(const __grid_constant__ CUtensorMap tmap, Geom g, StagedGeom sg, 
                 }
                 if (col < 4 * g.pitch4 && !TC_KNOCK(4)) {
                     const size_t o = (size_t)(unsigned)e * (size_t)(unsigned)ld;
+                    BLIP_ASSERT((long long)col < ld);
                     __stcs(vcol + o, q[0]);
                     if (MODE != 0) {
                         float gx = q[1], gy = q[2], gz = q[3];
@@ -510,6 +511,8 @@ eval_tc_kernel(const __grid_constant__ CUtensorMap tmap, Geom g, StagedGeom sg, 
                 const int4 loc = *reinterpret_cast<const int4*>(rec4 + 23);       // {plane in item or -1, byte offset of row (i2, i3), -, electron}
                 const int rowi = loc.y / (128 * 4);                               // y0 * 7 + z0
                 const int y0 = rowi / 7, z0 = rowi - 7 * y0;
+                BLIP_ASSERT((long long)it_u0 + u < g.M && loc.w >= 0 && (long long)loc.w < g.M);       // record and electron within the batch
+                BLIP_ASSERT(loc.x < it_nplanes - 3 && loc.y >= 0 && y0 < 4 && z0 < 4);                  // block of sites inside the item's planes / pencil
                 float wz[3][4];
 #pragma unroll
                 for (int k = 0; k < 3; ++k)
@@ -576,6 +579,8 @@ eval_tc_kernel(const __grid_constant__ CUtensorMap tmap, Geom g, StagedGeom sg, 
                     if (uc >= kTcND) TCW(smem_u32(&sm.dempty[d]), ((uc / kTcND) & 1u) ^ 1u, wc_d);
                     TCP(3);
                     tc_fence_after();
+                    BLIP_ASSERT(!ok || (sq >= it_seq0 && sq + 4 <= it_seq0 + (unsigned)it_nplanes && sq + 4 <= waited && sq >= released &&
+                                        sq + 4 - released <= kTcRT && (unsigned)inf.y < 4u));       // the unit's 4 planes: converted, not handed back, within the ring
                     if (ok && !TC_KNOCK(1)) {
                         const unsigned dcol = tbase + kTcDCol0 + d * 16;
                         const uint64_t bd0 = tc_bdesc(smem_u32(&sm.bt[b][0]));

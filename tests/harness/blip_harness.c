@@ -255,7 +255,7 @@ static int run_selftest(void)
 }
 
 /* The TiO2-sized shape in the launch configuration bench.py times (49,152 positions x 768
- * orbitals, staged kernel), three calls of each entry point: for the checked build. */
+ * orbitals, staged kernels), three calls of each entry point: for the checked build. */
 static int run_fullsize(void)
 {
     const double A[9] = {17.4, 0, 0, 0, 17.4, 0, 0, 0, 11.2};
@@ -272,15 +272,17 @@ static int run_fullsize(void)
     CUDA_OK(cudaMalloc((void**)&grad, sizeof(float) * 3 * (size_t)M * ld));
     CUDA_OK(cudaMalloc((void**)&lap, sizeof(float) * (size_t)M * ld));
     CUDA_OK(cudaMalloc((void**)&cout, sizeof(float) * 8 * (size_t)M));
-    int fails = 0;
+    int fails = 0, kernel_eval = 0;
     for (int rep = 0; rep < 3; ++rep) {
         BLIP_OK(blipgpu_eval(t, dpos, M, BLIPGPU_VGL, val, grad, lap, ld, NULL, NULL));
         BLIP_OK(blipgpu_eval(t, dpos, M, BLIPGPU_VALUE, val, NULL, NULL, ld, NULL, NULL));
+        kernel_eval = blipgpu_last_path(t);
         BLIP_OK(blipgpu_eval_contract(t, dpos, M, BLIPGPU_VGL, lap, ld, cout, NULL, NULL));
         CUDA_OK(cudaDeviceSynchronize());
     }
-    printf("fullsize: kernel=%d\n", blipgpu_last_path(t));
-    fails += blipgpu_last_path(t) != 2;
+    /* the storing calls run the tensor-core staged kernel (5), the contraction the FP32-pipe one (2) */
+    printf("fullsize: kernel=%d (eval), kernel=%d (contract)\n", kernel_eval, blipgpu_last_path(t));
+    fails += kernel_eval != 5 || blipgpu_last_path(t) != 2;
     {
         float* h = (float*)malloc(sizeof(float) * (size_t)M * ld);
         CUDA_OK(cudaMemcpy(h, val, sizeof(float) * (size_t)M * ld, cudaMemcpyDeviceToHost));
