@@ -54,6 +54,24 @@ def test_every_output_against_the_oracle(torch_cuda, blip, grid, L, lat, mode):
     t.close()
 
 
+@pytest.mark.parametrize("grid,L,M,path", [((45, 8, 8), 128, 6000, 5), ((130, 8, 12), 128, 9000, 5), ((130, 8, 12), 128, 9000, 2),
+                                            ((4, 372, 372), 128, 20000, 5)])
+def test_segmented_pencils_and_many_work_items(torch_cuda, blip, grid, L, M, path):
+    """Pencils cut into segments with a ragged last one (45 planes -> 4 segments of 12, 12, 12, 9), more
+    than 4 segments per pencil (the work items are then sorted by load only), and 93 x 93 pencils
+    (> 8,192 work items: left in id order, the empty ones skipped by every role of the kernel)."""
+    # spacings within 10 % of one another (DESIGN.md reading R13a: the Laplacian tolerance is tied to the largest one)
+    lat = ((0.26 * grid[0], 0.0, 0.0), (0.4, 0.25 * grid[1], 0.0), (0.1, 0.2, 0.255 * grid[2]))
+    A, c, pos = workloads.small_case(grid, L, M, lat, seed=grid[0] + path, spread=1.5)
+    t = blip.BlipTable(A, grid, L, c)
+    blip.blipgpu_set_tuning(t.handle, path=path)
+    val, grad, lap, cell = run_gpu(torch_cuda, blip, A, grid, c, pos, table=t)
+    assert blip.blipgpu_last_path(t.handle) == path
+    pick = np.arange(0, M, 3)
+    compare(A, grid, c, pos[pick], (val[pick], grad[pick], lap[pick], cell[pick]))
+    t.close()
+
+
 def test_every_cell_offset_in_a_pencil(torch_cuda, blip):
     """One electron in every cell of an 8 x 8 x 8 grid (all 16 (y0, z0) offsets of a 4 x 4 pencil,
     every plane) plus random ones: the weight tile is placed by z0, the A operand by y0."""
