@@ -75,3 +75,45 @@ def test_random_shape(torch_cuda, blip, seed):
                 assert np.abs(grad.cpu().numpy()[good] - ograd[good]).max() <= tg
                 assert np.abs(lap.cpu().numpy()[good] - olap[good]).max() <= tl
     t.close()
+
+
+@pytest.mark.parametrize("seed", range(16))
+def test_random_shape_tensor_core_kernel(torch_cuda, blip, seed):
+    """The same draw for the tensor-core staged kernel (tuning path 5 forced): orbital counts from one
+    ragged 128-orbital chunk to five, batches from just above the grouping threshold to 20,000,
+    grids from 4 points per axis (every block wraps; TMA boxes hang over the table on all sides)."""
+    torch = torch_cuda
+    rng = np.random.default_rng(5000 + seed)
+    grid = tuple(int(x) for x in rng.integers(4, 40, size=3))
+    L = int(rng.choice([125, 128, 129, 200, 256, 300, 513]))
+    M = int(rng.choice([2049, 5000, 20000]))
+    if rng.random() < 0.4:
+        lat = np.diag(rng.uniform(3, 12, size=3))
+    else:
+        lat = np.diag(rng.uniform(5, 12, size=3)) + rng.uniform(-1.5, 1.5, size=(3, 3))
+    while True:                                             # DESIGN.md reading R13a, as above
+        hs = oracle.spacing(lat, grid)
+        if hs.max() / hs.min() <= 10.0:
+            break
+        grid = tuple(int(x) for x in rng.integers(4, 40, size=3))
+    mode = int(rng.choice([0, 1, 1]))
+    spread = float(rng.choice([0.05, 1.0, 3.0, 30.0]))
+    A, c, pos = workloads.small_case(grid, L, M, lat, seed=seed, spread=spread)
+    if rng.random() < 0.3:
+        pos[rng.integers(0, M, size=2)] = np.nan
+    t = blip.BlipTable(A, grid, L, c)
+    blip.blipgpu_set_tuning(t.handle, 5, 0)
+    oval, ograd, olap, ocell = oracle.eval_fast(A, grid, c, pos, mode=mode)
+    tv, tg, tl = tolerances(A, grid, float(np.abs(c).max()))
+    good = ~np.isnan(oval).any(axis=1)
+    val, grad, lap, cell = t.eval(torch.from_numpy(pos).cuda(), mode=mode, want_cell=True)
+    torch.cuda.synchronize()
+    assert blip.blipgpu_last_path(t.handle) == 5
+    val = val.cpu().numpy()
+    assert np.array_equal(cell.cpu().numpy(), ocell)
+    assert np.isnan(val[~good]).all()
+    assert np.abs(val[good] - oval[good]).max() <= tv
+    if mode:
+        assert np.abs(grad.cpu().numpy()[good] - ograd[good]).max() <= tg
+        assert np.abs(lap.cpu().numpy()[good] - olap[good]).max() <= tl
+    t.close()
