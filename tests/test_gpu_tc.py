@@ -219,3 +219,36 @@ def test_replayed_from_a_cuda_graph(torch_cuda, blip):
             s.synchronize()
             assert torch.equal(val, eager[0]) and torch.equal(grad, eager[1]) and torch.equal(lap, eager[2])
     t.close()
+
+
+def test_soak_random_batch_sizes(torch_cuda, blip, tio2):
+    """Thousands of back-to-back calls with random batch sizes and position windows (every tenth the
+    full batch, whose checksum must never change): a lost hand-off between the kernel's five roles
+    would hang or flicker.  BLIP_SOAK_CALLS (read here) lengthens the run; profiles/r2_checks.md
+    records one with 300,000 calls."""
+    torch = torch_cuda
+    cfg, A, c, table = tio2
+    rng = np.random.default_rng(7)
+    p = torch.from_numpy(workloads.positions(cfg)).cuda()
+    Mmax, ld = p.shape[0], table.ld
+    val = torch.empty((Mmax, ld), dtype=torch.float32, device="cuda")
+    grad = torch.empty((Mmax, 3, ld), dtype=torch.float32, device="cuda")
+    lap = torch.empty((Mmax, ld), dtype=torch.float32, device="cuda")
+    ncalls = int(os.environ.get("BLIP_SOAK_CALLS", "5000"))
+    ref = None
+    try:
+        blip.blipgpu_set_tuning(table.handle, path=5)
+        for it in range(ncalls):
+            M = int(rng.integers(2049, Mmax + 1)) if it % 10 else Mmax
+            off = int(rng.integers(0, Mmax - M + 1))
+            blip.blipgpu_eval(table.handle, p[off:off + M], M, blip.VGL, val, grad, lap, ld)
+            if it % 10 == 0:
+                torch.cuda.synchronize()
+                s = (float(val[:, :cfg.norb].sum()), float(lap[:, :cfg.norb].abs().max()))
+                assert np.isfinite(s[0]) and np.isfinite(s[1])
+                ref = s if ref is None else ref
+                assert s == ref
+        torch.cuda.synchronize()
+        assert blip.blipgpu_last_path(table.handle) == 5
+    finally:
+        blip.blipgpu_set_tuning(table.handle, path=0)
