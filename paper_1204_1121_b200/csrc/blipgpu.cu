@@ -470,14 +470,19 @@ static const long long kSplitMax = 16384;
 // The staged path pays (BY+3)(BZ+3)/(BY BZ) table rows per cell whatever the batch; it wins
 // once the rows are shared by enough electrons (average number of electrons touching a row).
 static const double kStagedMinReuse = 6.0;
+// ... the tensor-core form spends less per electron and wins from 4.5 on (TiO2 table, L2 flushed:
+// 12,288 positions = 4.8 electrons per row: 0.235 ms against 0.247 ms for the grouped direct kernel
+// and 0.282 ms for the FP32-pipe staged kernel; 9,216 = 3.6: 0.224 against 0.196 ms)
+static const double kStagedMinReuseTc = 4.5;
 
-static bool use_staged(const blipgpu_table* t, long long M)
+// tc: the call can take the tensor-core form (storing epilogue, finite table)
+static bool use_staged(const blipgpu_table* t, long long M, bool tc)
 {
     if (!t->staged_ok || t->path == 1) return false;
     if (t->path == 2 || t->path == 5) return true;
     if (M <= kGroupThreshold) return false;
     const double sites = (double)t->g.n[0] * t->g.n[1] * t->g.n[2];
-    return 64.0 * (double)M / sites >= kStagedMinReuse;
+    return 64.0 * (double)M / sites >= (tc ? kStagedMinReuseTc : kStagedMinReuse);
 }
 
 // dvec != NULL: contraction mode (blipgpu_eval_contract): the orbitals are not stored but
@@ -491,7 +496,8 @@ static int launch_eval(blipgpu_table* t, const double* positions, long long M, i
         return launch_hess<float>(t, positions, M, val, grad, lap, ld, cell, s);
     const int* perm = nullptr;
     t->g.M = M;                                              // bound of the checked build's asserts
-    const bool staged = use_staged(t, M);
+    const bool tc_call = t->tc_ok && !dvec && !kvec && (t->path == 0 || t->path == 5);
+    const bool staged = use_staged(t, M, tc_call);
     const int kmode = mode == BLIPGPU_VALUE ? 0 : (t->diag ? 2 : 1);      // kernel template MODE
     if (t->profiling) CK(t, cudaEventRecord(t->pe[0], s));
     const bool grouped = staged || t->path == 1 ||
@@ -693,7 +699,7 @@ extern "C" int blipgpu_reserve(blipgpu_table* t, long long M_max)
 {
     if (!t || M_max < 0 || M_max >= (1LL << 31)) return BLIPGPU_EINVAL;
     if (M_max == 0) return BLIPGPU_OK;
-    if (use_staged(t, M_max) && t->tc_ok && (t->path == 0 || t->path == 5)) (void)ensure_tc_table(t, nullptr);
+    if (t->tc_ok && (t->path == 0 || t->path == 5) && use_staged(t, M_max, true)) (void)ensure_tc_table(t, nullptr);
     return ensure_workspace(t, M_max, nullptr);
 }
 
