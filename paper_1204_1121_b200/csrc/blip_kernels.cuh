@@ -1256,9 +1256,6 @@ struct StagedCfg {
 // EPI: what happens to a unit's results (a-5): 0 stored, 1 contracted with d (blipgpu_eval_contract),
 // 2 stored as complex orbitals with a Bloch phase (blipgpu_eval_complex).
 constexpr int kEpiStore = 0, kEpiContract = 1, kEpiComplex = 2;
-#ifdef BLIP_TC_PROF
-__device__ unsigned long long g_sp_prof[2];
-#endif
 template <int MODE, int EPI, int VEC, int BY, int BZ, int R, int NW>
 __global__ void __launch_bounds__((NW + 1) * 32, 1)
 eval_staged_kernel(const __grid_constant__ CUtensorMap tmap, Geom g, StagedGeom sg,
@@ -1278,10 +1275,6 @@ eval_staged_kernel(const __grid_constant__ CUtensorMap tmap, Geom g, StagedGeom 
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     wait_for_predecessor();
-#ifdef BLIP_TC_PROF
-    const long long sp_c0 = clock64();
-    unsigned long long sp_g0; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(sp_g0));
-#endif
     if (threadIdx.x == 0) {
         for (int s = 0; s < R; ++s) { mbar_init(smem_u32(&sm.full[s]), 1); mbar_init(smem_u32(&sm.empty[s]), NW); }
         for (int s = 0; s < (int)IQ; ++s) { mbar_init(smem_u32(&sm.ifull[s]), 1); mbar_init(smem_u32(&sm.iempty[s]), NW); }
@@ -1512,13 +1505,6 @@ eval_staged_kernel(const __grid_constant__ CUtensorMap tmap, Geom g, StagedGeom 
         __syncwarp();
         u += NW;
     }
-#ifdef BLIP_TC_PROF
-    if (threadIdx.x == 0) {
-        unsigned long long g1; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(g1));
-        atomicMax(&g_sp_prof[0], (unsigned long long)(clock64() - sp_c0));
-        atomicMax(&g_sp_prof[1], g1 - sp_g0);
-    }
-#endif
 }
 
 }  // namespace blip

@@ -248,30 +248,6 @@ __device__ __forceinline__ void tc_build_tile(const float4* rec4, const float* r
     }
 }
 
-#ifdef BLIP_TC_PROF
-__device__ int g_tc_knock;           // timing knock-outs (results wrong): 1 no MMAs, 2 no B build, 4 no output stores, 8 no plane conversion
-#define TC_KNOCK(bit) (g_tc_knock & (bit))
-__device__ unsigned long long g_tc_prof[64];
-#define TCP_DECL long long tcp_t = clock64(); long long tcp_a[6] = {0, 0, 0, 0, 0, 0}
-#define TCP(k) do { const long long t1_ = clock64(); tcp_a[k] += t1_ - tcp_t; tcp_t = t1_; } while (0)
-#define TCP_FLUSH(base, leader) do { if (blockIdx.x == 0 && (leader)) { for (int k_ = 0; k_ < 6; ++k_) atomicAdd(&g_tc_prof[(base) + k_], (unsigned long long)tcp_a[k_]); } } while (0)
-// wait that records: [0] calls satisfied at once, [1] calls that had to wait, [2] cycles waited
-__device__ __forceinline__ void mbar_wait_prof(unsigned bar, unsigned parity, long long* c)
-{
-    if (mbar_test(bar, parity)) { c[0] += 1; return; }
-    const long long t0 = clock64();
-    mbar_wait(bar, parity);
-    c[1] += 1; c[2] += clock64() - t0;
-}
-#define TCW(bar, par, c) mbar_wait_prof(bar, par, c)
-#else
-#define TCW(bar, par, c) mbar_wait(bar, par)
-#define TC_KNOCK(bit) false
-#define TCP_DECL do { } while (0)
-#define TCP(k) do { } while (0)
-#define TCP_FLUSH(base, leader) do { } while (0)
-#endif
-
 template <int MODE>
 __global__ void __launch_bounds__(kTcThreads, 1)
 eval_tc_kernel(const __grid_constant__ CUtensorMap tmap, Geom g, StagedGeom sg, TcScale scl,
@@ -284,10 +260,6 @@ eval_tc_kernel(const __grid_constant__ CUtensorMap tmap, Geom g, StagedGeom sg, 
     constexpr int PLANE_BYTES = kTcPlaneWords * 4;
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     wait_for_predecessor();
-#ifdef BLIP_TC_PROF
-    const long long tcp_start = clock64();
-    unsigned long long tcp_g0; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(tcp_g0));
-#endif
     if (warp == 0) {
         asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], 512;" :: "r"(smem_u32(&sm.tbase)) : "memory");
         asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
@@ -376,16 +348,13 @@ eval_tc_kernel(const __grid_constant__ CUtensorMap tmap, Geom g, StagedGeom sg, 
         const int cq = warp & 3, cg = warp >> 2;             // lane quarter; group cg converts the planes with (sequence number) % 2 == cg
         const unsigned tlane = tbase + ((unsigned)(cq * 32) << 16);
         const int orb = cq * 32 + lane;
-        TCP_DECL;
         for (unsigned n = 0;; ++n) {
             load_item(n);
-            TCP(0);
             if (it_nplanes < 0) break;
             for (int j = (int)((it_seq0 + (unsigned)cg) & 1u); j < it_nplanes; j += 2) {
                 const unsigned q = it_seq0 + (unsigned)j;
                 const unsigned s = q % kTcRS, t = q % kTcRT;
                 mbar_wait_relaxed(smem_u32(&sm.full[s]), (q / kTcRS) & 1u);
-                TCP(1);
                 // rows 0..3 of the plane (32 words, all loads in flight at once) wait in registers for the
                 // TMEM slot; rows 4..6 follow behind the first stores (56 words at once do not fit in the
                 // 64 registers a thread of this 928-thread CTA has)
@@ -411,29 +380,24 @@ eval_tc_kernel(const __grid_constant__ CUtensorMap tmap, Geom g, StagedGeom sg, 
                         }
                 };
                 unsigned ha[4][8], hb[4][8];
-                if (!TC_KNOCK(8)) ld_rows(ha, 0, 4);
+                ld_rows(ha, 0, 4);
                 if (q >= kTcRT) mbar_wait_relaxed(smem_u32(&sm.tempty[t]), ((q / kTcRT) & 1u) ^ 1u);
-                TCP(2);
                 tc_fence_after();
-                if (!TC_KNOCK(8)) { st_rows(ha, 0, 4); ld_rows(hb, 4, 3); st_rows(hb, 4, 3); }
+                st_rows(ha, 0, 4); ld_rows(hb, 4, 3); st_rows(hb, 4, 3);
                 asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
                 tc_fence_before();
                 __syncwarp();
                 if (lane == 0) { mbar_arrive(smem_u32(&sm.tfull[t])); mbar_arrive(smem_u32(&sm.empty[s])); }
-                TCP(3);
             }
             leave_item(n, false);
         }
-        TCP_FLUSH(0, warp == 0 && lane == 0);
     } else if (warp < kTcNC + kTcNE) {
         // ---- epilogue: group eg takes the units with (unit number) % 2 == eg; lane quarter sp
         const int eg = (warp - kTcNC) >> 2, sp = warp & 3;
         const unsigned tl = tbase + ((unsigned)(sp * 32) << 16) + kTcDCol0;
         unsigned ubase = 0;
-        TCP_DECL;
         for (unsigned n = 0;; ++n) {
             load_item(n);
-            TCP(0);
             if (it_nplanes < 0) break;
             const int col = it_chunk * 128 + sp * 32 + lane;
             float* const vcol = val + col;
@@ -442,7 +406,6 @@ eval_tc_kernel(const __grid_constant__ CUtensorMap tmap, Geom g, StagedGeom sg, 
             for (unsigned u = (ubase + (unsigned)eg) & 1u; u < it_nunits; u += 2) {      // (ubase + u) % 2 == eg
                 const unsigned uc = ubase + u, d = uc % kTcND;
                 mbar_wait_relaxed(smem_u32(&sm.dfull[d]), (uc / kTcND) & 1u);
-                TCP(1);
                 tc_fence_after();
                 const int4 inf = sm.info[uc % kTcNInfo];
                 unsigned r[10];
@@ -454,7 +417,6 @@ eval_tc_kernel(const __grid_constant__ CUtensorMap tmap, Geom g, StagedGeom sg, 
                 tc_fence_before();
                 __syncwarp();
                 if (lane == 0) mbar_arrive(smem_u32(&sm.dempty[d]));
-                TCP(2);
                 const int e = inf.z;
                 BLIP_ASSERT(e >= 0 && (long long)e < g.M);
                 float q[5];
@@ -463,7 +425,7 @@ eval_tc_kernel(const __grid_constant__ CUtensorMap tmap, Geom g, StagedGeom sg, 
                 if (inf.x < 0) {                             // non-finite position (R17): the same for the whole warp
                     q[0] = q[1] = q[2] = q[3] = q[4] = __int_as_float(0x7fc00000);
                 }
-                if (col < 4 * g.pitch4 && !TC_KNOCK(4)) {
+                if (col < 4 * g.pitch4) {
                     const size_t o = (size_t)(unsigned)e * (size_t)(unsigned)ld;
                     BLIP_ASSERT((long long)col < ld);
                     __stcs(vcol + o, q[0]);
@@ -481,22 +443,18 @@ eval_tc_kernel(const __grid_constant__ CUtensorMap tmap, Geom g, StagedGeom sg, 
                         __stcs(lcol + o, q[4]);
                     }
                 }
-                TCP(3);
             }
             ubase += it_nunits;
             leave_item(n, false);
         }
-        TCP_FLUSH(8, warp == kTcNC && lane == 0);
     } else if (warp < kTcNC + kTcNE + kTcNW) {
         // ---- weight warps: warp ww takes the units with (unit number) % kTcNW == ww
         const int ww = warp - (kTcNC + kTcNE);
         float4* const rec4 = sm.wrec[ww];
         const float* const recf = reinterpret_cast<const float*>(rec4);
         unsigned ubase = 0;
-        TCP_DECL;
         for (unsigned n = 0;; ++n) {
             load_item(n);
-            TCP(0);
             if (it_nplanes < 0) break;
             const float4* rsrc = recs + (size_t)it_u0 * (kRecFloats / 4);
             unsigned u = ((unsigned)ww + kTcNW - (ubase % kTcNW)) % kTcNW;
@@ -518,11 +476,9 @@ eval_tc_kernel(const __grid_constant__ CUtensorMap tmap, Geom g, StagedGeom sg, 
                 for (int k = 0; k < 3; ++k)
 #pragma unroll
                     for (int m = 0; m < 4; ++m) wz[k][m] = recf[80 + 4 * k + m];
-                TCP(1);
                 if (uc >= kTcNB) mbar_wait_relaxed(smem_u32(&sm.bempty[b]), ((uc / kTcNB) & 1u) ^ 1u);
-                TCP(2);
                 unsigned char* const bt = sm.bt[b];
-                if (!TC_KNOCK(2)) {
+                {
                     switch (z0) {                              // the same for the whole warp: placement of the 4 fp16 at compile time
                         case 0: tc_build_tile<0>(rec4, recf, wz, scl, bt, lane); break;
                         case 1: tc_build_tile<1>(rec4, recf, wz, scl, bt, lane); break;
@@ -534,54 +490,44 @@ eval_tc_kernel(const __grid_constant__ CUtensorMap tmap, Geom g, StagedGeom sg, 
                 asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
                 __syncwarp();
                 if (lane == 0) mbar_arrive(smem_u32(&sm.bfull[b]));
-                TCP(3);
             }
             ubase += it_nunits;
             leave_item(n, false);
         }
-        TCP_FLUSH(16, ww == 0 && lane == 0);
     } else {
-        // ---- issuers: one elected thread of warp ii takes the units with (unit number) % 2 == ii
+        // ---- issuers: one elected thread of warp ii takes the units with (unit number) % kTcNI == ii
         const int ii = warp - (kTcNC + kTcNE + kTcNW);
         if (tc_elect_one()) {
             unsigned ubase = 0, waited = 0, released = 0;
-#ifdef BLIP_TC_PROF
-            long long wc_t[3] = {0, 0, 0}, wc_b[3] = {0, 0, 0}, wc_d[3] = {0, 0, 0};
-#endif
             const unsigned tfull0 = smem_u32(&sm.tfull[0]), tempty0 = smem_u32(&sm.tempty[0]);
             // planes < end are no longer needed by this issuer: each is handed back to the converters
             // (commit: the arrival waits for the MMAs issued so far) once it has been seen full, so
             // that every arrival belongs to the current phase of its barrier
             auto pass_upto = [&](unsigned end) {
                 while (released < end) {
-                    if (released >= waited) { TCW(tfull0 + 8u * (released % kTcRT), (released / kTcRT) & 1u, wc_t); waited = released + 1; }
+                    if (released >= waited) { mbar_wait(tfull0 + 8u * (released % kTcRT), (released / kTcRT) & 1u); waited = released + 1; }
                     tc_commit(tempty0 + 8u * (released % kTcRT));
                     ++released;
                 }
             };
-            TCP_DECL;
             for (unsigned n = 0;; ++n) {
                 load_item(n);
-                TCP(0);
                 if (it_nplanes < 0) break;
                 for (unsigned u = ((unsigned)ii + kTcNI - (ubase % kTcNI)) % kTcNI; u < it_nunits; u += kTcNI) {
                     const unsigned uc = ubase + u, b = uc % kTcNB, d = uc % kTcND;
-                    TCW(smem_u32(&sm.bfull[b]), (uc / kTcNB) & 1u, wc_b);
-                    TCP(1);
+                    mbar_wait(smem_u32(&sm.bfull[b]), (uc / kTcNB) & 1u);
                     const int4 inf = sm.info[uc % kTcNInfo];
                     const bool ok = inf.x >= 0;
                     const unsigned sq = (unsigned)inf.x;
                     if (ok) {
                         pass_upto(sq);
-                        while (waited < sq + 4) { TCW(tfull0 + 8u * (waited % kTcRT), (waited / kTcRT) & 1u, wc_t); ++waited; }
+                        while (waited < sq + 4) { mbar_wait(tfull0 + 8u * (waited % kTcRT), (waited / kTcRT) & 1u); ++waited; }
                     }
-                    TCP(2);
-                    if (uc >= kTcND) TCW(smem_u32(&sm.dempty[d]), ((uc / kTcND) & 1u) ^ 1u, wc_d);
-                    TCP(3);
+                    if (uc >= kTcND) mbar_wait(smem_u32(&sm.dempty[d]), ((uc / kTcND) & 1u) ^ 1u);
                     tc_fence_after();
                     BLIP_ASSERT(!ok || (sq >= it_seq0 && sq + 4 <= it_seq0 + (unsigned)it_nplanes && sq + 4 <= waited && sq >= released &&
                                         sq + 4 - released <= kTcRT && (unsigned)inf.y < 4u));       // the unit's 4 planes: converted, not handed back, within the ring
-                    if (ok && !TC_KNOCK(1)) {
+                    if (ok) {
                         const unsigned dcol = tbase + kTcDCol0 + d * 16;
                         const uint64_t bd0 = tc_bdesc(smem_u32(&sm.bt[b][0]));
                         const unsigned ay = tbase + 4u * (unsigned)inf.y;
@@ -596,32 +542,13 @@ eval_tc_kernel(const __grid_constant__ CUtensorMap tmap, Geom g, StagedGeom sg, 
                     }
                     tc_commit(smem_u32(&sm.bempty[b]));
                     tc_commit(smem_u32(&sm.dfull[d]));
-                    TCP(4);
                 }
                 if (it_nplanes > 0) pass_upto(it_seq0 + (unsigned)it_nplanes);
-                TCP(5);
                 ubase += it_nunits;
                 leave_item(n, true);
             }
-            TCP_FLUSH(24, ii == 0);
-#ifdef BLIP_TC_PROF
-            if (blockIdx.x == 0 && ii == 0)
-                for (int k = 0; k < 3; ++k) { g_tc_prof[52 + k] = wc_b[k]; g_tc_prof[55 + k] = wc_t[k]; g_tc_prof[58 + k] = wc_d[k]; }
-#endif
         }
     }
-#ifdef BLIP_TC_PROF
-    if (threadIdx.x == 0) {
-        const unsigned long long dt = (unsigned long long)(clock64() - tcp_start);
-        atomicMax(&g_tc_prof[40], dt);
-        atomicMin(&g_tc_prof[41], dt);
-        atomicAdd(&g_tc_prof[42], dt);
-        unsigned long long g1; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(g1));
-        atomicMin(&g_tc_prof[43], tcp_g0);
-        atomicMax(&g_tc_prof[44], g1);
-        atomicMax(&g_tc_prof[45], g1 - tcp_g0);
-    }
-#endif
     tc_fence_before();
     __syncthreads();
     if (warp == 0) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, 512;" :: "r"(tbase) : "memory");

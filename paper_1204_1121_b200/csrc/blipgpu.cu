@@ -683,18 +683,6 @@ extern "C" int blipgpu_eval_f64(blipgpu_table* t, const double* positions, long 
     return BLIPGPU_OK;
 }
 
-#ifdef BLIP_TC_PROF
-extern "C" int blipgpu_tc_knock(int k) { return cudaMemcpyToSymbol(blip::g_tc_knock, &k, sizeof(int)) == cudaSuccess ? 0 : -3; }
-extern "C" int blipgpu_tc_prof(unsigned long long* out, int reset)
-{
-    if (out && cudaMemcpyFromSymbol(out, blip::g_tc_prof, sizeof(unsigned long long) * 64) != cudaSuccess) return -3;
-    if (out) (void)cudaMemcpyFromSymbol(out + 48, blip::g_sp_prof, sizeof(unsigned long long) * 2);
-    if (reset) { unsigned long long z2[2] = {0, 0}; (void)cudaMemcpyToSymbol(blip::g_sp_prof, z2, sizeof(z2)); }
-    if (reset) { unsigned long long z[64] = {0}; z[41] = ~0ull; z[43] = ~0ull; if (cudaMemcpyToSymbol(blip::g_tc_prof, z, sizeof(z)) != cudaSuccess) return -3; }
-    return 0;
-}
-#endif
-
 extern "C" int blipgpu_reserve(blipgpu_table* t, long long M_max)
 {
     if (!t || M_max < 0 || M_max >= (1LL << 31)) return BLIPGPU_EINVAL;
