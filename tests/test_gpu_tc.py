@@ -252,3 +252,38 @@ def test_soak_random_batch_sizes(torch_cuda, blip, tio2):
         assert blip.blipgpu_last_path(table.handle) == 5
     finally:
         blip.blipgpu_set_tuning(table.handle, path=0)
+
+
+def test_first_dense_call_inside_a_capture_runs_the_fp32_kernel(torch_cuda, blip):
+    """The fp16 copy of the table is built on the first dense call; a stream capture cannot allocate,
+    so a dense call captured before that (and without blipgpu_reserve) is served by the FP32-pipe
+    staged kernel — correct results either way — and later eager calls build the copy and switch."""
+    torch = torch_cuda
+    grid, L = (12, 8, 8), 256
+    A, c, pos = workloads.small_case(grid, L, 6000, ORTHO, seed=16)
+    t = blip.BlipTable(A, grid, L, c)
+    dpos = torch.from_numpy(pos).cuda()
+    M, ld = pos.shape[0], t.ld
+    val = torch.empty((M, ld), dtype=torch.float32, device="cuda"); grad = torch.empty((M, 3, ld), dtype=torch.float32, device="cuda")
+    lap = torch.empty((M, ld), dtype=torch.float32, device="cuda")
+    cell = torch.empty((M, 3), dtype=torch.int32, device="cuda")
+    s = torch.cuda.Stream()
+    with torch.cuda.stream(s):
+        # the grouping workspace (an allocation too) is sized ahead of the capture by a call forced to
+        # the grouped direct kernel, which does not build the table copy
+        blip.blipgpu_set_tuning(t.handle, path=1)
+        blip.blipgpu_eval(t.handle, dpos, M, blip.VGL, val, grad, lap, ld, stream=s)
+        blip.blipgpu_set_tuning(t.handle, path=0)
+        s.synchronize()
+        g = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(g, stream=s):
+            blip.blipgpu_eval(t.handle, dpos, M, blip.VGL, val, grad, lap, ld, cell, stream=s)
+        captured_path = blip.blipgpu_last_path(t.handle)
+        g.replay()
+        s.synchronize()
+    assert captured_path == 2
+    compare(A, grid, c, pos, (val.cpu().numpy()[:, :L], grad.cpu().numpy()[:, :, :L], lap.cpu().numpy()[:, :L], cell.cpu().numpy()))
+    out = run_gpu(torch_cuda, blip, A, grid, c, pos, table=t)
+    assert blip.blipgpu_last_path(t.handle) == 5
+    compare(A, grid, c, pos, out)
+    t.close()
