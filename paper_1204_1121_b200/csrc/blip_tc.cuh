@@ -101,7 +101,8 @@ __device__ __forceinline__ bool tc_elect_one()
 }
 constexpr unsigned kTcWaitHintNs = 100;
 // wait of a role that runs ahead of / behind the issuers: the hardware may park the warp for up to
-// ~1 us per poll instead of spinning in the issue slots the other roles need
+// 100 ns per poll instead of spinning in the issue slots the other roles need (1 us and sleeping
+// waits were slower: the wake-up latency costs more than the polls, profiles/r2_v2.md)
 __device__ __forceinline__ void mbar_wait_relaxed(unsigned bar, unsigned parity)
 {
     asm volatile(
@@ -164,8 +165,8 @@ __device__ __forceinline__ void tma_prefetch_5d(const CUtensorMap* tmap, int c0,
 }
 
 // The table of the tensor-core path (library-owned, built from the padded fp32 table when the handle
-// first takes this path, or by blipgpu_reserve): the ghost-padded table with every coefficient scaled by 2^kc and split in its two fp16
-// halves, z sites in pairs, 32-bit words
+// first takes this path, or by blipgpu_reserve): the ghost-padded table with every coefficient
+// scaled by 2^kc and split in its two fp16 halves, z sites in pairs, 32-bit words
 //     T16[p1][p2][zp][half][l] = { c_half[p1][p2][2 zp][l], c_half[p1][p2][2 zp + 1][l] << 16 }
 // — exactly the word a TMEM column of the A operand holds, so that the converter warps only move
 // words from the staged plane to tensor memory.  Same bytes per coefficient as fp32.
