@@ -216,12 +216,13 @@ __device__ __forceinline__ void tc_store_vec(unsigned char* tile, int n, const f
     *reinterpret_cast<uint4*>(tile + n * 16) = tc_place<Z0>(a1[0], a1[1]);
     *reinterpret_cast<uint4*>(tile + (n2 >> 3) * 256 + (n2 & 7) * 16) = tc_place<Z0>(a2[0], a2[1]);
 }
-template <int Z0>
+template <int Z0, int MODE>
 __device__ __forceinline__ void tc_build_tile(const float4* rec4, const float* recf, const float (&wz)[3][4], const TcScale& scl,
                                               unsigned char* bt, int lane)
 {
     const int colm = lane >> 1;
     const bool hb = lane & 1;
+    if (MODE == 0 && hb) return;                             // value only: rows 1..4 and 6..9 of the tiles stay zero for the whole launch
     const float4 cw = rec4[colm];
     const int m1 = colm >> 2, m2 = colm & 3;
     unsigned char* const tile = bt + (m1 * 2 + (m2 >> 1)) * 512 + (m2 & 1) * 128;
@@ -232,6 +233,7 @@ __device__ __forceinline__ void tc_build_tile(const float4* rec4, const float* r
         for (int m = 0; m < 4; ++m) w[m] = __fmul_rn(f, hb ? wz[1][m] : wz[0][m]);
         tc_store_vec<Z0>(tile, hb ? 3 : 0, w);
     }
+    if (MODE == 0) return;
     if (hb) {   // lap
         const float lb = recf[64 + colm];
         const float fa = __fmul_rn(cw.w, scl.sw[4]), fb = __fmul_rn(lb, scl.sw[4]), fc = __fmul_rn(cw.x, scl.sw[4]);
@@ -413,7 +415,9 @@ eval_tc_kernel(const __grid_constant__ CUtensorMap tmap, Geom g, StagedGeom sg, 
                 asm volatile("tcgen05.ld.sync.aligned.32x32b.x8.b32 {%0, %1, %2, %3, %4, %5, %6, %7}, [%8];"
                              : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7])
                              : "r"(tl + d * 16) : "memory");
-                asm volatile("tcgen05.ld.sync.aligned.32x32b.x2.b32 {%0, %1}, [%2];" : "=r"(r[8]), "=r"(r[9]) : "r"(tl + d * 16 + 8) : "memory");
+                if (MODE != 0)
+                    asm volatile("tcgen05.ld.sync.aligned.32x32b.x2.b32 {%0, %1}, [%2];" : "=r"(r[8]), "=r"(r[9]) : "r"(tl + d * 16 + 8) : "memory");
+                else r[8] = r[9] = 0u;
                 asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
                 tc_fence_before();
                 __syncwarp();
@@ -422,7 +426,8 @@ eval_tc_kernel(const __grid_constant__ CUtensorMap tmap, Geom g, StagedGeom sg, 
                 BLIP_ASSERT(e >= 0 && (long long)e < g.M);
                 float q[5];
 #pragma unroll
-                for (int k = 0; k < 5; ++k) q[k] = __fmul_rn(__fadd_rn(__uint_as_float(r[k]), __uint_as_float(r[k + 5])), scl.inv[k]);
+                for (int k = 0; k < 5; ++k)
+                    q[k] = (MODE != 0 || k == 0) ? __fmul_rn(__fadd_rn(__uint_as_float(r[k]), __uint_as_float(r[k + 5])), scl.inv[k]) : 0.f;
                 if (inf.x < 0) {                             // non-finite position (R17): the same for the whole warp
                     q[0] = q[1] = q[2] = q[3] = q[4] = __int_as_float(0x7fc00000);
                 }
@@ -481,10 +486,10 @@ eval_tc_kernel(const __grid_constant__ CUtensorMap tmap, Geom g, StagedGeom sg, 
                 unsigned char* const bt = sm.bt[b];
                 {
                     switch (z0) {                              // the same for the whole warp: placement of the 4 fp16 at compile time
-                        case 0: tc_build_tile<0>(rec4, recf, wz, scl, bt, lane); break;
-                        case 1: tc_build_tile<1>(rec4, recf, wz, scl, bt, lane); break;
-                        case 2: tc_build_tile<2>(rec4, recf, wz, scl, bt, lane); break;
-                        default: tc_build_tile<3>(rec4, recf, wz, scl, bt, lane); break;
+                        case 0: tc_build_tile<0, MODE>(rec4, recf, wz, scl, bt, lane); break;
+                        case 1: tc_build_tile<1, MODE>(rec4, recf, wz, scl, bt, lane); break;
+                        case 2: tc_build_tile<2, MODE>(rec4, recf, wz, scl, bt, lane); break;
+                        default: tc_build_tile<3, MODE>(rec4, recf, wz, scl, bt, lane); break;
                     }
                 }
                 if (lane == 0) sm.info[uc % kTcNInfo] = make_int4(loc.x >= 0 ? (int)(it_seq0 + (unsigned)loc.x) : -1, y0, loc.w, 0);
