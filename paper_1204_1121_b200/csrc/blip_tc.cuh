@@ -363,30 +363,32 @@ eval_tc_kernel(const __grid_constant__ CUtensorMap tmap, Geom g, StagedGeom sg, 
                 // 64 registers a thread of this 928-thread CTA has)
                 const unsigned* src = &sm.plane[s][orb];
                 const unsigned tcol = tlane + t * kTcPlaneCols;
-                auto ld_rows = [&](unsigned (&h)[4][8], int y0, int ny) {
+                // word (y, z pair k, half) of this orbital; a half's 28 words are 28 consecutive TMEM columns
+                auto word = [&](int y, int k, int half) { return src[((y * 4 + k) * 2 + half) * 128]; };
+                unsigned a1[16], a2[16];                     // rows 0..3, halves 1 and 2
 #pragma unroll
-                    for (int y = 0; y < 4; ++y)
-                        if (y < ny)
-#pragma unroll
-                            for (int k = 0; k < 4; ++k) {
-                                h[y][k] = src[(((y0 + y) * 4 + k) * 2) * 128]; h[y][4 + k] = src[(((y0 + y) * 4 + k) * 2 + 1) * 128];
-                            }
-                };
-                auto st_rows = [&](const unsigned (&h)[4][8], int y0, int ny) {
-#pragma unroll
-                    for (int y = 0; y < 4; ++y)
-                        if (y < ny) {
-                            asm volatile("tcgen05.st.sync.aligned.32x32b.x4.b32 [%0], {%1, %2, %3, %4};"
-                                         :: "r"(tcol + 4 * (y0 + y)), "r"(h[y][0]), "r"(h[y][1]), "r"(h[y][2]), "r"(h[y][3]) : "memory");
-                            asm volatile("tcgen05.st.sync.aligned.32x32b.x4.b32 [%0], {%1, %2, %3, %4};"
-                                         :: "r"(tcol + 28 + 4 * (y0 + y)), "r"(h[y][4]), "r"(h[y][5]), "r"(h[y][6]), "r"(h[y][7]) : "memory");
-                        }
-                };
-                unsigned ha[4][8], hb[4][8];
-                ld_rows(ha, 0, 4);
+                for (int i = 0; i < 16; ++i) { a1[i] = word(i >> 2, i & 3, 0); a2[i] = word(i >> 2, i & 3, 1); }
                 if (q >= kTcRT) mbar_wait_relaxed(smem_u32(&sm.tempty[t]), ((q / kTcRT) & 1u) ^ 1u);
                 tc_fence_after();
-                st_rows(ha, 0, 4); ld_rows(hb, 4, 3); st_rows(hb, 4, 3);
+#define BLIP_TC_ST16(col, v)                                                                                          \
+                asm volatile("tcgen05.st.sync.aligned.32x32b.x16.b32 [%0], {%1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, %16};" \
+                             :: "r"(col), "r"(v[0]), "r"(v[1]), "r"(v[2]), "r"(v[3]), "r"(v[4]), "r"(v[5]), "r"(v[6]), "r"(v[7]), "r"(v[8]),   \
+                                "r"(v[9]), "r"(v[10]), "r"(v[11]), "r"(v[12]), "r"(v[13]), "r"(v[14]), "r"(v[15]) : "memory")
+                BLIP_TC_ST16(tcol, a1);
+                BLIP_TC_ST16(tcol + 28, a2);
+#undef BLIP_TC_ST16
+                unsigned b1[12], b2[12];                     // rows 4..6
+#pragma unroll
+                for (int i = 0; i < 12; ++i) { b1[i] = word(4 + (i >> 2), i & 3, 0); b2[i] = word(4 + (i >> 2), i & 3, 1); }
+#define BLIP_TC_ST8(col, v, o)                                                                                         \
+                asm volatile("tcgen05.st.sync.aligned.32x32b.x8.b32 [%0], {%1, %2, %3, %4, %5, %6, %7, %8};"              \
+                             :: "r"(col), "r"(v[o]), "r"(v[o + 1]), "r"(v[o + 2]), "r"(v[o + 3]), "r"(v[o + 4]), "r"(v[o + 5]), "r"(v[o + 6]), "r"(v[o + 7]) : "memory")
+#define BLIP_TC_ST4(col, v, o)                                                                                         \
+                asm volatile("tcgen05.st.sync.aligned.32x32b.x4.b32 [%0], {%1, %2, %3, %4};" :: "r"(col), "r"(v[o]), "r"(v[o + 1]), "r"(v[o + 2]), "r"(v[o + 3]) : "memory")
+                BLIP_TC_ST8(tcol + 16, b1, 0); BLIP_TC_ST4(tcol + 24, b1, 8);
+                BLIP_TC_ST8(tcol + 28 + 16, b2, 0); BLIP_TC_ST4(tcol + 28 + 24, b2, 8);
+#undef BLIP_TC_ST8
+#undef BLIP_TC_ST4
                 asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
                 tc_fence_before();
                 __syncwarp();
