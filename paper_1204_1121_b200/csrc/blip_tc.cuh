@@ -262,6 +262,7 @@ eval_tc_kernel(const __grid_constant__ CUtensorMap tmap, Geom g, StagedGeom sg, 
     constexpr unsigned IQ = kItemQueue;
     constexpr int PLANE_BYTES = kTcPlaneWords * 4;
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const bool idx32 = (unsigned long long)g.M * 3ull * (unsigned long long)ld < (1ull << 32);
     wait_for_predecessor();
     if (warp == 0) {
         asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], 512;" :: "r"(smem_u32(&sm.tbase)) : "memory");
@@ -408,6 +409,7 @@ eval_tc_kernel(const __grid_constant__ CUtensorMap tmap, Geom g, StagedGeom sg, 
             float* const vcol = val + col;
             float* const gcol = grad + col;
             float* const lcol = lap + col;
+            const bool col_ok = col < 4 * g.pitch4;
             for (unsigned u = (ubase + (unsigned)eg) & 1u; u < it_nunits; u += 2) {      // (ubase + u) % 2 == eg
                 const unsigned uc = ubase + u, d = uc % kTcND;
                 mbar_wait_relaxed(smem_u32(&sm.dfull[d]), (uc / kTcND) & 1u);
@@ -430,20 +432,33 @@ eval_tc_kernel(const __grid_constant__ CUtensorMap tmap, Geom g, StagedGeom sg, 
 #pragma unroll
                 for (int k = 0; k < 5; ++k)
                     q[k] = (MODE != 0 || k == 0) ? __fmul_rn(__fadd_rn(__uint_as_float(r[k]), __uint_as_float(r[k + 5])), scl.inv[k]) : 0.f;
-                if (inf.x < 0) {                             // non-finite position (R17): the same for the whole warp
-                    q[0] = q[1] = q[2] = q[3] = q[4] = __int_as_float(0x7fc00000);
+                if (inf.x < 0)                               // non-finite position (R17): the same for the whole warp, and rare
+                    asm volatile("mov.b32 %0, 0x7fc00000; mov.b32 %1, 0x7fc00000; mov.b32 %2, 0x7fc00000; mov.b32 %3, 0x7fc00000; mov.b32 %4, 0x7fc00000;"
+                                 : "=f"(q[0]), "=f"(q[1]), "=f"(q[2]), "=f"(q[3]), "=f"(q[4]));
+                if (!col_ok) continue;
+                float gx = q[1], gy = q[2], gz = q[3];
+                if (MODE == 1) {
+                    gx = __fmaf_rn(g.J[0], q[1], __fmaf_rn(g.J[3], q[2], __fmul_rn(g.J[6], q[3])));
+                    gy = __fmaf_rn(g.J[1], q[1], __fmaf_rn(g.J[4], q[2], __fmul_rn(g.J[7], q[3])));
+                    gz = __fmaf_rn(g.J[2], q[1], __fmaf_rn(g.J[5], q[2], __fmul_rn(g.J[8], q[3])));
                 }
-                if (col < 4 * g.pitch4) {
+                BLIP_ASSERT((long long)col < ld);
+                if (idx32) {
+                    // all element offsets of this call fit in 32 bits (the host checked M x 3 ld): one
+                    // multiply-add per array instead of 64-bit pointer arithmetic
+                    const unsigned o = (unsigned)e * (unsigned)ld + (unsigned)col;
+                    __stcs(val + o, q[0]);
+                    if (MODE != 0) {
+                        const unsigned og = 3u * (unsigned)e * (unsigned)ld + (unsigned)col;
+                        __stcs(grad + og, gx);
+                        __stcs(grad + (og + (unsigned)ld), gy);
+                        __stcs(grad + (og + 2u * (unsigned)ld), gz);
+                        __stcs(lap + o, q[4]);
+                    }
+                } else {
                     const size_t o = (size_t)(unsigned)e * (size_t)(unsigned)ld;
-                    BLIP_ASSERT((long long)col < ld);
                     __stcs(vcol + o, q[0]);
                     if (MODE != 0) {
-                        float gx = q[1], gy = q[2], gz = q[3];
-                        if (MODE == 1) {
-                            gx = __fmaf_rn(g.J[0], q[1], __fmaf_rn(g.J[3], q[2], __fmul_rn(g.J[6], q[3])));
-                            gy = __fmaf_rn(g.J[1], q[1], __fmaf_rn(g.J[4], q[2], __fmul_rn(g.J[7], q[3])));
-                            gz = __fmaf_rn(g.J[2], q[1], __fmaf_rn(g.J[5], q[2], __fmul_rn(g.J[8], q[3])));
-                        }
                         float* const gp = gcol + 3 * o;
                         __stcs(gp, gx);
                         __stcs(gp + ld, gy);
