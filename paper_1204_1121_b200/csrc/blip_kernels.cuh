@@ -342,7 +342,7 @@ struct StagedRec {
     float  lb[16];
     float  wz[3][4];
     int4   loc;         // {i1 - first plane of the pencil segment (-1: non-finite position),
-                        //  byte offset of row (i2, i3) in a staged plane, unused, electron id}
+                        //  byte offset of row (i2, i3) in a staged plane, (i2 % BY) << 8 | (i3 % BZ), electron id}
 };
 static_assert(sizeof(StagedRec) == sizeof(ElecRec), "one record layout");
 
@@ -435,12 +435,14 @@ __device__ __forceinline__ void write_staged_record(const Geom& g, const StagedG
                           __fmul_rn(g.Q[2], ax[2][2][2]), __fmul_rn(g.Q[2], ax[2][2][3]));
     // StagedRec::loc: plane within the pencil segment, byte offset of row (i2, i3) in a plane of
     // (by+3) x (bz+3) rows of tile_floats floats
-    int pl = -1, off = 0;
+    int pl = -1, off = 0, yz = 0;
     if (ic[0] >= 0) {
         pl = ic[0] % sg.seg;
-        off = ((ic[1] % sg.by) * (sg.bz + 3) + (ic[2] % sg.bz)) * tile_floats * 4;
+        const int y0 = ic[1] % sg.by, z0 = ic[2] % sg.bz;
+        off = (y0 * (sg.bz + 3) + z0) * tile_floats * 4;
+        yz = (y0 << 8) | z0;                                 // the cell's offset in its pencil, for the tensor-core kernel
     }
-    out[23] = make_float4(__int_as_float(pl), __int_as_float(off), 0.f, __int_as_float(e));
+    out[23] = make_float4(__int_as_float(pl), __int_as_float(off), __int_as_float(yz), __int_as_float(e));
 }
 
 // a-4 (3/3) for the staged path, three-kernel form: one thread per electron takes its slot in

@@ -490,8 +490,7 @@ eval_tc_kernel(const __grid_constant__ CUtensorMap tmap, Geom g, StagedGeom sg, 
                 __syncwarp();
                 if (u + kTcNW < it_nunits && lane < kRecFloats / 4) pre = __ldg(rsrc + (size_t)(u + kTcNW) * (kRecFloats / 4) + lane);
                 const int4 loc = *reinterpret_cast<const int4*>(rec4 + 23);       // {plane in item or -1, byte offset of row (i2, i3), -, electron}
-                const int rowi = loc.y / (128 * 4);                               // y0 * 7 + z0
-                const int y0 = rowi / 7, z0 = rowi - 7 * y0;
+                const int y0 = loc.z >> 8, z0 = loc.z & 255;                      // the cell's offset in its 4 x 4 pencil
                 BLIP_ASSERT((long long)it_u0 + u < g.M && loc.w >= 0 && (long long)loc.w < g.M);       // record and electron within the batch
                 BLIP_ASSERT(loc.x < it_nplanes - 3 && loc.y >= 0 && y0 < 4 && z0 < 4);                  // block of sites inside the item's planes / pencil
                 float wz[3][4];
