@@ -287,3 +287,31 @@ def test_first_dense_call_inside_a_capture_runs_the_fp32_kernel(torch_cuda, blip
     assert blip.blipgpu_last_path(t.handle) == 5
     compare(A, grid, c, pos, out)
     t.close()
+
+
+def test_outputs_beyond_32_bit_element_offsets(torch_cuda, blip):
+    """700,000 positions x 2,048 orbitals: the gradient array has 4.3e9 elements, so the epilogue takes
+    its 64-bit addressing (smaller calls use 32-bit element offsets).  2,000 sampled positions, spread
+    over the whole batch, against the oracle."""
+    torch = torch_cuda
+    grid, L, M = (8, 8, 8), 2048, 700000
+    A, c, _ = workloads.small_case(grid, L, 1, ORTHO, seed=21)
+    rng = np.random.default_rng(22)
+    pos = rng.random((M, 3)) @ np.asarray(A).reshape(3, 3)
+    t = tc_table(blip, A, grid, c)
+    dpos = torch.from_numpy(pos).cuda()
+    ld = t.ld
+    assert 3 * M * ld >= 2 ** 32
+    val = torch.empty((M, ld), dtype=torch.float32, device="cuda")
+    grad = torch.empty((M, 3, ld), dtype=torch.float32, device="cuda")
+    lap = torch.empty((M, ld), dtype=torch.float32, device="cuda")
+    blip.blipgpu_eval(t.handle, dpos, M, blip.VGL, val, grad, lap, ld)
+    torch.cuda.synchronize()
+    assert blip.blipgpu_last_path(t.handle) == 5
+    pick = np.sort(rng.choice(M, size=2000, replace=False))
+    pick[-1] = M - 1
+    ip = torch.from_numpy(pick).cuda()
+    gpu = (val[ip].cpu().numpy(), grad[ip].cpu().numpy(), lap[ip].cpu().numpy(), None)
+    del val, grad, lap
+    compare(A, grid, c, pos[pick], gpu)
+    t.close()
