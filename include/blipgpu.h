@@ -205,6 +205,55 @@ int blipgpu_eval_complex(blipgpu_table* t, const double* positions, long long M,
  * are sized by that call itself.  Errors: EINVAL, ENOMEM, ECUDA. */
 int blipgpu_reserve(blipgpu_table* t, long long M_max);
 
+/*
+ * blipgpu_eval_static — blipgpu_eval for callers that must not allocate device memory while they
+ * sample.  Two kinds of caller are meant.  A QMC code that, once its walkers are set up, hands
+ * all remaining device memory to an arena of its own: a cudaMalloc issued by a library after that
+ * point fails.  And a code that runs other walkers on other streams of the same GPU: cudaMalloc
+ * and cudaFree stall the whole device until those streams drain, which such a code cannot afford
+ * inside its sampling loop.  blipgpu_eval grows its grouping workspace with cudaMalloc when a
+ * batch is larger than any before it (and builds the tensor-core copy of the table on the first
+ * dense batch); this call never does.  It calls no cudaMalloc, cudaFree or other allocating
+ * routine, whatever the batch.
+ *
+ * What it runs: steps a-1..a-5 as the grouped direct-gather path of blipgpu_eval — positions are
+ * counted into bricks of 4x4x4 cells, a prefix sum turns the counts into slots, the positions are
+ * scattered into brick order, and one warp per position gathers the 64 coefficient rows
+ * (blip::bin_kernel, scan_kernel, scatter_kernel, eval_direct_kernel).  The four arrays those
+ * kernels need between them (brick of each position, count and slot per brick, sorted order) do
+ * not come from the handle's workspace but from ONE fixed array that is part of the library
+ * image: BLIPGPU_STATIC_BYTES (768 KiB) of device memory on every GPU that loads the library,
+ * held until the process exits, used or not.  The table is still the handle's: create the handle
+ * with blipgpu_create during set-up, while allocating is still allowed.
+ *
+ *   arguments, output layout, alignment rules and non-finite positions: as blipgpu_eval;
+ *   mode            BLIPGPU_VALUE or BLIPGPU_VGL (VGH uses no workspace: call blipgpu_eval)
+ *   M               <= BLIPGPU_STATIC_MAX_POSITIONS, else BLIPGPU_ELIMIT
+ *   the table       at most BLIPGPU_STATIC_MAX_BRICKS bricks, ceil(n1/4) ceil(n2/4) ceil(n3/4)
+ *                   (every config of BASELINE.json fits; a 128^3 grid is the limit), else ELIMIT
+ *
+ * Results: the bits blipgpu_eval returns when it runs the direct-gather kernel (fp32 FMAs); a
+ * dense batch, which blipgpu_eval gives to its tensor-core kernel, differs from that in the last
+ * bits, both within the tolerances of the fp64 definition.
+ *
+ * Rules that come with the fixed array.
+ *  - Every call on a device uses the same array, whatever the handle and the stream.  Calls that
+ *    may overlap on the GPU (two streams, two host threads) race on it and return garbage: order
+ *    them yourself (one stream, or events).  Calls on different GPUs are independent.
+ *  - The array keeps what the previous call left in it.  The call clears the brick counts it is
+ *    about to use (a memset on `stream`) before it counts; nothing else needs a clean start.
+ *  - The first call on each device looks up the device address of the array (the handle's device
+ *    must be current, as for every call).  That look-up is a set-up step: make the first call on
+ *    a device before you begin any stream capture.  Later calls on that device only launch.
+ * Errors: EINVAL (as blipgpu_eval; mode VGH), ELIMIT, ECUDA.
+ */
+#define BLIPGPU_ELIMIT  (-5)                      /* larger than blipgpu_eval_static's fixed array allows */
+#define BLIPGPU_STATIC_MAX_POSITIONS 65536
+#define BLIPGPU_STATIC_MAX_BRICKS    32768
+#define BLIPGPU_STATIC_BYTES (8 * BLIPGPU_STATIC_MAX_POSITIONS + 8 * BLIPGPU_STATIC_MAX_BRICKS)
+int blipgpu_eval_static(blipgpu_table* t, const double* positions, long long M, int mode,
+                        float* val, float* grad, float* lap, long long ld, int* cell, void* stream);
+
 /* blipgpu_destroy — free the table and workspace.  destroy(NULL) is a no-op returning OK. */
 int blipgpu_destroy(blipgpu_table* t);
 

@@ -14,7 +14,8 @@ import numpy as np
 from . import _build
 
 VALUE, VGL, VGH = 0, 1, 2
-OK, EINVAL, ENOMEM, ECUDA, EARCH = 0, -1, -2, -3, -4
+OK, EINVAL, ENOMEM, ECUDA, EARCH, ELIMIT = 0, -1, -2, -3, -4, -5
+STATIC_MAX_POSITIONS, STATIC_MAX_BRICKS = 65536, 32768     # blipgpu_eval_static: BLIPGPU_STATIC_MAX_* of blipgpu.h
 
 _lib = None
 _c_dp = ctypes.POINTER(ctypes.c_double)
@@ -42,6 +43,9 @@ SIGNATURES = {
     "blipgpu_eval_complex": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_void_p, ctypes.c_longlong, ctypes.c_int,
                                             ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p,
                                             ctypes.c_longlong, ctypes.c_void_p, ctypes.c_void_p]),
+    "blipgpu_eval_static": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_void_p, ctypes.c_longlong, ctypes.c_int,
+                                           ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p,
+                                           ctypes.c_longlong, ctypes.c_void_p, ctypes.c_void_p]),
     "blipgpu_reserve": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_longlong]),
     "blipgpu_destroy": (ctypes.c_int, [ctypes.c_void_p]),
     "blipgpu_info": (ctypes.c_int, [ctypes.c_void_p, _c_ip, _c_ip, _c_llp, _c_llp]),
@@ -160,6 +164,17 @@ def blipgpu_eval_complex(handle, positions, M, mode, val, grad, lap, ld, cell=No
     rc = lib().blipgpu_eval_complex(handle, _ptr(positions), int(M), int(mode), _ptr(val), _ptr(grad), _ptr(lap),
                                     int(ld), _ptr(cell), _stream_ptr(stream))
     _check(rc, "blipgpu_eval_complex", handle)
+
+
+def blipgpu_eval_static(handle, positions, M, mode, val, grad, lap, ld, cell=None, stream=None):
+    """blipgpu_eval for callers that may not allocate device memory while sampling (their own arena owns
+    the GPU's memory, or cudaMalloc's device-wide stall would hit walkers on other streams): the grouping
+    workspace is a fixed 768 KiB array inside the library instead of a cudaMalloc'ed one.  At most
+    STATIC_MAX_POSITIONS positions and STATIC_MAX_BRICKS 4x4x4-cell bricks (else ELIMIT); calls on one GPU
+    share that array, so they must not overlap; make the first call on a device before any stream capture."""
+    rc = lib().blipgpu_eval_static(handle, _ptr(positions), int(M), int(mode), _ptr(val), _ptr(grad), _ptr(lap),
+                                   int(ld), _ptr(cell), _stream_ptr(stream))
+    _check(rc, "blipgpu_eval_static", handle)
 
 
 def blipgpu_reserve(handle, M_max):

@@ -11,6 +11,7 @@
 #include <cmath>
 #include <cstdlib>
 #include <cstring>
+#include <mutex>
 #include <new>
 
 namespace {
@@ -762,6 +763,7 @@ extern "C" const char* blipgpu_strerror(int code)
         case BLIPGPU_ENOMEM: return "out of memory";
         case BLIPGPU_ECUDA: return "CUDA runtime error (see blipgpu_last_cuda_error)";
         case BLIPGPU_EARCH: return "device is not compute capability 10.x (sm_100a code only, no fallback)";
+        case BLIPGPU_ELIMIT: return "batch or table too large for blipgpu_eval_static's fixed workspace (BLIPGPU_STATIC_MAX_POSITIONS / _BRICKS)";
         default: return "unknown blipgpu error code";
     }
 }
@@ -769,4 +771,110 @@ extern "C" const char* blipgpu_strerror(int code)
 extern "C" int blipgpu_last_cuda_error(const blipgpu_table* t)
 {
     return t ? t->last_cuda : g_create_cuda_error;
+}
+
+// ------------------------------------------------------------------------------------------------
+// blipgpu_eval_static — the grouped direct-gather path of blipgpu_eval for callers that must not
+// allocate device memory once they are sampling (a host code that has given the rest of the GPU
+// to its own arena, or that cannot take the device-wide stall of cudaMalloc / cudaFree while its
+// other streams run walkers; include/blipgpu.h has the full contract).  The same four kernels as
+// launch_eval's three-launch grouping + eval_direct_kernel; what differs is where their workspace
+// lives: not in the handle (cudaMalloc, grown on demand) but in the array below, which is part of
+// the library image, so this entry point calls no cudaMalloc, cudaFree or allocating routine.
+//
+//   g_static_scratch   [hist: MAX_BRICKS u32][offs: MAX_BRICKS u32][bin: MAX_POSITIONS i32][perm: MAX_POSITIONS i32]
+//                      = BLIPGPU_STATIC_BYTES (768 KiB) on every GPU that loads the library, until exit.
+//
+// In host code the NAME g_static_scratch is only the host-side stand-in the runtime registers the
+// array under, not a device address — a kernel handed `g_static_scratch` itself would fault, or on
+// a system where the GPU can reach host memory quietly use the wrong bytes.  The device address
+// comes from cudaGetSymbolAddress, asked once per device with that device current and kept in
+// g_static_ptr[device ordinal]; that look-up is the set-up step the header tells callers to get
+// done (first call) before any stream capture.  All calls on a device share the array: the brick
+// counts are cleared at the start of each call (the rest is fully rewritten before it is read),
+// and calls that overlap on the GPU race — documented, not detected.
+// ------------------------------------------------------------------------------------------------
+static __device__ __align__(256) unsigned char g_static_scratch[BLIPGPU_STATIC_BYTES];
+
+namespace {
+constexpr int kStaticMaxDevices = 64;
+constexpr size_t kStaticOffs = sizeof(unsigned) * BLIPGPU_STATIC_MAX_BRICKS;           // byte offsets into the array,
+constexpr size_t kStaticBin = 2 * sizeof(unsigned) * BLIPGPU_STATIC_MAX_BRICKS;       // each a multiple of 256
+constexpr size_t kStaticPerm = kStaticBin + sizeof(int) * BLIPGPU_STATIC_MAX_POSITIONS;
+static_assert(kStaticPerm + sizeof(int) * BLIPGPU_STATIC_MAX_POSITIONS == BLIPGPU_STATIC_BYTES, "layout fills the array");
+static_assert(kStaticOffs % 256 == 0 && kStaticBin % 256 == 0 && kStaticPerm % 256 == 0, "sub-arrays stay 256-byte aligned");
+
+std::mutex g_static_mu;
+unsigned char* g_static_ptr[kStaticMaxDevices];          // device address of g_static_scratch on device d; NULL: not asked yet
+
+// Device address of the array on the CURRENT device (asked from the runtime the first time).
+cudaError_t static_scratch_address(unsigned char** out)
+{
+    int dev = -1;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return e;
+    if (dev < 0 || dev >= kStaticMaxDevices) return cudaErrorInvalidDevice;
+    std::lock_guard<std::mutex> lock(g_static_mu);
+    if (!g_static_ptr[dev]) {
+        void* p = nullptr;
+        e = cudaGetSymbolAddress(&p, g_static_scratch);
+        if (e != cudaSuccess) return e;
+        if (!p) return cudaErrorInvalidSymbol;
+        g_static_ptr[dev] = static_cast<unsigned char*>(p);
+    }
+    *out = g_static_ptr[dev];
+    return cudaSuccess;
+}
+}  // namespace
+
+extern "C" int blipgpu_eval_static(blipgpu_table* t, const double* positions, long long M, int mode,
+                                   float* val, float* grad, float* lap, long long ld, int* cell, void* stream)
+{
+    if (mode != BLIPGPU_VALUE && mode != BLIPGPU_VGL) return BLIPGPU_EINVAL;
+    int rc = check_eval_args(t, positions, M, mode, val, grad, lap, ld);
+    if (rc != BLIPGPU_OK || M == 0) return rc;
+    if (((uintptr_t)val & 15) || (mode == BLIPGPU_VGL && (((uintptr_t)grad & 15) || ((uintptr_t)lap & 15))))
+        return BLIPGPU_EINVAL;
+    const int nbins = t->nbins_direct;
+    if (M > BLIPGPU_STATIC_MAX_POSITIONS || nbins > BLIPGPU_STATIC_MAX_BRICKS) return BLIPGPU_ELIMIT;
+
+    cudaStream_t s = (cudaStream_t)stream;
+    unsigned char* base = nullptr;
+    CK(t, static_scratch_address(&base));
+    unsigned* hist = reinterpret_cast<unsigned*>(base);
+    unsigned* offs = reinterpret_cast<unsigned*>(base + kStaticOffs);
+    int* bin = reinterpret_cast<int*>(base + kStaticBin);
+    int* perm = reinterpret_cast<int*>(base + kStaticPerm);
+
+    blip::Geom g = t->g;                                     // the handle's copy is left alone
+    g.M = M;
+    // a-4: the counts must start at zero and the array holds whatever the last call (any handle, any
+    // stream) left: clear the bins of THIS table.  bin / offs / perm are written before they are read.
+    CK(t, cudaMemsetAsync(hist, 0, sizeof(unsigned) * (size_t)nbins, s));
+    const unsigned nb = (unsigned)((M + 255) / 256);
+    blip::bin_kernel<<<nb, 256, 0, s>>>(g, t->sg, 0, positions, M, bin, hist, cell);
+    blip::scan_kernel<<<1, blip::kScanThreads, 0, s>>>(hist, offs, nbins, M, 0, g, t->sg, nullptr, nullptr);
+    blip::scatter_kernel<<<nb, 256, 0, s>>>(bin, offs, M, perm);
+    CK(t, cudaGetLastError());
+    // a-1..a-3, a-5: one warp per position in brick order, results to the caller's order (cell: done above)
+    const int kmode = mode == BLIPGPU_VALUE ? 0 : (t->diag ? 2 : 1);
+    const int nq = t->nq;
+    const dim3 grid((unsigned)((M + blip::kWarpsPerBlock - 1) / blip::kWarpsPerBlock),
+                    (unsigned)((t->g.pitch4 + 32 * nq - 1) / (32 * nq)));
+    const dim3 block(blip::kWarpsPerBlock * 32);
+#define BLIP_LAUNCH(MODE, NQ)                                                                         \
+    blip::eval_direct_kernel<MODE, NQ><<<grid, block, 0, s>>>(g, t->table, positions, perm, M, val, grad, lap, ld, \
+                                                              nullptr, 0, nullptr, nullptr, nullptr)
+    if (kmode == 0) {
+        if (nq == 1) BLIP_LAUNCH(0, 1); else if (nq == 2) BLIP_LAUNCH(0, 2); else BLIP_LAUNCH(0, 3);
+    } else if (kmode == 2) {
+        if (nq == 1) BLIP_LAUNCH(2, 1); else if (nq == 2) BLIP_LAUNCH(2, 2); else BLIP_LAUNCH(2, 3);
+    } else {
+        if (nq == 1) BLIP_LAUNCH(1, 1); else if (nq == 2) BLIP_LAUNCH(1, 2); else BLIP_LAUNCH(1, 3);
+    }
+#undef BLIP_LAUNCH
+    CK(t, cudaGetLastError());
+    t->launches += 4;
+    t->last_path = 1;
+    return BLIPGPU_OK;
 }
