@@ -436,7 +436,7 @@ __device__ __forceinline__ void write_staged_record(const Geom& g, const StagedG
     // StagedRec::loc: plane within the pencil segment, byte offset of row (i2, i3) in a plane of
     // (by+3) x (bz+3) rows of tile_floats floats
     int pl = -1, off = 0, yz = 0;
-    if (ic[0] >= 0) {
+    if (ic[0] >= 0 && ic[1] >= 0 && ic[2] >= 0) {            // finite on every axis, as bin_of / bin_kernel decide it
         pl = ic[0] % sg.seg;
         const int y0 = ic[1] % sg.by, z0 = ic[2] % sg.bz;
         off = (y0 * (sg.bz + 3) + z0) * tile_floats * 4;

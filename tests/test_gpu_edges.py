@@ -174,6 +174,36 @@ def test_non_finite_positions(torch_cuda, blip):
         compare(A, (6, 6, 6), c, pos[:M][good], (val[good], grad[good], lap[good], cell[good]))
 
 
+@pytest.mark.parametrize("path", [0, 1, 2, 5])
+def test_overflow_on_a_single_axis(torch_cuda, blip, path):
+    """Finite coordinates whose FRACTIONAL coordinate overflows on one axis only (sub-bohr lattice
+    vectors, |r| near 1e308): the position is non-finite for the method — NaN outputs, cell = -1 on
+    all three axes (include/blipgpu.h) — whichever axis it is and whichever kernel runs; its
+    neighbours in the batch are unaffected."""
+    grid, L = (12, 8, 12), 132
+    lat = np.diag([0.5, 0.05, 0.5])
+    A, c, pos = workloads.small_case(grid, L, 3000, lat, seed=13)
+    bad = [3, 1000, 1001, 2999]
+    pos[bad[0]] = (1.7e308, 0.01, 0.2)                       # axis 0 only
+    pos[bad[1]] = (0.3, 1e308, 0.1)                          # axis 1 only
+    pos[bad[2]] = (0.1, 0.02, -1.7e308)                      # axis 2 only
+    pos[bad[3]] = (0.2, -1e307, 1.2e308)                     # axes 1 and 2
+    assert np.isfinite(pos).all()
+    t = blip.BlipTable(A, grid, L, c)
+    blip.blipgpu_set_tuning(t.handle, path=path)
+    val, grad, lap, cell = run_gpu(torch_cuda, blip, A, grid, c, pos, table=t)
+    assert blip.blipgpu_last_path(t.handle) == (path if path else 5)
+    oval, ograd, olap, ocell = oracle.eval_fast(A, grid, c, pos)
+    assert np.array_equal(cell, ocell) and (cell[bad] == -1).all()
+    nanrows = np.isnan(oval).all(axis=1)
+    assert nanrows.sum() == 4 and nanrows[bad].all()
+    assert np.array_equal(np.isnan(val).all(axis=1), nanrows)
+    assert np.isnan(grad[nanrows]).all() and np.isnan(lap[nanrows]).all()
+    good = ~nanrows
+    compare(A, grid, c, pos[good], (val[good], grad[good], lap[good], cell[good]))
+    t.close()
+
+
 def test_adversarial_cell_indices(torch_cuda, blip):
     """exact grid planes, denormal and tiny negative coordinates, +-1e3 cells, 1 ulp either
     side of a plane: GPU cell == oracle cell bit for bit."""
