@@ -255,14 +255,15 @@ template <int MODE>
 __global__ void __launch_bounds__(kTcThreads, 1)
 eval_tc_kernel(const __grid_constant__ CUtensorMap tmap, Geom g, StagedGeom sg, TcScale scl,
                const float4* __restrict__ recs, const int4* __restrict__ order, int* __restrict__ meta,
-               int nchunk, float* __restrict__ val, float* __restrict__ grad, float* __restrict__ lap, long long ld)
+               int nchunk, float* __restrict__ val, float* __restrict__ grad, float* __restrict__ lap, long long ld,
+               int idx32_arg /* every output element offset of this call fits 32 bits (tc_launch derives it from M and ld) */)
 {
     extern __shared__ __align__(128) unsigned char smem_raw[];
     TcSmem& sm = *reinterpret_cast<TcSmem*>(smem_raw);
     constexpr unsigned IQ = kItemQueue;
     constexpr int PLANE_BYTES = kTcPlaneWords * 4;
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    const bool idx32 = (unsigned long long)g.M * 3ull * (unsigned long long)ld < (1ull << 32);
+    const bool idx32 = idx32_arg != 0;
     wait_for_predecessor();
     if (warp == 0) {
         asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], 512;" :: "r"(smem_u32(&sm.tbase)) : "memory");

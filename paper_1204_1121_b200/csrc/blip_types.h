@@ -40,7 +40,7 @@ struct Geom {
     int L;              // orbitals
     int pitch4;         // table row pitch in float4 (= ceil(L/4))
     int diag;           // J diagonal (lattice vectors along the Cartesian axes): the kernels' MODE 2
-    long long M;        // positions of the current call (set per launch; read by the BLIP_CHECKED build only)
+    long long M;        // positions of the current call: set per launch, read only by the asserts of the BLIP_CHECKED build
 };
 
 // Geometry of the staged path: pencils of BY x BZ cells running along axis 1, cut into

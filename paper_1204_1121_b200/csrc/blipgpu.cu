@@ -97,10 +97,13 @@ cudaError_t tc_prepare()
     if (e == cudaSuccess) e = cudaFuncSetAttribute(blip::eval_tc_kernel<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(blip::TcSmem));
     return e;
 }
-cudaError_t tc_launch(int mode, unsigned nctas, cudaStream_t s, const StagedArgs& a, const blip::TcScale& scl)
+cudaError_t tc_launch(int mode, unsigned nctas, cudaStream_t s, const StagedArgs& a, const blip::TcScale& scl, long long M)
 {
+    // the epilogue addresses val / grad / lap with 32-bit element offsets when the largest one of this
+    // call, (M - 1) * 3 * ld + 3 * ld - 1 (the gradient's), fits; decided here, next to the launch
+    const int idx32 = (unsigned long long)M * 3ull * (unsigned long long)a.ld < (1ull << 32) ? 1 : 0;
 #define BLIP_TC(MODE) launch_pdl(blip::eval_tc_kernel<MODE>, nctas, blip::kTcThreads, sizeof(blip::TcSmem), s, *a.tmap, *a.g, *a.sg, scl, \
-                                 a.recs, a.order, a.meta, a.nchunk, a.val, a.grad, a.lap, a.ld)
+                                 a.recs, a.order, a.meta, a.nchunk, a.val, a.grad, a.lap, a.ld, idx32)
     if (mode == 0) return BLIP_TC(0);
     if (mode == 2) return BLIP_TC(2);
     return BLIP_TC(1);
@@ -493,10 +496,10 @@ static int launch_eval(blipgpu_table* t, const double* positions, long long M, i
                        cudaStream_t s, const float* dvec = nullptr, long long ldd = 0, float* cout = nullptr,
                        const double* kvec = nullptr)
 {
+    t->g.M = M;                                              // bound of the checked build's asserts (nothing else reads it)
     if (mode == BLIPGPU_VGH)                                  // full Hessian: the per-position kernel, fp32
         return launch_hess<float>(t, positions, M, val, grad, lap, ld, cell, s);
     const int* perm = nullptr;
-    t->g.M = M;                                              // bound of the checked build's asserts
     const bool tc_call = t->tc_ok && !dvec && !kvec && (t->path == 0 || t->path == 5);
     const bool staged = use_staged(t, M, tc_call);
     const int kmode = mode == BLIPGPU_VALUE ? 0 : (t->diag ? 2 : 1);      // kernel template MODE
@@ -566,7 +569,7 @@ static int launch_eval(blipgpu_table* t, const double* positions, long long M, i
             for (int q = 0; q < 5; ++q) { scl.sw[q] = t->tc_scale[1 + q]; scl.inv[q] = t->tc_scale[6 + q]; }
             StagedArgs a16 = a;
             a16.tmap = &t->tmap16;
-            CK(t, tc_launch(kmode, (unsigned)t->nsm, s, a16, scl));
+            CK(t, tc_launch(kmode, (unsigned)t->nsm, s, a16, scl, M));
             t->last_path = 5;
         } else {
             CK(t, staged_launch(kmode, (unsigned)t->nsm, s, a));
@@ -672,6 +675,7 @@ extern "C" int blipgpu_eval_f64(blipgpu_table* t, const double* positions, long 
         return BLIPGPU_EINVAL;
     if (M >= (1LL << 31)) return BLIPGPU_EINVAL;
     cudaStream_t s = (cudaStream_t)stream;
+    t->g.M = M;                                              // bound of the checked build's asserts
     if (mode == BLIPGPU_VGH) return launch_hess<double>(t, positions, M, val, grad, lap, ld, cell, s);
     const dim3 grid((unsigned)M, (unsigned)((t->g.pitch4 + 31) / 32));
     if (mode == BLIPGPU_VALUE)
