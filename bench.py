@@ -16,6 +16,7 @@ Prints ONE JSON line on rank 0 (see DESIGN.md "Measurement" for every key).
 `--impl reference` times the CPU fp64 oracle (oracle/) on the host cores instead.
 """
 import argparse
+import hashlib
 import json
 import os
 import sys
@@ -307,17 +308,47 @@ def roofline_block(torch, blip, handle, cfg, M, L, mode_vgl, k_ms, g_ms, n_rows,
                               "-> fp32, two-term splits of both operands) per electron and 128 orbitals, not on the FP32 pipe; "
                               "SURVEY.md §8d's binding bound max(R_compulsory, R_fp32) is kept as the yardstick (frac > 1 would "
                               "mean faster than the FP32 pipe could be at its peak)")
-    traffic_file = os.path.join(ROOT, "profiles", "traffic.json")     # written from ncu --set full captures
+    out.update(recorded_traffic(f"{cfg.name}:{'vgl' if mode_vgl else 'value'}", comp_bytes))
+    return out
+
+
+def kernel_source_digest(files):
+    """sha256 over the named source files (repo-relative, in the given order): ties a number taken in a
+    separate ncu capture to the kernel sources it was taken from."""
+    h = hashlib.sha256()
+    for f in files:
+        with open(os.path.join(ROOT, f), "rb") as fh:
+            h.update(f.encode() + b"\0" + fh.read() + b"\0")
+    return h.hexdigest()
+
+
+def recorded_traffic(key, comp_bytes):
+    """DRAM bytes per launch of the dominant kernel.  NOT measured in this run: it comes from a separate
+    `ncu --set full` capture, recorded by hand in profiles/traffic.json together with the sha256 of the
+    kernel's source files at the capture (`kernel_sources`, `kernel_sources_sha256`).  It is put on the
+    line only while those files are unchanged; after any edit to them the line carries `traffic: null`
+    and `traffic_stale` instead, until the capture is redone (`python bench.py --traffic-digests` prints
+    the current digests to paste into the file)."""
+    out = {"traffic": None}
     try:
-        with open(traffic_file) as fh:
-            tr = json.load(fh)
-        key = f"{cfg.name}:{'vgl' if mode_vgl else 'value'}"
-        if key in tr:
-            out["traffic"] = tr[key]["dram_bytes_per_launch"]
-            out["traffic_source"] = tr[key].get("source")
-            out["traffic_over_compulsory"] = tr[key]["dram_bytes_per_launch"] / comp_bytes
+        with open(os.path.join(ROOT, "profiles", "traffic.json")) as fh:
+            entry = json.load(fh).get(key)
     except Exception:
-        pass
+        entry = None
+    if not entry:
+        return out
+    try:
+        now = kernel_source_digest(entry["kernel_sources"])
+    except Exception:
+        now = None
+    if now is not None and now == entry.get("kernel_sources_sha256"):
+        out["traffic"] = entry["dram_bytes_per_launch"]
+        out["traffic_over_compulsory"] = entry["dram_bytes_per_launch"] / comp_bytes
+        out["traffic_source"] = "separate ncu capture, not this run: " + str(entry.get("source"))
+    else:
+        out["traffic_stale"] = ("profiles/traffic.json has " + str(entry.get("dram_bytes_per_launch")) + " B per launch for this "
+                                "kernel, captured from other sources than the ones loaded now (" + ", ".join(entry.get("kernel_sources", []))
+                                + " changed since): not reported")
     return out
 
 
@@ -414,7 +445,7 @@ def measure_config(torch, blip, name, steps, fp32_meas, nsm, mode_vgl=True):
         rows = distinct_rows(torch, cells, cfg.grid)
         roof = roofline_block(torch, blip, w.handle, cfg, w.M, w.L, mode_vgl, k_ms, g_ms, rows, fp32_meas, nsm)
         keep = ("bound", "achieved", "peak", "unit", "frac", "kernel", "kernel_ms", "grouping_ms", "binding", "bound_ms",
-                "contract_frac", "compulsory_hbm_frac", "distinct_rows", "traffic", "traffic_source")
+                "contract_frac", "compulsory_hbm_frac", "distinct_rows", "traffic", "traffic_source", "traffic_stale")
         return {"workload": f"{cfg.name}: BASELINE.json configs[{list(workloads.CONFIGS).index(cfg.name)}]",
                 "positions": w.M, "orbitals": w.L, "grid": list(cfg.grid), "table_bytes": cfg.table_bytes,
                 "mode": "value+grad+lap" if mode_vgl else "value", "steps": steps, "ms_per_step": ms,
@@ -520,8 +551,6 @@ def run_gpu(args):
             line["contract"] = run_contract(torch, blip, handle, cfg, w.hpos, w.dpos, stream, args)
             line["f64"] = run_f64(torch, blip, handle, cfg, w.dpos, stream)
             line["hessian"] = run_hessian(torch, blip, handle, cfg, w.dpos, stream)
-            ups = -(-M * ((L + 127) // 128) // nsm)                       # units (electron x 128 orbitals) per SM of this step
-            tc = blip.blipgpu_probe_tensor(handle, ups, stream)
             fp32_staged = None
             if "eval_tc_kernel" in roofline["kernel"]:                    # the FP32-pipe staged kernel on the same batch, same run
                 blip.blipgpu_set_tuning(handle, 2, 0)
@@ -532,11 +561,9 @@ def run_gpu(args):
                                "speedup": k2 / roofline["kernel_ms"]}
             line["tensor_core_recast"] = {
                 "shipped": fp32_staged,
-                "units_per_sm": ups, "ms_fp32_ffma2_form": tc[0], "ms_tf32x3_mma_sync_form": tc[1], "ms_tf32x1_mma_sync_form": tc[2],
-                "note": "arithmetic of one step from a shared-memory tile, no TMA / plane hand-offs (csrc/blip_tcprobe.cuh): "
-                        "the K = 64 per-electron recast D[128][5] = C^T[128][64] W[64][5] on mma.sync.m16n8k8 tf32 with the "
-                        "3-term split the tolerances need, against the packed-FP32 form (SURVEY.md §8f NEXT-2); `shipped` = the "
-                        "tcgen05 kernel that replaced the FP32-pipe staged kernel for this workload, both timed here"}
+                "note": "`shipped` = the tcgen05 kernel that replaced the FP32-pipe staged kernel for this workload, both timed "
+                        "here (SURVEY.md §8f NEXT-2).  The mma.sync tf32 form of the recast was measured and rejected in round 2 "
+                        "(profiles/r2_v1.md); its probe is the harness program tests/harness/mma_sync_probe.cu, no longer in the library"}
             if L % 2 == 0:
                 line["complex"] = run_complex(torch, blip, w, args)
         if world == 1 and not args.no_configs:
@@ -756,7 +783,15 @@ def main():
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-contract", action="store_true", help="skip the blipgpu_eval_contract timing")
+    ap.add_argument("--traffic-digests", action="store_true",
+                    help="print the current sha256 of every profiles/traffic.json entry's kernel sources and exit (no GPU needed)")
     args = ap.parse_args()
+    if args.traffic_digests:
+        with open(os.path.join(ROOT, "profiles", "traffic.json")) as fh:
+            for key, entry in json.load(fh).items():
+                now = kernel_source_digest(entry["kernel_sources"])
+                print(key, now, "current" if now == entry.get("kernel_sources_sha256") else "STALE")
+        return 0
     world = int(os.environ.get("WORLD_SIZE", "1"))
     if args.gpus != world:
         if "RANK" in os.environ or args.gpus < 1:

@@ -39,16 +39,6 @@ int blipgpu_set_tuning(blipgpu_table* t, int path, int nq);
  * the run sees.  Errors: EINVAL, ENOMEM, ECUDA. */
 int blipgpu_probe_fp32(blipgpu_table* t, double* tflops, void* stream);
 
-/* blipgpu_probe_tensor — the measurement behind "tensor cores only if the dense recast is shown
- * to win" (BASELINE.json north_star; §VI.E).  Runs `units_per_sm` units (one
- * electron x 128 orbitals: D[128][5] = C^T[128][64] W[64][5] from a shared-memory tile) on every
- * SM with the launch shape of the staged kernel, three ways, and returns their times in ms[0..2]
- * (HOST): [0] packed FP32 FMAs as the shipped kernel issues them, [1] mma.sync.m16n8k8 tf32 with
- * the 3-term hi/lo split that the tolerances require, [2] a single tf32 term (fails the
- * tolerances; the tensor-pipe floor of the recast).  csrc/blip_tcprobe.cuh has the details.
- * Synchronises.  Errors: EINVAL, ENOMEM, ECUDA. */
-int blipgpu_probe_tensor(blipgpu_table* t, int units_per_sm, double* ms, void* stream);
-
 /* blipgpu_last_path — which gather+FMA kernel the last blipgpu_eval / blipgpu_eval_host of this
  * handle launched: 1 direct (one warp per electron, rows from L2/HBM), 2 staged (table planes
  * through shared memory, FP32 pipe), 5 staged on the tensor cores (table planes through tensor memory), 3 split (four warps per electron, small batches), 4 the fp64 kernel of blipgpu_eval_f64; 0 before

@@ -51,7 +51,6 @@ SIGNATURES = {
     "blipgpu_info": (ctypes.c_int, [ctypes.c_void_p, _c_ip, _c_ip, _c_llp, _c_llp]),
     "blipgpu_set_tuning": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_int, ctypes.c_int]),
     "blipgpu_probe_fp32": (ctypes.c_int, [ctypes.c_void_p, _c_dp, ctypes.c_void_p]),
-    "blipgpu_probe_tensor": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_int, _c_dp, ctypes.c_void_p]),
     "blipgpu_last_path": (ctypes.c_int, [ctypes.c_void_p]),
     "blipgpu_launch_count": (ctypes.c_longlong, [ctypes.c_void_p]),
     "blipgpu_set_profiling": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_int]),
@@ -196,13 +195,6 @@ def blipgpu_probe_fp32(handle, stream=None):
     v = ctypes.c_double()
     _check(lib().blipgpu_probe_fp32(handle, ctypes.byref(v), _stream_ptr(stream)), "blipgpu_probe_fp32", handle)
     return v.value
-
-
-def blipgpu_probe_tensor(handle, units_per_sm=2000, stream=None):
-    """ms for `units_per_sm` units per SM: (packed FP32 FMA form, 3-term tf32 mma.sync form, 1-term tf32 form)."""
-    v = (ctypes.c_double * 3)()
-    _check(lib().blipgpu_probe_tensor(handle, int(units_per_sm), v, _stream_ptr(stream)), "blipgpu_probe_tensor", handle)
-    return tuple(v)
 
 
 def blipgpu_last_path(handle):

@@ -6,7 +6,6 @@
 #include "blipgpu.h"
 #include "blipgpu_dev.h"
 #include "blip_host.h"
-#include "blip_tcprobe.cuh"
 
 int blip_default_nq(int pitch4);     // blipgpu.cu
 
@@ -108,45 +107,6 @@ extern "C" int blipgpu_probe_fp32(blipgpu_table* t, double* tflops, void* stream
     cudaFree(out);
     t->launches += 3;
     return rc;
-}
-
-template <int FORM>
-static cudaError_t tc_probe_run(int nsm, float* out, int units_per_warp, cudaStream_t s, float* ms)
-{
-    cudaError_t e = cudaFuncSetAttribute(blip::tc_probe_kernel<FORM>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                         (int)sizeof(blip::TcSmem));
-    cudaEvent_t e0 = nullptr, e1 = nullptr;
-    if (e == cudaSuccess) e = cudaEventCreate(&e0);
-    if (e == cudaSuccess) e = cudaEventCreate(&e1);
-    for (int rep = 0; rep < 3 && e == cudaSuccess; ++rep) {          // the last of three runs is timed
-        e = cudaEventRecord(e0, s);
-        blip::tc_probe_kernel<FORM><<<nsm, blip::kTcWarps * 32, sizeof(blip::TcSmem), s>>>(out, units_per_warp, 1e-3f);
-        if (e == cudaSuccess) e = cudaGetLastError();
-        if (e == cudaSuccess) e = cudaEventRecord(e1, s);
-        if (e == cudaSuccess) e = cudaEventSynchronize(e1);
-        if (e == cudaSuccess) e = cudaEventElapsedTime(ms, e0, e1);
-    }
-    if (e0) cudaEventDestroy(e0);
-    if (e1) cudaEventDestroy(e1);
-    return e;
-}
-
-extern "C" int blipgpu_probe_tensor(blipgpu_table* t, int units_per_sm, double* ms, void* stream)
-{
-    if (!t || !ms || units_per_sm < blip::kTcWarps) return BLIPGPU_EINVAL;
-    cudaStream_t s = (cudaStream_t)stream;
-    const int upw = units_per_sm / blip::kTcWarps;
-    float* out = nullptr;
-    CK(t, cudaMalloc(&out, sizeof(float) * (size_t)t->nsm * blip::kTcWarps * 5 * 128));
-    float v[3] = {0.f, 0.f, 0.f};
-    cudaError_t e = tc_probe_run<0>(t->nsm, out, upw, s, &v[0]);
-    if (e == cudaSuccess) e = tc_probe_run<1>(t->nsm, out, upw, s, &v[1]);
-    if (e == cudaSuccess) e = tc_probe_run<2>(t->nsm, out, upw, s, &v[2]);
-    cudaFree(out);
-    t->launches += 9;
-    if (e != cudaSuccess) { t->last_cuda = (int)e; (void)cudaGetLastError(); return BLIPGPU_ECUDA; }
-    for (int k = 0; k < 3; ++k) ms[k] = v[k];
-    return BLIPGPU_OK;
 }
 
 extern "C" int blipgpu_last_path(const blipgpu_table* t) { return t ? t->last_path : 0; }

@@ -52,5 +52,18 @@ def build_tcgen05_check(force=False):
     return exe
 
 
+def build_mma_sync_probe(force=False):
+    """tests/harness/mma_sync_probe.cu (+ .cuh) -> tests/harness/mma_sync_probe (nvcc, sm_100a): the settled
+    mma.sync tf32 recast experiment of SURVEY.md §8f NEXT-2, kept out of the shipped library."""
+    if ROOT not in sys.path:
+        sys.path.insert(0, ROOT)
+    from paper_1204_1121_b200 import _build
+    srcs = [os.path.join(HERE, "mma_sync_probe.cu"), os.path.join(HERE, "mma_sync_probe.cuh")]
+    exe = os.path.join(HERE, "mma_sync_probe")
+    if force or not os.path.exists(exe) or any(os.path.getmtime(x) > os.path.getmtime(exe) for x in srcs):
+        subprocess.run([_build.nvcc(), "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-o", exe, srcs[0]], check=True)
+    return exe
+
+
 if __name__ == "__main__":
     print(build(force=True, checked="--checked" in sys.argv))

@@ -1,7 +1,9 @@
-// blip_tcprobe.cuh — timing probe for the tensor-core recast of the gather + FMA step
+// mma_sync_probe.cuh — timing probe for the tensor-core recast of the gather + FMA step
 // (§VI.E, Eq. 13-15: psi = A(r_j) . Theta is a matrix
-// product, rejected by the paper because A changes with r_j).  Developer instrumentation
-// (include/blipgpu_dev.h), not on the evaluation path; its outputs are not orbitals.
+// product, rejected by the paper because A changes with r_j).  A settled experiment, kept as a
+// harness program (tests/harness/mma_sync_probe.cu) outside the shipped library: the mma.sync
+// form lost to packed FP32 FMAs (profiles/r2_v1.md), the tcgen05 form of csrc/blip_tc.cuh won.
+// Its outputs are not orbitals.
 //
 // What it times.  One "unit" of the staged kernel is one electron x 128 orbitals: the 64 site
 // rows of the electron's 4x4x4 block, already in shared memory, against 5 weight vectors
@@ -24,12 +26,12 @@
 //   form 2  form 1 with a single tf32 term (64 MMAs per unit, no split): the tensor-pipe floor
 //           of the recast if precision were not an issue.
 #pragma once
-#include "blip_types.h"
+#include <cuda_runtime.h>
 
-namespace blip {
+namespace blip_probe {
 
-constexpr int kTcWarps = 16;
-constexpr int kTcPitch = 136;                               // floats per site row of the padded tile
+constexpr int kProbeWarps = 16;
+constexpr int kProbePitch = 136;                               // floats per site row of the padded tile
 
 __device__ __forceinline__ void mma_tf32(float (&d)[4], const unsigned (&a)[4], unsigned b0, unsigned b1)
 {
@@ -38,23 +40,23 @@ __device__ __forceinline__ void mma_tf32(float (&d)[4], const unsigned (&a)[4], 
                  : "r"(a[0]), "r"(a[1]), "r"(a[2]), "r"(a[3]), "r"(b0), "r"(b1));
 }
 
-struct TcSmem {
-    float tile[64 * kTcPitch];                               // 64 site rows x 128 orbitals (+ 8 pad)
-    float wts[kTcWarps][3][3][4];                            // per warp: per-axis w, w', w'' at the 4 sites
-    float dfrag[kTcWarps][8][16 * 9];                        // per warp: D of one orbital tile, [16 orbitals][8 + 1 pad]
+struct ProbeSmem {
+    float tile[64 * kProbePitch];                               // 64 site rows x 128 orbitals (+ 8 pad)
+    float wts[kProbeWarps][3][3][4];                            // per warp: per-axis w, w', w'' at the 4 sites
+    float dfrag[kProbeWarps][8][16 * 9];                        // per warp: D of one orbital tile, [16 orbitals][8 + 1 pad]
 };
 
 template <int FORM>
-__global__ void __launch_bounds__(kTcWarps * 32, 1)
-tc_probe_kernel(float* __restrict__ out, int units_per_warp, float seed)
+__global__ void __launch_bounds__(kProbeWarps * 32, 1)
+mma_sync_probe_kernel(float* __restrict__ out, int units_per_warp, float seed)
 {
-    extern __shared__ __align__(16) unsigned char tc_raw[];
-    TcSmem& sm = *reinterpret_cast<TcSmem*>(tc_raw);
+    extern __shared__ __align__(16) unsigned char probe_raw[];
+    ProbeSmem& sm = *reinterpret_cast<ProbeSmem*>(probe_raw);
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    for (int i = threadIdx.x; i < 64 * kTcPitch; i += blockDim.x) sm.tile[i] = seed * (float)((i * 2654435761u) >> 20);
+    for (int i = threadIdx.x; i < 64 * kProbePitch; i += blockDim.x) sm.tile[i] = seed * (float)((i * 2654435761u) >> 20);
     if (lane < 12) for (int k = 0; k < 3; ++k) sm.wts[warp][lane >> 2][k][lane & 3] = seed * (float)(lane + 3 * k + 1);
     __syncthreads();
-    float* orow = out + ((size_t)blockIdx.x * kTcWarps + warp) * 5 * 128;      // one unit's worth of output rows, rewritten
+    float* orow = out + ((size_t)blockIdx.x * kProbeWarps + warp) * 5 * 128;      // one unit's worth of output rows, rewritten
     float drift = 0.f;
     if (FORM == 0) {
         // ---- packed FP32 form: lane owns 4 orbitals; 16 columns x (4 LDS.128 + 36 FFMA2)
@@ -82,7 +84,7 @@ tc_probe_kernel(float* __restrict__ out, int units_per_warp, float seed)
                 ulonglong2 c[4];
 #pragma unroll
                 for (int m = 0; m < 4; ++m)
-                    asm volatile("ld.shared.v2.b64 {%0, %1}, [%2];" : "=l"(c[m].x), "=l"(c[m].y) : "r"(base + (4 * col + m) * (kTcPitch * 4)));
+                    asm volatile("ld.shared.v2.b64 {%0, %1}, [%2];" : "=l"(c[m].x), "=l"(c[m].y) : "r"(base + (4 * col + m) * (kProbePitch * 4)));
 #pragma unroll
                 for (int p = 0; p < 2; ++p) {
                     const u64 c0 = p ? c[0].y : c[0].x, c1 = p ? c[1].y : c[1].x, c2 = p ? c[2].y : c[2].x, c3 = p ? c[3].y : c[3].x;
@@ -133,8 +135,8 @@ tc_probe_kernel(float* __restrict__ out, int units_per_warp, float seed)
 #pragma unroll
                 for (int ks = 0; ks < 8; ++ks) {
                     // A fragment: C^T[orbital][site]: (g, t), (g + 8, t), (g, t + 4), (g + 8, t + 4)
-                    const float x0 = col[(8 * ks + t) * kTcPitch], x1 = col[(8 * ks + t) * kTcPitch + 8];
-                    const float x2 = col[(8 * ks + t + 4) * kTcPitch], x3 = col[(8 * ks + t + 4) * kTcPitch + 8];
+                    const float x0 = col[(8 * ks + t) * kProbePitch], x1 = col[(8 * ks + t) * kProbePitch + 8];
+                    const float x2 = col[(8 * ks + t + 4) * kProbePitch], x3 = col[(8 * ks + t + 4) * kProbePitch + 8];
                     unsigned ahi[4] = {__float_as_uint(x0) & 0xffffe000u, __float_as_uint(x1) & 0xffffe000u,
                                        __float_as_uint(x2) & 0xffffe000u, __float_as_uint(x3) & 0xffffe000u};
                     mma_tf32(d, ahi, bhi[ks][0], bhi[ks][1]);
@@ -166,4 +168,4 @@ tc_probe_kernel(float* __restrict__ out, int units_per_warp, float seed)
     if (drift == 123.456f) out[0] = drift;
 }
 
-}  // namespace blip
+}  // namespace blip_probe

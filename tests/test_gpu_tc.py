@@ -4,6 +4,7 @@ layout makes special (ragged orbital chunks, grids that are not a multiple of th
 every z offset of an electron in its pencil, non-finite positions, tables of very different
 scale), run-to-run bit identity, and the fall-backs."""
 import os
+import re
 import subprocess
 import sys
 
@@ -29,6 +30,17 @@ def test_tcgen05_facts_the_kernel_relies_on():
     r = subprocess.run([exe], capture_output=True, text=True, timeout=120)
     assert r.returncode == 0, r.stdout + r.stderr
     assert "tcgen05_check: 0 failure(s)" in r.stdout
+
+
+def test_mma_sync_probe_harness_program_runs():
+    """tests/harness/mma_sync_probe.cu — the settled mma.sync tf32 recast experiment,
+    moved out of libblipgpu.so: it still builds and times its three forms."""
+    exe = harness_build.build_mma_sync_probe()
+    r = subprocess.run([exe, "400"], capture_output=True, text=True, timeout=120)
+    assert r.returncode == 0, r.stdout + r.stderr
+    ms = [float(x) for x in re.findall(r"([0-9.]+) ms", r.stdout)]
+    assert len(ms) == 3 and all(m > 0 for m in ms), r.stdout
+
 
 TRICLINIC = ((20.0, 0.0, 0.0), (3.0, 19.0, 0.0), (2.0, 2.0, 24.0))
 ORTHO = ((10.0, 0.0, 0.0), (0.0, 9.0, 0.0), (0.0, 0.0, 8.0))
