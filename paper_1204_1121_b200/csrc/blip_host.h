@@ -21,7 +21,8 @@ struct blipgpu_table {
     int tc_ok = 0;                   // tensor-core form of the staged kernel usable (finite table, shared memory fits)
     unsigned* table16 = nullptr;     // device, the table of the tensor-core path: scaled fp16 halves, z pairs (blip_tc.cuh)
     CUtensorMap tmap16;              // its 5-D TMA descriptor
-    float tc_scale[11] = {0};        // blip::TcScale: 2^kc of the coefficients, 2^kq and 1 / 2^(kc + kq) per quantity
+    float tc_scale[11] = {0};        // blip::TcScale: [1..5] 2^kq of the weights of quantity q, [6..10] 2^-kq ([0] unused)
+    float* tc_oscale = nullptr;      // device [2][pitch]: 2^k_l per orbital applied to the fp16 table, and 2^-k_l (built with table16)
     int nchunk = 0;                  // staged path: orbital chunks of 128
     int nsm = 0;                     // SMs of the device (CTAs of the persistent staged kernel)
     long long l2_bytes = 0;          // L2 capacity of the device

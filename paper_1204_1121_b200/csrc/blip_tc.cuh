@@ -20,8 +20,11 @@
 //
 // Precision.  The tensor core multiplies fp16 (11 significant bits); north_star's tolerances
 // need ~2^-20.  Both operands are split exactly in two fp16 halves after an exact power-of-two
-// scaling: c' = c 2^kc = c1 + c2 (c1 = rn16(c'), c2 = rn16(c' - c1): 22 bits), W' = W 2^kq =
-// W1 + W2 likewise.  The B tile carries [W1 | W2] in its N dimension (columns 0..4 and 5..9), the A
+// scaling: c' = c 2^k_l = c1 + c2 (c1 = rn16(c'), c2 = rn16(c' - c1): 22 bits), W' = W 2^kq =
+// W1 + W2 likewise.  The coefficient scale is PER ORBITAL l (the M rows of the MMA are orbitals):
+// 2^k_l max|c_l| in [2^8, 2^9), so an orbital whose amplitude is far below the table's maximum keeps
+// its own 22 bits instead of falling on the fp16 subnormal floor of a table-wide scale; the epilogue
+// lane that holds orbital l undoes it with one more exact multiply (reading R12a).  The B tile carries [W1 | W2] in its N dimension (columns 0..4 and 5..9), the A
 // operand is issued twice (c1, c2) into the same accumulators, so that D[:, q] + D[:, 5 + q] =
 // (c1 + c2)(W1 + W2) summed over the sites in fp32: all four cross terms, error ~2^-21 of
 // sum |c W|.  Per electron and 128 orbitals: 4 planes x 2 row pairs x 2 halves = 16 MMAs.
@@ -74,10 +77,10 @@ static_assert(kTcNB % kTcNW == 0 && kTcNB % kTcNI == 0, "a B slot belongs to one
 static_assert(kTcND % kTcNI == 0 && kTcND % 2 == 0, "an accumulator slot belongs to one issuer and one epilogue group");
 
 struct TcScale {
-    float sc;           // 2^kc applied to the coefficients
     float sw[5];        // 2^kq applied to the weights of quantity q (val, T1, T2, T3, lap)
-    float inv[5];       // 1 / (sc sw[q])
+    float inv[5];       // 1 / sw[q]; the per-orbital 2^-k_l comes from the `oscale` array (tc_colscale_kernel)
 };
+constexpr int kTcMaxScaleExp = 100; // |k_l| <= 100: the host admits tables with max|c| < 2^100 only, and 2^-(k_l + kq) stays a normal fp32
 
 struct TcSmem {
     alignas(128) unsigned plane[kTcRS][kTcPlaneWords];       // [y 7][z pair 4][half 2][128 orbitals], one TMA box
@@ -170,8 +173,9 @@ __device__ __forceinline__ void tma_prefetch_5d(const CUtensorMap* tmap, int c0,
 //     T16[p1][p2][zp][half][l] = { c_half[p1][p2][2 zp][l], c_half[p1][p2][2 zp + 1][l] << 16 }
 // — exactly the word a TMEM column of the A operand holds, so that the converter warps only move
 // words from the staged plane to tensor memory.  Same bytes per coefficient as fp32.
+// oscale[l] = 2^k_l, the scale of orbital l (tc_colscale_kernel).
 __global__ void __launch_bounds__(256)
-tc_table_kernel(Geom g, float sc, int nzp, const float* __restrict__ padded /* [np1][np2][np3][pitch], the fp32 table */,
+tc_table_kernel(Geom g, const float* __restrict__ oscale, int nzp, const float* __restrict__ padded /* [np1][np2][np3][pitch], the fp32 table */,
                 unsigned* __restrict__ dst, long long total)
 {
     const long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x;
@@ -181,6 +185,7 @@ tc_table_kernel(Geom g, float sc, int nzp, const float* __restrict__ padded /* [
     const long long r = idx / pitch;                         // (p1 np2 + p2) nzp + zp
     const int zp = (int)(r % nzp);
     const long long p12 = r / nzp;
+    const float sc = __ldg(oscale + l);
     float c[2] = {0.f, 0.f};
 #pragma unroll
     for (int h = 0; h < 2; ++h) {
@@ -256,7 +261,8 @@ __global__ void __launch_bounds__(kTcThreads, 1)
 eval_tc_kernel(const __grid_constant__ CUtensorMap tmap, Geom g, StagedGeom sg, TcScale scl,
                const float4* __restrict__ recs, const int4* __restrict__ order, int* __restrict__ meta,
                int nchunk, float* __restrict__ val, float* __restrict__ grad, float* __restrict__ lap, long long ld,
-               int idx32_arg /* every output element offset of this call fits 32 bits (tc_launch derives it from M and ld) */)
+               int idx32_arg /* every output element offset of this call fits 32 bits (tc_launch derives it from M and ld) */,
+               const float* __restrict__ oinv /* [pitch] 2^-k_l: undoes the per-orbital scale of the fp16 table */)
 {
     extern __shared__ __align__(128) unsigned char smem_raw[];
     TcSmem& sm = *reinterpret_cast<TcSmem*>(smem_raw);
@@ -411,6 +417,7 @@ eval_tc_kernel(const __grid_constant__ CUtensorMap tmap, Geom g, StagedGeom sg, 
             float* const gcol = grad + col;
             float* const lcol = lap + col;
             const bool col_ok = col < 4 * g.pitch4;
+            const float oi = col_ok ? __ldg(oinv + col) : 1.0f;      // this lane's orbital: 2^-k_l
             for (unsigned u = (ubase + (unsigned)eg) & 1u; u < it_nunits; u += 2) {      // (ubase + u) % 2 == eg
                 const unsigned uc = ubase + u, d = uc % kTcND;
                 mbar_wait_relaxed(smem_u32(&sm.dfull[d]), (uc / kTcND) & 1u);
@@ -432,7 +439,7 @@ eval_tc_kernel(const __grid_constant__ CUtensorMap tmap, Geom g, StagedGeom sg, 
                 float q[5];
 #pragma unroll
                 for (int k = 0; k < 5; ++k)
-                    q[k] = (MODE != 0 || k == 0) ? __fmul_rn(__fadd_rn(__uint_as_float(r[k]), __uint_as_float(r[k + 5])), scl.inv[k]) : 0.f;
+                    q[k] = (MODE != 0 || k == 0) ? __fmul_rn(__fmul_rn(__fadd_rn(__uint_as_float(r[k]), __uint_as_float(r[k + 5])), oi), scl.inv[k]) : 0.f;   // two exact power-of-two multiplies
                 if (inf.x < 0)                               // non-finite position (R17): the same for the whole warp, and rare
                     asm volatile("mov.b32 %0, 0x7fc00000; mov.b32 %1, 0x7fc00000; mov.b32 %2, 0x7fc00000; mov.b32 %3, 0x7fc00000; mov.b32 %4, 0x7fc00000;"
                                  : "=f"(q[0]), "=f"(q[1]), "=f"(q[2]), "=f"(q[3]), "=f"(q[4]));
@@ -577,7 +584,37 @@ eval_tc_kernel(const __grid_constant__ CUtensorMap tmap, Geom g, StagedGeom sg, 
     if (warp == 0) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, 512;" :: "r"(tbase) : "memory");
 }
 
-// max |c| of the caller's table (for the power-of-two scaling); non-finite entries set bit 31 of the result
+// max |c_l| of every orbital column l of the padded table [nrows][pitch], as the bits of a non-negative float,
+// into colmax[pitch] (zero on entry).  Thread = column, CTAs stride over the rows: coalesced.
+__global__ void __launch_bounds__(256) tc_colmax_kernel(const float* __restrict__ padded, long long nrows, int pitch, unsigned* __restrict__ colmax)
+{
+    const int l = blockIdx.y * blockDim.x + threadIdx.x;
+    if (l >= pitch) return;
+    unsigned m = 0;
+    for (long long r = blockIdx.x; r < nrows; r += gridDim.x)
+        m = max(m, __float_as_uint(__ldg(padded + (size_t)r * (size_t)pitch + l)) & 0x7fffffffu);
+    if (m) atomicMax(colmax + l, m);
+}
+
+// Per-orbital power-of-two scale of the fp16 table: oscale[l] = 2^k_l with 2^k_l max|c_l| in [2^8, 2^9)
+// (k_l clamped to +-kTcMaxScaleExp; 1 for an all-zero column, which the pad columns l >= L are), and
+// oscale[pitch + l] = 2^-k_l for the epilogue.  Both exact.
+__global__ void __launch_bounds__(256) tc_colscale_kernel(const unsigned* __restrict__ colmax, int pitch, float* __restrict__ oscale)
+{
+    const int l = blockIdx.x * blockDim.x + threadIdx.x;
+    if (l >= pitch) return;
+    const float a = __uint_as_float(colmax[l]);
+    int k = 0;
+    if (a > 0.f) {
+        int ex;
+        (void)frexpf(a, &ex);                                // a = m 2^ex, m in [0.5, 1)
+        k = min(kTcMaxScaleExp, max(-kTcMaxScaleExp, 9 - ex));
+    }
+    oscale[l] = ldexpf(1.0f, k);
+    oscale[pitch + l] = ldexpf(1.0f, -k);
+}
+
+// max |c| of the caller's table (admission to the tensor-core path: finite, below 2^100); non-finite entries set bit 31 of the result
 __global__ void __launch_bounds__(256) tc_absmax_kernel(const float* __restrict__ src, long long nfloats, unsigned* __restrict__ out)
 {
     unsigned m = 0;

@@ -97,13 +97,14 @@ cudaError_t tc_prepare()
     if (e == cudaSuccess) e = cudaFuncSetAttribute(blip::eval_tc_kernel<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(blip::TcSmem));
     return e;
 }
-cudaError_t tc_launch(int mode, unsigned nctas, cudaStream_t s, const StagedArgs& a, const blip::TcScale& scl, long long M)
+cudaError_t tc_launch(int mode, unsigned nctas, cudaStream_t s, const StagedArgs& a, const blip::TcScale& scl, long long M,
+                      const float* oinv)
 {
     // the epilogue addresses val / grad / lap with 32-bit element offsets when the largest one of this
     // call, (M - 1) * 3 * ld + 3 * ld - 1 (the gradient's), fits; decided here, next to the launch
     const int idx32 = (unsigned long long)M * 3ull * (unsigned long long)a.ld < (1ull << 32) ? 1 : 0;
 #define BLIP_TC(MODE) launch_pdl(blip::eval_tc_kernel<MODE>, nctas, blip::kTcThreads, sizeof(blip::TcSmem), s, *a.tmap, *a.g, *a.sg, scl, \
-                                 a.recs, a.order, a.meta, a.nchunk, a.val, a.grad, a.lap, a.ld, idx32)
+                                 a.recs, a.order, a.meta, a.nchunk, a.val, a.grad, a.lap, a.ld, idx32, oinv)
     if (mode == 0) return BLIP_TC(0);
     if (mode == 2) return BLIP_TC(2);
     return BLIP_TC(1);
@@ -182,13 +183,26 @@ static bool ensure_tc_table(blipgpu_table* t, cudaStream_t s)
     const int nzp = (t->g.np[2] + 1) / 2;
     const long long words = (long long)t->g.np[0] * t->g.np[1] * nzp * 2 * t->pitch;
     bool fine = cudaMalloc(&t->table16, sizeof(unsigned) * (size_t)words) == cudaSuccess;
+    unsigned* colmax = nullptr;                              // max |c_l| per orbital, only needed here
+    const int pitch = (int)t->pitch;
+    fine = fine && cudaMalloc(&t->tc_oscale, sizeof(float) * 2 * (size_t)pitch) == cudaSuccess &&
+           cudaMalloc(&colmax, sizeof(unsigned) * (size_t)pitch) == cudaSuccess &&
+           cudaMemsetAsync(colmax, 0, sizeof(unsigned) * (size_t)pitch, s) == cudaSuccess;
     if (fine) {
+        const float* padded = reinterpret_cast<const float*>(t->table);
+        const dim3 cgrid((unsigned)(t->nrows < 8LL * t->nsm ? t->nrows : 8LL * t->nsm), (unsigned)((pitch + 255) / 256));
+        blip::tc_colmax_kernel<<<cgrid, 256, 0, s>>>(padded, t->nrows, pitch, colmax);
+        blip::tc_colscale_kernel<<<(unsigned)((pitch + 255) / 256), 256, 0, s>>>(colmax, pitch, t->tc_oscale);
         const long long total = words / 2;
-        blip::tc_table_kernel<<<(unsigned)((total + 255) / 256), 256, 0, s>>>(t->g, t->tc_scale[0], nzp, reinterpret_cast<const float*>(t->table),
-                                                                           t->table16, total);
+        blip::tc_table_kernel<<<(unsigned)((total + 255) / 256), 256, 0, s>>>(t->g, t->tc_oscale, nzp, padded, t->table16, total);
         fine = cudaGetLastError() == cudaSuccess && cudaStreamSynchronize(s) == cudaSuccess && build_tensor_map16(t, nzp);
     }
-    if (!fine) { cudaFree(t->table16); t->table16 = nullptr; t->tc_ok = 0; (void)cudaGetLastError(); }
+    cudaFree(colmax);
+    if (!fine) {
+        cudaFree(t->table16); cudaFree(t->tc_oscale);
+        t->table16 = nullptr; t->tc_oscale = nullptr; t->tc_ok = 0;
+        (void)cudaGetLastError();
+    }
     return fine;
 }
 
@@ -379,8 +393,10 @@ extern "C" int blipgpu_create(const double* lattice, const int* grid, int norb,
             if (e == cudaSuccess) t->staged_ok = 1; else (void)cudaGetLastError();
         }
         // tensor-core form: a finite table (a NaN or Inf would reach electrons that do not touch it
-        // through the zero-weight rows of an MMA) and power-of-two scales that bring the coefficients
-        // to <= 2^9 and the weights of every quantity to <= 2^8 in fp16 (blip_tc.cuh)
+        // through the zero-weight rows of an MMA) with max|c| < 2^100, and power-of-two scales that bring
+        // the coefficients of every orbital to < 2^9 (per orbital, chosen on the device when the fp16
+        // table is built: ensure_tc_table) and the weights of every quantity to <= 2^8 in fp16 (blip_tc.cuh);
+        // 2^-kq within 2^+-26 so that 2^-(k_l + kq) is a normal fp32 for every orbital
         if (t->staged_ok && !(absmax_bits & 0x80000000u) && (size_t)prop.sharedMemPerBlockOptin >= sizeof(blip::TcSmem) &&
             tc_prepare() == cudaSuccess) {
             float amax;
@@ -390,12 +406,12 @@ extern "C" int blipgpu_create(const double* lattice, const int* grid, int norb,
             const double bound[5] = {1.0, jd[0], jd[1], jd[2],
                                      2.0 * (std::fabs(Q[0]) + std::fabs(Q[1]) + std::fabs(Q[2])) +
                                          4.0 * (std::fabs(Q[3]) + std::fabs(Q[4]) + std::fabs(Q[5]))};
-            t->tc_scale[0] = pow2_scale((double)amax, 9);
-            bool fine = std::isfinite(t->tc_scale[0]) && t->tc_scale[0] > 0.f;
+            t->tc_scale[0] = 1.0f;
+            bool fine = amax < std::ldexp(1.0f, blip::kTcMaxScaleExp);
             for (int q = 0; q < 5; ++q) {
                 t->tc_scale[1 + q] = pow2_scale(bound[q], 8);
-                t->tc_scale[6 + q] = 1.0f / (t->tc_scale[0] * t->tc_scale[1 + q]);
-                fine = fine && std::isfinite(t->tc_scale[1 + q]) && t->tc_scale[1 + q] > 0.f && std::isfinite(t->tc_scale[6 + q]) && t->tc_scale[6 + q] > 0.f;
+                t->tc_scale[6 + q] = 1.0f / t->tc_scale[1 + q];
+                fine = fine && std::isfinite(t->tc_scale[1 + q]) && t->tc_scale[6 + q] >= std::ldexp(1.0f, -26) && t->tc_scale[6 + q] <= std::ldexp(1.0f, 26);
             }
             t->tc_ok = fine ? 1 : 0;
         }
@@ -423,7 +439,7 @@ extern "C" int blipgpu_create(const double* lattice, const int* grid, int norb,
 extern "C" int blipgpu_destroy(blipgpu_table* t)
 {
     if (!t) return BLIPGPU_OK;
-    cudaFree(t->table); cudaFree(t->table16); cudaFree(t->bin); cudaFree(t->perm); cudaFree(t->recs); cudaFree(t->hist); cudaFree(t->offs); cudaFree(t->counters); cudaFree(t->gstate);
+    cudaFree(t->table); cudaFree(t->table16); cudaFree(t->tc_oscale); cudaFree(t->bin); cudaFree(t->perm); cudaFree(t->recs); cudaFree(t->hist); cudaFree(t->offs); cudaFree(t->counters); cudaFree(t->gstate);
     cudaFree(t->order); cudaFree(t->meta); cudaFree(t->kvec);
     cudaFree(t->d_pos); cudaFree(t->d_val); cudaFree(t->d_grad); cudaFree(t->d_lap); cudaFree(t->d_cell);
     for (int k = 0; k < 3; ++k) if (t->pe[k]) cudaEventDestroy(t->pe[k]);
@@ -565,11 +581,10 @@ static int launch_eval(blipgpu_table* t, const double* positions, long long M, i
                               val, grad, lap, ld, dvec, ldd, cout, positions, kvec};
         if ((t->path == 5 || t->path == 0) && t->tc_ok && !dvec && !kvec && ensure_tc_table(t, s)) {   // storing epilogue: on the tensor cores
             blip::TcScale scl;
-            scl.sc = t->tc_scale[0];
             for (int q = 0; q < 5; ++q) { scl.sw[q] = t->tc_scale[1 + q]; scl.inv[q] = t->tc_scale[6 + q]; }
             StagedArgs a16 = a;
             a16.tmap = &t->tmap16;
-            CK(t, tc_launch(kmode, (unsigned)t->nsm, s, a16, scl, M));
+            CK(t, tc_launch(kmode, (unsigned)t->nsm, s, a16, scl, M, t->tc_oscale + t->pitch));
             t->last_path = 5;
         } else {
             CK(t, staged_launch(kmode, (unsigned)t->nsm, s, a));

@@ -13,7 +13,8 @@ import pytest
 
 import oracle
 import workloads
-from test_gpu_parity import compare, compare_all, run_gpu, tolerances, torch_cuda, blip, tio2  # noqa: F401 (fixtures)
+from test_gpu_parity import (GRAD_TOL, LAP_TOL, VAL_TOL, compare, compare_all, run_gpu, tolerances,  # noqa: F401 (fixtures)
+                             torch_cuda, blip, tio2)
 
 pytestmark = pytest.mark.gpu
 
@@ -116,8 +117,8 @@ def test_non_finite_positions_and_far_away_ones(torch_cuda, blip):
 
 @pytest.mark.parametrize("scale", [1e-12, 3e-4, 1.0, 7e5, 1e20])
 def test_table_scale(torch_cuda, blip, scale):
-    """The coefficients go through fp16 after a power-of-two scaling by the table's max |c|: tables
-    far outside the fp16 range keep north_star's tolerances (which are relative to max |c|)."""
+    """The coefficients go through fp16 after a power-of-two scaling by each orbital's max |c_l|: tables
+    far outside the fp16 range keep north_star's tolerances."""
     grid, L = (9, 10, 13), 130
     A, c, pos = workloads.small_case(grid, L, 3000, TRICLINIC, seed=11)
     c = (c * np.float32(scale)).astype(np.float32)
@@ -127,9 +128,47 @@ def test_table_scale(torch_cuda, blip, scale):
     t.close()
 
 
+@pytest.mark.parametrize("mode", [1, 0])
+def test_orbitals_of_very_different_norm_keep_their_own_accuracy(torch_cuda, blip, mode):
+    """Real blip tables hold orbitals of very different amplitude (PAPER.md:298-322 relies on
+    fp32-accurate orbitals).  The fp16 table is scaled per orbital (the M rows of the MMA are orbitals),
+    so every orbital meets north_star's factors against ITS OWN max|c_l| — 2e-5, 2e-5 / h, 5e-5 / h^2 —
+    not only against the table's maximum: amplitudes from 1 down to 1e-6 across the 130 orbitals, a
+    few all-zero ones, and one orbital 1e-30 of the rest (a table-wide scale would return its fp16
+    subnormal floor: relative errors of 1e-2 and worse from 1e-4 down)."""
+    grid, L = (9, 10, 13), 130
+    A, c, pos = workloads.small_case(grid, L, 3000, TRICLINIC, seed=15)
+    amp = (10.0 ** (-6.0 * np.arange(L) / (L - 1))).astype(np.float32)
+    rng = np.random.default_rng(16)
+    amp = amp[rng.permutation(L)]                           # amplitudes in no particular order along a 128-orbital chunk
+    amp[[5, 64, 129]] = 0.0
+    amp[100] = 1e-30
+    c = (c * amp).astype(np.float32)
+    t = tc_table(blip, A, grid, c)
+    val, grad, lap, cell = run_gpu(torch_cuda, blip, A, grid, c, pos, mode=mode, table=t)
+    assert blip.blipgpu_last_path(t.handle) == 5
+    oval, ograd, olap, ocell = oracle.eval_fast(A, grid, c, pos, mode=mode)
+    assert np.array_equal(cell, ocell)
+    cmax_l = np.abs(c).reshape(-1, L).max(axis=0).astype(np.float64)
+    h = float(oracle.spacing(A, grid).max())
+    worst = {}
+    for name, got, want, fac in (("val", val, oval, VAL_TOL), ("grad", grad, ograd, GRAD_TOL / h), ("lap", lap, olap, LAP_TOL / h ** 2)):
+        if got is None:
+            continue
+        err = np.abs(got.astype(np.float64) - want)
+        err = err.max(axis=tuple(range(err.ndim - 1)))      # worst over positions (and components), per orbital
+        zero = cmax_l == 0
+        assert (err[zero] == 0).all(), f"{name}: an all-zero orbital must return exact zeros"
+        frac = err[~zero] / (fac * cmax_l[~zero])
+        worst[name] = float(frac.max())
+        assert frac.max() <= 1.0, f"{name}: orbital {np.flatnonzero(~zero)[frac.argmax()]} is at {frac.max():.2f} of ITS tolerance"
+    print("per-orbital worst fraction of tolerance:", worst)
+    t.close()
+
+
 def test_sparse_table_with_a_few_large_entries(torch_cuda, blip):
-    """Most coefficients tiny against max |c| (they fall into fp16's subnormal range after scaling):
-    the error bound is absolute in max |c|, so the tolerances hold."""
+    """Most coefficients tiny against their orbital's max |c_l| (they fall into fp16's subnormal range
+    after scaling): the error bound is absolute in max |c_l|, so the tolerances hold."""
     grid, L = (9, 10, 13), 130
     A, c, pos = workloads.small_case(grid, L, 3000, TRICLINIC, seed=12)
     c = (c * np.float32(1e-6)).astype(np.float32)

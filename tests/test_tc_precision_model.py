@@ -9,7 +9,9 @@ cross products are exact in fp32 and are added in fp32.  The test shows that
   of north_star's tolerances (2e-5 max|c| for values, 5e-5 max|c| / h^2 for Laplacians);
 * one fp16 term per operand is NOT enough (it breaks the value tolerance), i.e. the second MMA per
   coefficient term and the [W1 | W2] stacking of the weight tile are needed;
-* the scaling keeps tables from 1e-12 to 1e20 and weights up to 1e4 inside the fp16 range.
+* the scaling keeps tables from 1e-12 to 1e20 and weights up to 1e4 inside the fp16 range;
+* the coefficient scale is per orbital: an orbital 1e-6 of the table's maximum keeps the tolerances
+  against its own max|c_l|, which a table-wide scale does not.
 """
 import numpy as np
 import pytest
@@ -68,6 +70,29 @@ def test_site_sum_error_against_the_tolerances(cscale, wbound):
     # value weights sum to 1 (wbound = 1 row): tolerance 2e-5 max|c|; Laplacian weights are bounded by
     # ~12 / h^2 in magnitude sum: tolerance 5e-5 max|c| / h^2 — either way the model is 20 x inside
     assert worst <= 1e-6
+
+
+def test_per_orbital_scale_keeps_small_orbitals_accurate():
+    """The scale is chosen per orbital (2^k_l max|c_l| in [2^8, 2^9)), not per table: an orbital 1e-6 of
+    the table's maximum keeps an error of ~2^-21 of ITS sum |c W|.  Under a table-wide scale the same
+    orbital sits on the fp16 subnormal floor (absolute error 2^-25 per coefficient on the scaled
+    axis) and misses the value tolerance measured against its own max|c_l| by orders of magnitude."""
+    rng = np.random.default_rng(3)
+    table_max, amp = np.float32(6.0), np.float32(1e-6)
+    worst_own, worst_global = 0.0, 0.0
+    for trial in range(200):
+        c = (rng.standard_normal(64) * amp).astype(np.float32)
+        w = rng.dirichlet(np.ones(64)).astype(np.float32)
+        own_max = np.float32(6.0) * amp
+        exact = float(np.dot(c.astype(np.float64), w.astype(np.float64)))
+        sw = pow2_scale(1.0, 8)
+        e_own = abs(tc_sum(c, w, pow2_scale(own_max, 9), sw) - exact)
+        e_glob = abs(tc_sum(c, w, pow2_scale(table_max, 9), sw) - exact)
+        assert e_own <= 2.0 ** -20 * float(np.abs(c.astype(np.float64) * w).sum()) + 1e-36
+        worst_own = max(worst_own, e_own / (2e-5 * float(own_max)))
+        worst_global = max(worst_global, e_glob / (2e-5 * float(own_max)))
+    assert worst_own <= 0.05                                 # 20 x inside the value tolerance against its own max
+    assert worst_global > 1.0                                # a table-wide scale breaks it for this orbital
 
 
 def test_one_fp16_term_is_not_enough():
