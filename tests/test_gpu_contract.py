@@ -30,18 +30,25 @@ def run_contract(torch, blip, table, pos, d, mode=1, ldd=None, want_cell=False):
     return out.cpu().numpy(), None if cell is None else cell.cpu().numpy()
 
 
-def check(A, grid, c, pos, d, out, mode=1):
+def check(A, grid, c, pos, d, out, mode=1, margin=0.05):
+    """Bound: every orbital value may be off by the tolerance, so the contraction by tol x sum_l |d_l|
+    (worst case, all errors aligned).  Rounding errors do not align: the measured error must stay
+    below `margin` = 5 % of that bound (it sits at ~0.1 % of it), so that a regression of the
+    kernel's accuracy by two orders of magnitude fails here, not only one of four."""
     oval, ograd, olap, _ = oracle.eval_fast(A, grid, c, pos, mode=mode)
     ref = oracle.contract(oval, ograd if mode == 1 else None, olap if mode == 1 else None, d)
     tv, tg, tl = tolerances(A, grid, float(np.abs(c).max()))
     w = float(np.abs(d).sum(axis=1).max())
-    assert np.abs(out[:, 0] - ref[:, 0]).max() <= tv * w
+    frac = {"val": float(np.abs(out[:, 0] - ref[:, 0]).max() / (tv * w))}
     if mode == 1:
-        assert np.abs(out[:, 1:4] - ref[:, 1:4]).max() <= tg * w
-        assert np.abs(out[:, 4] - ref[:, 4]).max() <= tl * w
+        frac["grad"] = float(np.abs(out[:, 1:4] - ref[:, 1:4]).max() / (tg * w))
+        frac["lap"] = float(np.abs(out[:, 4] - ref[:, 4]).max() / (tl * w))
         assert not out[:, 5:].any()
     else:
         assert not out[:, 1:].any()
+    print("contraction error as a fraction of the bound:", {k: round(v, 4) for k, v in frac.items()})
+    assert max(frac.values()) < margin, frac
+    return frac
 
 
 @pytest.mark.parametrize("grid,L,M,lat,path", [
@@ -94,11 +101,14 @@ def test_contract_tio2_full_size_every_output(torch_cuda, blip):
     t.close()
     tv, tg, tl = tolerances(A, cfg.grid, float(np.abs(c).max()))
     assert not out[:, 5:].any()
+    worst = 0.0
     for lo in range(0, pos.shape[0], 8192):
         hi = min(lo + 8192, pos.shape[0])
         oval, ograd, olap, _ = oracle.eval_fast(A, cfg.grid, c, pos[lo:hi])
         ref = oracle.contract_rows(oval, ograd, olap, d[lo:hi])
         w = float(np.abs(d[lo:hi]).sum(axis=1).max())
-        assert np.abs(out[lo:hi, 0] - ref[:, 0]).max() <= tv * w
-        assert np.abs(out[lo:hi, 1:4] - ref[:, 1:4]).max() <= tg * w
-        assert np.abs(out[lo:hi, 4] - ref[:, 4]).max() <= tl * w
+        worst = max(worst, float(np.abs(out[lo:hi, 0] - ref[:, 0]).max() / (tv * w)),
+                    float(np.abs(out[lo:hi, 1:4] - ref[:, 1:4]).max() / (tg * w)),
+                    float(np.abs(out[lo:hi, 4] - ref[:, 4]).max() / (tl * w)))
+    print("contraction error as a fraction of the worst-case bound, all 49,152 positions:", round(worst, 4))
+    assert worst < 0.05, worst                               # see check(): ~0.1 % expected

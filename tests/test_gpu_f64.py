@@ -84,3 +84,43 @@ def test_f64_tio2_sampled_and_fp32_path_against_it(torch_cuda, blip):
     assert np.abs(grad.cpu().numpy() - out[1]).max() <= 2e-5 * cmax / h
     assert np.abs(lap.cpu().numpy() - out[2]).max() <= 5e-5 * cmax / h ** 2
     t.close()
+
+
+def test_f64_tio2_full_size_every_output(torch_cuda, blip):
+    """All 49,152 positions x 768 orbitals of the TiO2 configuration through blipgpu_eval_f64, every
+    output against the oracle at the fp64 tolerance, in slabs of 8,192 positions (the fp64 outputs
+    of the whole batch would be 1.5 GB on each side)."""
+    cfg = workloads.CONFIGS["tio2"]
+    A = workloads.lattice(cfg)
+    c = workloads.coefficients(cfg.grid, cfg.norb)
+    pos = workloads.positions(cfg)
+    t = blip.BlipTable(A, cfg.grid, cfg.norb, c)
+    try:
+        for lo in range(0, pos.shape[0], 8192):
+            p = pos[lo:lo + 8192]
+            check(A, cfg.grid, c, p, run_f64(torch_cuda, blip, t, p, cfg.norb))
+    finally:
+        t.close()
+
+
+def test_f64_meets_the_bound_on_strongly_anisotropic_grids(torch_cuda, blip):
+    """DESIGN.md reading R13a: beyond a spacing ratio of ~10 the fp32 kernels' Laplacian rounding
+    (which scales with 1 / h_min^2) can pass north_star's bound (stated with h_max);
+    blipgpu_eval_f64 is what such tables are given.  Grid 8 x 8 x 32 on a 4.3 x 11.4 x 3.6 cell
+    (ratio 12.7) and a harsher 6 x 40 x 6 on 9 x 1.5 x 9 (ratio 40): the fp64 path meets north_star's
+    fp32 bound with h = h_max by orders of magnitude, and its own 1e-12 bound with h_min."""
+    for grid, lat, L, M in (((8, 8, 32), np.diag([4.3, 11.4, 3.6]), 130, 3000), ((6, 40, 6), np.diag([9.0, 1.5, 9.0]), 24, 500)):
+        A, c, pos = workloads.small_case(grid, L, M, lat, seed=sum(grid))
+        sp = oracle.spacing(A, grid)
+        assert sp.max() / sp.min() > 12
+        t = blip.BlipTable(A, grid, L, c)
+        try:
+            out = run_f64(torch_cuda, blip, t, pos, L)
+            check(A, grid, c, pos, out)                       # 1e-12 with h_min
+            oval, ograd, olap, _ = oracle.eval_fast(A, grid, c, pos)
+            cmax, h = float(np.abs(c).max()), float(sp.max())
+            assert np.abs(out[0] - oval).max() <= 1e-6 * 2e-5 * cmax
+            assert np.abs(out[1] - ograd).max() <= 1e-6 * 2e-5 * cmax / h
+            assert np.abs(out[2] - olap).max() <= 1e-4 * 5e-5 * cmax / h ** 2
+        finally:
+            t.close()

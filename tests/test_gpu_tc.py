@@ -366,3 +366,39 @@ def test_outputs_beyond_32_bit_element_offsets(torch_cuda, blip):
     del val, grad, lap
     compare(A, grid, c, pos[pick], gpu)
     t.close()
+
+
+def test_two_tensor_core_handles_on_two_streams_at_once(torch_cuda, blip):
+    """Every CTA of the tensor-core kernel allocates all 512 tensor-memory columns of its SM
+    (tcgen05.alloc blocks until they are free).  Two handles evaluating on two streams at the same
+    time must therefore serialise per SM, not deadlock: its 185 KB of shared memory keep a second CTA
+    off the SM until the first has exited and released its columns.  20 rounds of overlapping calls
+    (each stream's kernel is launched while the other's may still run), every result bit-identical
+    to the same call made alone."""
+    torch = torch_cuda
+    grid, L, M = (12, 12, 16), 256, 6000
+    A1, c1, p1 = workloads.small_case(grid, L, M, TRICLINIC, seed=31)
+    A2, c2, p2 = workloads.small_case(grid, L, M, ORTHO, seed=32)
+    t1, t2 = tc_table(blip, A1, grid, c1), tc_table(blip, A2, grid, c2)
+    try:
+        alone = []
+        for t, p in ((t1, p1), (t2, p2)):
+            val, grad, lap, _ = t.eval(torch.from_numpy(p).cuda(), mode=blip.VGL)
+            torch.cuda.synchronize()
+            assert blip.blipgpu_last_path(t.handle) == 5
+            alone.append((val.clone(), grad.clone(), lap.clone()))
+        s1, s2 = torch.cuda.Stream(), torch.cuda.Stream()
+        d1, d2 = torch.from_numpy(p1).cuda(), torch.from_numpy(p2).cuda()
+        outs = [[torch.empty_like(x) for x in alone[0]], [torch.empty_like(x) for x in alone[1]]]
+        torch.cuda.synchronize()
+        for _ in range(20):
+            for t, d, s, o in ((t1, d1, s1, outs[0]), (t2, d2, s2, outs[1])):
+                blip.blipgpu_eval(t.handle, d, M, blip.VGL, o[0], o[1], o[2], t.ld, None, s)
+        s1.synchronize()
+        s2.synchronize()
+        for o, a in zip(outs, alone):
+            for x, y in zip(o, a):
+                assert torch.equal(x[..., :L], y[..., :L])
+    finally:
+        t1.close()
+        t2.close()
