@@ -134,9 +134,10 @@ class ClockSampler:
 # ---------------------------------------------------------------------------------------------
 # CPU legs (the only places bench.py executes oracle/): cpu_baseline and --impl reference
 # ---------------------------------------------------------------------------------------------
-def oracle_sample(cfg, coeffs, sample_positions, mode_vgl, repeats=1):
+def oracle_sample(cfg, coeffs, sample_positions, mode_vgl, repeats=1, keep=None):
     """Times the oracle as it stands (gcc -O2, OpenMP over positions) on `sample_positions`
-    positions x all orbitals of the workload.  Returns (evals/s, seconds, threads)."""
+    positions x all orbitals of the workload.  Returns (evals/s, seconds, threads); keep (a list)
+    receives the oracle's outputs of the last repeat."""
     import oracle
     A = workloads.lattice(cfg)
     pos = workloads.positions(cfg, M=sample_positions)
@@ -145,22 +146,61 @@ def oracle_sample(cfg, coeffs, sample_positions, mode_vgl, repeats=1):
     best = None
     for _ in range(repeats):
         t0 = time.perf_counter()
-        oracle.eval_fast(A, cfg.grid, coeffs, pos, mode=mode)
+        out = oracle.eval_fast(A, cfg.grid, coeffs, pos, mode=mode)
         dt = time.perf_counter() - t0
         best = dt if best is None else min(best, dt)
+    if keep is not None:
+        keep[:] = list(out)
     return pos.shape[0] * cfg.norb / best, best, oracle.num_threads()
 
 
-def cpu_baseline(cfg, coeffs, mode_vgl):
+def cpu_baseline(cfg, coeffs, mode_vgl, gpu_outputs=None):
+    """The oracle as it stands on the box's cores: on all of them (OpenMP) and on ONE (the paper compares
+    with a single core, Table II), each on a bounded sample.  gpu_outputs
+    = (val, grad, lap) torch tensors of the timed call: the all-core sample's results are then compared
+    with the same positions of the GPU's — `parity`, the error as a fraction of north_star's tolerances,
+    taken outside every timed region."""
+    import oracle
     # bounded sample: ~10-30 s of CPU work.  Calibrate on 256 positions, then size the sample.
     rate, _, threads = oracle_sample(cfg, coeffs, min(256, cfg.M), mode_vgl)
     target_s = 4.0                                                     # wall seconds x threads ~ CPU work
     n = int(min(cfg.M, max(256, rate * target_s / cfg.norb)))
-    rate, secs, threads = oracle_sample(cfg, coeffs, n, mode_vgl)
-    return {"value": rate, "unit": UNIT, "cores": threads, "kind": "oracle",
-            "sample": f"first {n} positions x {cfg.norb} orbitals of {cfg.name}, {secs:.2f} s wall on "
-                      f"{threads} threads, fp64, gcc -O2 (oracle/blip_oracle.c, untuned)",
-            "paper_context": PAPER_CONTEXT}
+    kept = []
+    rate, secs, threads = oracle_sample(cfg, coeffs, n, mode_vgl, keep=kept)
+    out = {"value": rate, "unit": UNIT, "cores": threads, "kind": "oracle",
+           "sample": f"first {n} positions x {cfg.norb} orbitals of {cfg.name}, {secs:.2f} s wall on "
+                     f"{threads} threads, fp64, gcc -O2 (oracle/blip_oracle.c, untuned)",
+           "paper_context": PAPER_CONTEXT}
+    if gpu_outputs is not None and kept:
+        A = workloads.lattice(cfg)
+        h = float(oracle.spacing(A, cfg.grid).max())
+        cmax = float(np.abs(coeffs).max())
+        tol = (2e-5 * cmax, 2e-5 * cmax / h, 5e-5 * cmax / (h * h))
+        par = {"positions": n, "orbitals": cfg.norb,
+               "note": "max |gpu - oracle| over the sample, as a fraction of north_star's tolerance (2e-5 max|c|, 2e-5 max|c| / h, "
+                       "5e-5 max|c| / h^2); the GPU outputs are those of the timed call's last step"}
+        for name, g, o, t in zip(("val", "grad", "lap"), gpu_outputs, kept[:3], tol):
+            if g is None or o is None:
+                continue
+            err, m0 = 0.0, 0
+            while m0 < n:                                              # in slabs: the fp64 difference of the whole batch is GBs
+                m1 = min(n, m0 + 4096)
+                err = max(err, float(np.abs(g[m0:m1, ..., :cfg.norb].cpu().numpy().astype(np.float64) - o[m0:m1]).max()))
+                m0 = m1
+            par[name] = err / t
+        out["parity"] = par
+    del kept
+    # one core
+    prev = oracle.num_threads()
+    oracle.set_num_threads(1)
+    try:
+        n1 = int(min(cfg.M, max(64, rate / max(threads, 1) * target_s / cfg.norb)))
+        rate1, secs1, _ = oracle_sample(cfg, coeffs, n1, mode_vgl)
+    finally:
+        oracle.set_num_threads(prev)
+    out["single_thread"] = {"value": rate1, "unit": UNIT, "cores": 1,
+                            "sample": f"first {n1} positions x {cfg.norb} orbitals of {cfg.name}, {secs1:.2f} s wall on 1 thread"}
+    return out
 
 
 def run_reference(args):
@@ -230,6 +270,11 @@ def needs_l2_flush(cfg, args):
 # ---------------------------------------------------------------------------------------------
 KERNEL_NAMES = {1: "blip::eval_direct_kernel", 2: "blip::eval_staged_kernel", 3: "blip::eval_split_kernel",
                 5: "blip::eval_tc_kernel (tcgen05.mma, coefficient planes in tensor memory)"}
+# `dtype` of the line = the arithmetic the timed kernel computes in (not a precision claim; `parity_frac` is that)
+DTYPE_OF_PATH = {5: "f32 (tcgen05 kind::f16 MMAs on exact two-term fp16 splits of coefficients and weights, per-orbital "
+                    "power-of-two scale, fp32 accumulate; fp64 cell map)",
+                 1: "f32 (packed FP32 FMAs; fp64 cell map)", 2: "f32 (packed FP32 FMAs; fp64 cell map)",
+                 3: "f32 (packed FP32 FMAs; fp64 cell map)"}
 FMA_PER_EVAL_CONTRACT = {True: 320, False: 64}      # SURVEY.md §8d R_fp32: five weights per site x 64 sites
 
 
@@ -308,7 +353,20 @@ def roofline_block(torch, blip, handle, cfg, M, L, mode_vgl, k_ms, g_ms, n_rows,
                               "-> fp32, two-term splits of both operands) per electron and 128 orbitals, not on the FP32 pipe; "
                               "SURVEY.md §8d's binding bound max(R_compulsory, R_fp32) is kept as the yardstick (frac > 1 would "
                               "mean faster than the FP32 pipe could be at its peak)")
+    out["kernel_ms_note"] = ("kernel_ms / grouping_ms come from events the library records between the grouping launch and the "
+                             "gather + FMA launch (blipgpu_set_profiling); an event there defeats the programmatic dependent launch "
+                             "that overlaps the two in the timed steps, so kernel_ms + grouping_ms can exceed ms_per_step")
     out.update(recorded_traffic(f"{cfg.name}:{'vgl' if mode_vgl else 'value'}", comp_bytes))
+    # what physically limits the kernel that ran (the §8d figure above is a yardstick once the FMAs run on
+    # the tensor cores): compulsory HBM bytes and, from the separate ncu capture, DRAM bytes moved and pipe use
+    phys = {"hbm_compulsory_frac": out["compulsory_hbm_frac"]}
+    if out.get("traffic"):
+        phys["dram_frac"] = out["traffic"] / t / 1e9 / peak_hbm
+    pipes = out.pop("ncu_pipes", None)
+    if pipes:
+        phys.update(pipes)
+        phys["pipes_source"] = "separate ncu capture (profiles/traffic.json), not this run"
+    out["physical"] = phys
     return out
 
 
@@ -345,6 +403,8 @@ def recorded_traffic(key, comp_bytes):
         out["traffic"] = entry["dram_bytes_per_launch"]
         out["traffic_over_compulsory"] = entry["dram_bytes_per_launch"] / comp_bytes
         out["traffic_source"] = "separate ncu capture, not this run: " + str(entry.get("source"))
+        if entry.get("pipes"):
+            out["ncu_pipes"] = entry["pipes"]                  # e.g. tensor_pipe_busy, lsu_pipe_busy (fractions of elapsed cycles)
     else:
         out["traffic_stale"] = ("profiles/traffic.json has " + str(entry.get("dram_bytes_per_launch")) + " B per launch for this "
                                 "kernel, captured from other sources than the ones loaded now (" + ", ".join(entry.get("kernel_sources", []))
@@ -445,7 +505,7 @@ def measure_config(torch, blip, name, steps, fp32_meas, nsm, mode_vgl=True):
         rows = distinct_rows(torch, cells, cfg.grid)
         roof = roofline_block(torch, blip, w.handle, cfg, w.M, w.L, mode_vgl, k_ms, g_ms, rows, fp32_meas, nsm)
         keep = ("bound", "achieved", "peak", "unit", "frac", "kernel", "kernel_ms", "grouping_ms", "binding", "bound_ms",
-                "contract_frac", "compulsory_hbm_frac", "distinct_rows", "traffic", "traffic_source", "traffic_stale")
+                "contract_frac", "compulsory_hbm_frac", "distinct_rows", "traffic", "traffic_source", "traffic_stale", "physical")
         return {"workload": f"{cfg.name}: BASELINE.json configs[{list(workloads.CONFIGS).index(cfg.name)}]",
                 "positions": w.M, "orbitals": w.L, "grid": list(cfg.grid), "table_bytes": cfg.table_bytes,
                 "mode": "value+grad+lap" if mode_vgl else "value", "steps": steps, "ms_per_step": ms,
@@ -492,6 +552,7 @@ def run_gpu(args):
     barrier()
     with ClockSampler(local_rank) as clocks:
         ms_total, launches = time_steps(torch, w, args.steps, 0, flush, barrier)
+    timed_path = blip.blipgpu_last_path(handle)                       # the gather + FMA kernel the timed steps ran
     ms_total = max_over_ranks(dist, ms_total, "cuda")
     ms_step = ms_total / args.steps
     evals_step = M * L * world
@@ -509,6 +570,8 @@ def run_gpu(args):
     blip.blipgpu_eval(handle, w.dpos, M, w.mode, w.val, w.grad, w.lap, ld, cellbuf, stream)
     torch.cuda.synchronize()
     n_rows = distinct_rows(torch, cellbuf, cfg.grid)
+    m_walker = min(M, max(1, cfg.electrons))                           # batch of the f64 / Hessian calls: one walker
+    n_rows_walker = distinct_rows(torch, cellbuf[:m_walker].contiguous(), cfg.grid)
     del cellbuf
     roofline = roofline_block(torch, blip, handle, cfg, M, L, mode_vgl, k_ms, g_ms, n_rows, fp32_meas, nsm)
 
@@ -540,17 +603,29 @@ def run_gpu(args):
         line = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": max(args.warmup, 3), "ms_per_step": ms_step, "higher_is_better": True,
-            "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+            "scaling": "weak", "vs_baseline": None, "dtype": DTYPE_OF_PATH.get(timed_path, "f32"), "data": "synthetic",
             "config": workload_config(cfg, args), "positions_per_s": M * world / (ms_step * 1e-3),
             "clocks": clocks.summary(), "e2e": e2e, "gpu_launches": int(launches),
             "roofline": roofline,
         }
         if world == 1 and not args.no_cpu_baseline:
-            line["cpu_baseline"] = cpu_baseline(cfg, w.coeffs, mode_vgl)
+            line["cpu_baseline"] = cpu_baseline(cfg, w.coeffs, mode_vgl, (w.val, w.grad, w.lap) if w.M == cfg.M else None)
+            if "parity" in line["cpu_baseline"]:
+                line["parity_frac"] = line["cpu_baseline"]["parity"]
         if mode_vgl and not args.no_contract:
             line["contract"] = run_contract(torch, blip, handle, cfg, w.hpos, w.dpos, stream, args)
             line["f64"] = run_f64(torch, blip, handle, cfg, w.dpos, stream)
             line["hessian"] = run_hessian(torch, blip, handle, cfg, w.dpos, stream)
+            ev, evw = M * L, m_walker * L
+            line["contract"]["roofline"] = compact_roofline(line["contract"]["ms_per_step"], M, L, n_rows, 32.0 * M,
+                                                            4.0 * M * ld + 24.0 * M, 325, fp32_meas)
+            line["f64"]["roofline"] = compact_roofline(line["f64"]["ms_per_call"], m_walker, L, n_rows_walker, 40.0 * evw, 24.0 * m_walker,
+                                                       None, fp32_meas, "fp64 FMAs: no measured fp64 peak for this pool, HBM bounds only")
+            for name, width in (("f32", 4.0), ("f64", 8.0)):
+                if name in line["hessian"]:
+                    line["hessian"][name]["roofline"] = compact_roofline(
+                        line["hessian"][name]["ms_per_call"], m_walker, L, n_rows_walker, 10.0 * width * evw, 24.0 * m_walker,
+                        640 if name == "f32" else None, fp32_meas, "10 quantities per site: 640 FMA per evaluation")
             fp32_staged = None
             if "eval_tc_kernel" in roofline["kernel"]:                    # the FP32-pipe staged kernel on the same batch, same run
                 blip.blipgpu_set_tuning(handle, 2, 0)
@@ -566,6 +641,8 @@ def run_gpu(args):
                         "(profiles/r2_v1.md); its probe is the harness program tests/harness/mma_sync_probe.cu, no longer in the library"}
             if L % 2 == 0:
                 line["complex"] = run_complex(torch, blip, w, args)
+                line["complex"]["roofline"] = compact_roofline(line["complex"]["ms_per_step"], M, L, n_rows, 20.0 * M * L, 24.0 * M + 12.0 * L,
+                                                               320, fp32_meas, "phase epilogue (fp64 k.r, sincospi, product rule) not counted")
         if world == 1 and not args.no_configs:
             # the other BASELINE.json configs (north_star item 4): sweep on this table, then small, tiny, large
             block = {}
@@ -603,6 +680,29 @@ def run_c_harness():
         return json.loads(r.stdout.strip().splitlines()[-1])
     except Exception as exc:                                          # the benchmark line must still be printed
         return {"error": repr(exc)}
+
+
+def compact_roofline(ms, M, L, rows, out_bytes, in_bytes, fma_per_eval, fp32_meas, note=None):
+    """The roofline object of the §8(f) entry points, same rules as roofline_block: R_gather
+    (256 B per evaluation + the call's own input / output bytes) unless the call beats it by sharing rows
+    on chip, then R_compulsory (distinct rows once + the same bytes); against R_fp32 where the arithmetic
+    is fp32 (fma_per_eval None: fp64 arithmetic, no measured fp64 peak for this pool — HBM bounds only)."""
+    peak_hbm, _, _ = measured_peaks()
+    evals, t = M * L, ms * 1e-3
+    t_gather = (256.0 * evals + out_bytes + in_bytes) / (peak_hbm * 1e9)
+    t_comp = (4.0 * rows * L + out_bytes + in_bytes) / (peak_hbm * 1e9)
+    beats = t < t_gather
+    cands = {"R_compulsory" if beats else "R_gather": t_comp if beats else t_gather}
+    bound_ms = {"R_gather": 1e3 * t_gather, "R_compulsory": 1e3 * t_comp}
+    if fma_per_eval:
+        cands["R_fp32"] = 2.0 * fma_per_eval * evals / fp32_meas
+        bound_ms["R_fp32"] = 1e3 * cands["R_fp32"]
+    name = max(cands, key=cands.get)
+    out = {"bound": "alu" if name == "R_fp32" else "hbm", "binding": name, "frac": cands[name] / t, "bound_ms": bound_ms,
+           "distinct_rows": int(rows), "hbm_peak_GBps": peak_hbm}
+    if note:
+        out["note"] = note
+    return out
 
 
 def run_contract(torch, blip, handle, cfg, hpos, dpos, stream, args):
