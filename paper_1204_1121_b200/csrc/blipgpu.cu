@@ -34,7 +34,7 @@ cudaError_t launch_pdl(void (*kernel)(KArgs...), dim3 grid, dim3 block, size_t s
 // The staged kernel as shipped (blip::eval_staged_kernel template constants): 4 orbitals per
 // lane (128 per tile row), pencils of 4 x 4 cells, a ring of 8 table planes in shared memory,
 // 16 consumer warps.  The other shapes that were measured (4 x 8 pencils with a 5-plane ring;
-// 8 and 12 warps) lost and are not built (profiles/r1_v3.md).
+// 8 and 12 warps) lost and are not built (round 1; profiles/r1_v3.md, in the git history up to cef06e0).
 constexpr int kSVec = 4, kSBY = 4, kSBZ = 4, kSRing = 8, kSWarps = 16;
 constexpr int kSC = 32 * kSVec;
 using StagedShape = blip::StagedCfg<kSVec, kSBY, kSBZ, kSRing, kSWarps>;
