@@ -98,6 +98,11 @@ int blipgpu_create(const double* lattice, const int* grid, int norb, const float
  * workspace must grow the call synchronises `stream` once — blipgpu_reserve avoids that (the first
  * dense batch of a handle also builds the library's second copy of the table, the fp16 form its
  * tensor-core kernel reads; blipgpu_reserve with that batch size does it ahead of time).
+ * Which kernel a handle's dense batches run is decided once, by the first of them or by
+ * blipgpu_reserve: if the fp16 copy cannot be built at that moment (no memory, or the call is being
+ * captured in a CUDA graph, where nothing can be allocated) the handle keeps the FP32-pipe kernel
+ * for all later dense batches too, so that the same handle and inputs always return the same bits
+ * (the two kernels differ in the last bits; both meet the tolerances).
  * The call keeps no state on the host between calls and leaves its device workspace as it
  * found it, so once the workspace is reserved it may be captured in a CUDA graph and
  * replayed.
@@ -201,7 +206,8 @@ int blipgpu_eval_complex(blipgpu_table* t, const double* positions, long long M,
  * synchronises the stream once), and, if batches of M_max positions are dense enough for the
  * staged kernels, build the fp16 copy of the table the tensor-core kernel reads (as much device
  * memory again as the table).  Optional; needed before a call is captured in a CUDA graph (a
- * capture cannot allocate: a dense call captured without it runs the FP32-pipe kernel).  The device staging buffers of blipgpu_eval_host
+ * capture cannot allocate: a dense call captured without it runs the FP32-pipe kernel, and the handle
+ * then stays on that kernel).  The device staging buffers of blipgpu_eval_host
  * are sized by that call itself.  Errors: EINVAL, ENOMEM, ECUDA. */
 int blipgpu_reserve(blipgpu_table* t, long long M_max);
 

@@ -170,7 +170,8 @@ static bool build_tensor_map16(blipgpu_table* t, int nzp);
 // The fp16-pair table of the tensor-core kernel (blip_tc.cuh) and its TMA descriptor, built from the
 // padded fp32 table the first time the handle takes that path (or by blipgpu_reserve): tables that
 // never see a dense batch — the 6.3 GB one of the large config — do not pay for it.  Allocates and
-// synchronises, like a workspace growth.  On failure the handle keeps the FP32-pipe staged kernel.
+// synchronises, like a workspace growth.  On failure (out of memory, or a stream capture in progress)
+// the handle keeps the FP32-pipe staged kernel for good: tc_ok = 0.
 static bool ensure_tc_table(blipgpu_table* t, cudaStream_t s)
 {
     if (t->table16) return true;
@@ -178,7 +179,12 @@ static bool ensure_tc_table(blipgpu_table* t, cudaStream_t s)
     cudaStreamCaptureStatus cap = cudaStreamCaptureStatusNone;
     if (cudaStreamIsCapturing(s, &cap) != cudaSuccess || cap != cudaStreamCaptureStatusNone) {
         (void)cudaGetLastError();
-        return false;                                     // no allocation inside a capture: this call runs the FP32 kernel
+        // no allocation inside a capture: this call runs the FP32 kernel — and so do all later dense
+        // batches of the handle.  Which arithmetic a handle's dense batches get is decided ONCE (here, by
+        // the first of them, or ahead of time by blipgpu_reserve): the same handle and inputs return the
+        // same bits whether a call is replayed from the graph or made eagerly afterwards.
+        t->tc_ok = 0;
+        return false;
     }
     const int nzp = (t->g.np[2] + 1) / 2;
     const long long words = (long long)t->g.np[0] * t->g.np[1] * nzp * 2 * t->pitch;

@@ -308,7 +308,9 @@ def test_soak_random_batch_sizes(torch_cuda, blip, tio2):
 def test_first_dense_call_inside_a_capture_runs_the_fp32_kernel(torch_cuda, blip):
     """The fp16 copy of the table is built on the first dense call; a stream capture cannot allocate,
     so a dense call captured before that (and without blipgpu_reserve) is served by the FP32-pipe
-    staged kernel — correct results either way — and later eager calls build the copy and switch."""
+    staged kernel — correct results either way — and the handle then STAYS on that kernel: the kernel
+    of a handle's dense batches is decided once, so a later eager call returns the bits the graph
+    replay returned.  With blipgpu_reserve ahead of the capture both run the tensor-core kernel."""
     torch = torch_cuda
     grid, L = (12, 8, 8), 256
     A, c, pos = workloads.small_case(grid, L, 6000, ORTHO, seed=16)
@@ -334,9 +336,26 @@ def test_first_dense_call_inside_a_capture_runs_the_fp32_kernel(torch_cuda, blip
         s.synchronize()
     assert captured_path == 2
     compare(A, grid, c, pos, (val.cpu().numpy()[:, :L], grad.cpu().numpy()[:, :, :L], lap.cpu().numpy()[:, :L], cell.cpu().numpy()))
+    replayed = val.cpu().numpy()[:, :L].copy()
     out = run_gpu(torch_cuda, blip, A, grid, c, pos, table=t)
-    assert blip.blipgpu_last_path(t.handle) == 5
+    assert blip.blipgpu_last_path(t.handle) == 2            # decided once: still the FP32-pipe kernel
+    assert np.array_equal(out[0], replayed)                 # ... hence the same bits as the replay
     compare(A, grid, c, pos, out)
+    assert blip.lib().blipgpu_set_tuning(t.handle, 5, 0) == blip.EINVAL
+    t.close()
+    # the same with blipgpu_reserve before the capture: the tensor-core kernel, captured and eager
+    t = blip.BlipTable(A, grid, L, c)
+    blip.blipgpu_reserve(t.handle, M)
+    with torch.cuda.stream(s):
+        g = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(g, stream=s):
+            blip.blipgpu_eval(t.handle, dpos, M, blip.VGL, val, grad, lap, ld, cell, stream=s)
+        assert blip.blipgpu_last_path(t.handle) == 5
+        g.replay()
+        s.synchronize()
+    replayed = val.cpu().numpy()[:, :L].copy()
+    out = run_gpu(torch_cuda, blip, A, grid, c, pos, table=t)
+    assert blip.blipgpu_last_path(t.handle) == 5 and np.array_equal(out[0], replayed)
     t.close()
 
 
