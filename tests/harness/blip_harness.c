@@ -11,16 +11,20 @@
  *                                  line on stdout.
  *   blip_harness fullsize          the TiO2-sized launch configuration (49,152 x 768, staged kernel)
  *                                  three times through eval / eval_contract: for the checked build.
- *   blip_harness selftest          every kernel once on a small table (staged, direct, split,
- *                                  fp64, contraction; both modes): exit code 0 iff all calls
- *                                  return OK, the results are finite and the staged kernel
- *                                  returns the bits of the direct one.  This is the program the
- *                                  compute-sanitizer runs of profiles/ are taken on.
+ *   blip_harness selftest [oracle] every kernel once on a small table (staged, tensor-core staged,
+ *                                  direct, split, fp64, contraction; both modes): exit code 0 iff all
+ *                                  calls return OK, the results are finite and the staged kernel
+ *                                  returns the bits of the direct one; with the path of
+ *                                  oracle/libblip_oracle.so as second argument (loaded with dlopen,
+ *                                  never linked) also iff every kernel's val / grad / lap are within
+ *                                  north_star's tolerances of the CPU fp64 oracle.  This is the program
+ *                                  the compute-sanitizer runs of profiles/ are taken on.
  *
  * Table values and positions come from a 64-bit LCG: timing and memory safety do not depend
  * on them, and parity with the oracle is the business of tests/test_gpu_*.py, not of this file.
  */
 #include <cuda_runtime_api.h>
+#include <dlfcn.h>
 #include <math.h>
 #include <stdio.h>
 #include <stdlib.h>
@@ -61,7 +65,8 @@ static double now_s(void)
         }                                                                                \
     } while (0)
 
-static blipgpu_table* make_table(const double A[9], const int n[3], int L)
+/* keep != NULL: the caller gets (and frees) the host copy of the table */
+static blipgpu_table* make_table_keep(const double A[9], const int n[3], int L, float** keep)
 {
     const size_t count = (size_t)n[0] * n[1] * n[2] * (size_t)L;
     float* c = (float*)malloc(count * sizeof(float));
@@ -69,8 +74,41 @@ static blipgpu_table* make_table(const double A[9], const int n[3], int L)
     for (size_t i = 0; i < count; ++i) c[i] = (float)(2.0 * lcg_uniform() - 1.0);
     blipgpu_table* t = NULL;
     BLIP_OK(blipgpu_create(A, n, L, c, 0, NULL, &t));
-    free(c);
+    if (keep) *keep = c; else free(c);
     return t;
+}
+
+static blipgpu_table* make_table(const double A[9], const int n[3], int L)
+{
+    return make_table_keep(A, n, L, NULL);
+}
+
+/* The CPU fp64 oracle (oracle/libblip_oracle.so; test infrastructure, never linked into the product or
+ * into this program): `selftest <path to the library>` loads it at run time and checks every kernel's
+ * outputs against it with north_star's tolerances; the other modes of this program never touch it. */
+typedef int (*oracle_eval_fn)(const double*, const int*, int, const float*, const double*, long long, int,
+                              double*, double*, double*, int*);
+typedef int (*oracle_spacing_fn)(const double*, const int*, double*);
+
+/* largest |gpu - oracle| of a call's outputs as a fraction of its tolerance (val, grad, lap: tol[0..2]);
+ * h = [val nv | grad 3 nv | lap nv] with row pitch ld, the oracle's arrays are dense in L */
+static double oracle_fraction(const float* h, size_t nv, long long Mp, int L, long long ld, int mode,
+                              const double* oval, const double* ograd, const double* olap, const double tol[3])
+{
+    double worst = 0.0;
+    for (long long j = 0; j < Mp; ++j)
+        for (int l = 0; l < L; ++l) {
+            double f = fabs((double)h[j * ld + l] - oval[j * L + l]) / tol[0];
+            if (!(f <= worst)) worst = f;                    /* NaN counts as a failure */
+            if (mode == 0) continue;
+            for (int i = 0; i < 3; ++i) {
+                f = fabs((double)h[nv + (3 * j + i) * ld + l] - ograd[(3 * j + i) * L + l]) / tol[1];
+                if (!(f <= worst)) worst = f;
+            }
+            f = fabs((double)h[4 * nv + j * ld + l] - olap[j * L + l]) / tol[2];
+            if (!(f <= worst)) worst = f;
+        }
+    return worst;
 }
 
 static double* make_positions(const double A[9], long long M, double spread)
@@ -161,14 +199,35 @@ static int all_finite(const float* x, size_t n)
     return 1;
 }
 
-static int run_selftest(void)
+static int run_selftest(const char* oracle_lib)
 {
     const double A[9] = {20, 0, 0, 3, 19, 0, 2, 2, 24};
     const int n[3] = {17, 12, 19};
     const int L = 257;
     const long long ld = 260, M = 6000;
-    blipgpu_table* t = make_table(A, n, L);
+    float* htable = NULL;
+    blipgpu_table* t = make_table_keep(A, n, L, &htable);
     double* hpos = make_positions(A, M, 3.0);
+    double *oval = NULL, *ograd = NULL, *olap = NULL, tol[3] = {0, 0, 0};
+    if (oracle_lib) {
+        void* so = dlopen(oracle_lib, RTLD_NOW);
+        if (!so) { fprintf(stderr, "cannot load the oracle %s: %s\n", oracle_lib, dlerror()); return 2; }
+        oracle_eval_fn oeval = (oracle_eval_fn)dlsym(so, "blip_oracle_eval");
+        oracle_spacing_fn ospacing = (oracle_spacing_fn)dlsym(so, "blip_oracle_spacing");
+        if (!oeval || !ospacing) { fprintf(stderr, "oracle symbols missing\n"); return 2; }
+        oval = (double*)malloc(sizeof(double) * (size_t)M * L);
+        ograd = (double*)malloc(sizeof(double) * 3 * (size_t)M * L);
+        olap = (double*)malloc(sizeof(double) * (size_t)M * L);
+        double hs[3], cmax = 0.0;
+        if (!oval || !ograd || !olap || oeval(A, n, L, htable, hpos, M, 1, oval, ograd, olap, NULL) != 0 || ospacing(A, n, hs) != 0) {
+            fprintf(stderr, "oracle evaluation failed\n");
+            return 2;
+        }
+        const double hmax = fmax(hs[0], fmax(hs[1], hs[2]));
+        for (size_t i = 0; i < (size_t)n[0] * n[1] * n[2] * (size_t)L; ++i) cmax = fmax(cmax, fabs((double)htable[i]));
+        tol[0] = 2e-5 * cmax; tol[1] = 2e-5 * cmax / hmax; tol[2] = 5e-5 * cmax / (hmax * hmax);     /* north_star */
+    }
+    free(htable);
     double* dpos = NULL;
     float *val = NULL, *grad = NULL, *lap = NULL, *dvec = NULL, *cout = NULL;
     double *val64 = NULL, *grad64 = NULL, *lap64 = NULL;
@@ -211,7 +270,10 @@ static int run_selftest(void)
             const size_t used = (size_t)Mp * ld;
             int ok = all_finite(h, used) && (mode == 0 || (all_finite(h + nv, 3 * used) && all_finite(h + 4 * nv, used)));
             if (path == 1) ok = ok && memcmp(h_staged, h_other, sizeof(float) * (mode ? 5 : 1) * nv) == 0;
-            printf("selftest mode=%d path=%d M=%lld kernel=%d: %s\n", mode, path, Mp, blipgpu_last_path(t), ok ? "ok" : "FAIL");
+            double frac = -1.0;
+            if (oval) { frac = oracle_fraction(h, nv, Mp, L, ld, mode, oval, ograd, olap, tol); ok = ok && frac <= 1.0; }
+            printf("selftest mode=%d path=%d M=%lld kernel=%d: %s (worst error %.4f of the tolerance against the oracle)\n", mode, path, Mp,
+                   blipgpu_last_path(t), ok ? "ok" : "FAIL", frac);
             fails += !ok;
             if (path == 2) {
                 /* the tensor-core staged kernel (tuning path 5) on the same batch: finite, and close to the
@@ -221,6 +283,8 @@ static int run_selftest(void)
                 BLIP_OK(blipgpu_eval(t, dpos, Mp, mode, val, grad, lap, ld, cell, NULL));
                 CUDA_OK(cudaDeviceSynchronize());
                 CUDA_OK(cudaMemcpy(h_other, val, sizeof(float) * nv, cudaMemcpyDeviceToHost));
+                CUDA_OK(cudaMemcpy(h_other + nv, grad, sizeof(float) * 3 * nv, cudaMemcpyDeviceToHost));
+                CUDA_OK(cudaMemcpy(h_other + 4 * nv, lap, sizeof(float) * nv, cudaMemcpyDeviceToHost));
                 double worst = 0.0, scale = 0.0;
                 for (size_t i = 0; i < used; ++i) {
                     const double d = fabs((double)h_other[i] - (double)h_staged[i]);
@@ -228,8 +292,10 @@ static int run_selftest(void)
                     if (fabs((double)h_staged[i]) > scale) scale = fabs((double)h_staged[i]);
                 }
                 ok = all_finite(h_other, used) && blipgpu_last_path(t) == 5 && worst <= 1e-5 * scale;
-                printf("selftest mode=%d path=5 M=%lld kernel=%d: %s (largest |value - FP32-pipe value| %.2e of %.2e)\n", mode, Mp,
-                       blipgpu_last_path(t), ok ? "ok" : "FAIL", worst, scale);
+                double frac5 = -1.0;
+                if (oval) { frac5 = oracle_fraction(h_other, nv, Mp, L, ld, mode, oval, ograd, olap, tol); ok = ok && frac5 <= 1.0; }
+                printf("selftest mode=%d path=5 M=%lld kernel=%d: %s (worst error %.4f of the tolerance against the oracle; largest "
+                       "|value - FP32-pipe value| %.2e of %.2e)\n", mode, Mp, blipgpu_last_path(t), ok ? "ok" : "FAIL", frac5, worst, scale);
                 fails += !ok;
                 BLIP_OK(blipgpu_set_tuning(t, path, 0));
             }
@@ -245,7 +311,7 @@ static int run_selftest(void)
         CUDA_OK(cudaDeviceSynchronize());
         printf("selftest f64 mode=%d: ok\n", mode);
     }
-    free(h_staged); free(h_other); free(hpos);
+    free(h_staged); free(h_other); free(hpos); free(oval); free(ograd); free(olap);
     cudaFree(dpos); cudaFree(val); cudaFree(grad); cudaFree(lap); cudaFree(dvec); cudaFree(cout); cudaFree(cell);
     cudaFree(val64); cudaFree(grad64); cudaFree(lap64);
     BLIP_OK(blipgpu_destroy(t));
@@ -299,8 +365,8 @@ static int run_fullsize(void)
 int main(int argc, char** argv)
 {
     if (argc >= 2 && strcmp(argv[1], "latency") == 0) return run_latency(argc >= 3 ? atoi(argv[2]) : 400);
-    if (argc >= 2 && strcmp(argv[1], "selftest") == 0) return run_selftest();
+    if (argc >= 2 && strcmp(argv[1], "selftest") == 0) return run_selftest(argc >= 3 ? argv[2] : NULL);
     if (argc >= 2 && strcmp(argv[1], "fullsize") == 0) return run_fullsize();
-    fprintf(stderr, "usage: %s latency [calls] | selftest | fullsize\n", argv[0]);
+    fprintf(stderr, "usage: %s latency [calls] | selftest [path/to/libblip_oracle.so] | fullsize\n", argv[0]);
     return 64;
 }

@@ -34,7 +34,7 @@ def build(force=False, checked=False):
         return exe
     cmd = ["gcc", "-O2", "-std=c11", "-D_POSIX_C_SOURCE=200809L", "-Wall", "-Wextra", "-I", os.path.join(ROOT, "include"),
            "-I", os.path.join(CUDA, "include"), "-o", exe, SRC, "-L", libdir, "-l" + name,
-           "-L", os.path.join(CUDA, "lib64"), "-lcudart", "-lm",
+           "-L", os.path.join(CUDA, "lib64"), "-lcudart", "-lm", "-ldl",
            "-Wl,-rpath," + libdir, "-Wl,-rpath," + os.path.join(CUDA, "lib64")]
     subprocess.run(cmd, check=True)
     return exe

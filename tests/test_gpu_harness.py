@@ -21,12 +21,25 @@ def test_harness_builds_as_plain_c():
     assert r.returncode == 64 and "usage" in r.stderr
 
 
+def oracle_library():
+    """oracle/libblip_oracle.so, built if need be: handed to the self-test as an argument (it loads it
+    with dlopen; the harness is never linked against the oracle, bench.py's latency mode never sees it)."""
+    from oracle import build as oracle_build
+    return oracle_build.build()
+
+
 @pytest.mark.gpu
 def test_harness_selftest():
-    r = subprocess.run([harness_build.build(), "selftest"], capture_output=True, text=True, timeout=600)
+    """Every kernel through the plain-C caller, each checked against the CPU fp64 oracle with
+    north_star's tolerances (the tensor-core kernel too: against the oracle, not only against the
+    FP32-pipe kernel)."""
+    import re
+    r = subprocess.run([harness_build.build(), "selftest", oracle_library()], capture_output=True, text=True, timeout=600)
     assert r.returncode == 0, r.stdout + r.stderr
     assert "selftest: 0 failure(s)" in r.stdout
     assert "kernel=2" in r.stdout and "kernel=1" in r.stdout and "kernel=3" in r.stdout and "kernel=5" in r.stdout
+    fracs = [float(x) for x in re.findall(r"worst error ([0-9.]+) of the tolerance against the oracle", r.stdout)]
+    assert len(fracs) == 8 and 0.0 < max(fracs) < 0.5, r.stdout        # 4 kernels x 2 modes, a few % expected
 
 
 @pytest.mark.gpu
@@ -35,7 +48,7 @@ def test_harness_selftest_on_the_checked_build():
     slot, unit, staged plane and output index is compared with its bound inside the kernels and a
     violation traps (the stand-in for compute-sanitizer memcheck, which is closed on this pool)."""
     exe = harness_build.build(checked=True)
-    r = subprocess.run([exe, "selftest"], capture_output=True, text=True, timeout=900)
+    r = subprocess.run([exe, "selftest", oracle_library()], capture_output=True, text=True, timeout=900)
     assert r.returncode == 0, r.stdout + r.stderr
     assert "selftest: 0 failure(s)" in r.stdout and "BLIP_ASSERT" not in r.stdout + r.stderr
     r = subprocess.run([exe, "fullsize"], capture_output=True, text=True, timeout=900)
